@@ -1,0 +1,190 @@
+/*
+ * cbct.h -- C ABI of libcbct: the forward-backward-splitting (FBS) hot path of
+ * Jia et al., "GPU-based Fast Low-dose Cone Beam CT Reconstruction via Total
+ * Variation" (arxiv 1001.0599), hand-written CUDA for sm_100a (NVIDIA B200), one GPU.
+ *
+ * Citations are PAPER.md line numbers (L..) with the equation / section they fall in;
+ * "reading S.." refers to the list of readings in DESIGN.md section 4.
+ *
+ * Conventions common to every call
+ *   - Pointers named d_* are CALLER-OWNED DEVICE pointers (contiguous fp32), h_* are
+ *     caller-owned HOST pointers.  The library never frees or reallocates them.
+ *   - Volume layout  f[(k*ny + j)*nx + i]  (x fastest; z = rotation axis = superior-inferior).
+ *     Projection layout  p[(a*nv + jv)*nu + iu]  (u fastest; a = view index).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Operator calls are asynchronous on that stream; calls that fill a report
+ *     synchronise the stream before returning.
+ *   - The handle owns every scratch buffer (allocated at create; timed calls allocate
+ *     nothing).  A handle is NOT thread-safe: one call at a time per handle.
+ *   - Errors are return codes only; nothing throws or exits across the ABI.  After an
+ *     error the outputs are unspecified.  cbct_last_error() gives a thread-local message.
+ *   - Same binary + same inputs => bitwise identical outputs (no floating-point atomics,
+ *     fixed launch shapes, fixed-order fp64 reductions).
+ *   - There is no CPU fallback: without an sm_100 device create returns CBCT_ERR_UNSUPPORTED.
+ */
+#ifndef CBCT_H
+#define CBCT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cbct_geometry cbct_geometry; /* opaque */
+
+typedef enum {
+    CBCT_OK = 0,
+    CBCT_ERR_INVALID_ARG = 1, /* NULL pointer, non-positive size/pitch, bad level count ... */
+    CBCT_ERR_GEOMETRY = 2,    /* sad >= sdd, volume reaches the source or the detector plane,
+                                 a ray direction the driving-axis traversal cannot take */
+    CBCT_ERR_CUDA = 3,        /* a CUDA runtime call failed (message in cbct_last_error) */
+    CBCT_ERR_OOM = 4,         /* device allocation failed */
+    CBCT_ERR_UNSUPPORTED = 5  /* no sm_100 device */
+} cbct_status;
+
+enum { CBCT_BC_ZERO = 0, CBCT_BC_REFLECT = 1 };
+
+/* Circular cone-beam acquisition (L89-L93 Eq. 1, Fig. 1, Appendix A2, A6 L401):
+ *   view angle t:  e_n = (cos t, sin t, 0), e_u = (sin t, -cos t, 0), e_v = (0,0,1),
+ *   source S = -sad e_n, detector point P(u,v) = S + sdd e_n + u e_u + v e_v  (sdd = L0),
+ *   voxel (i,j,k) centre  x_i = (i - (nx-1)/2) hx + vol_off[0]  (same for y, z),
+ *   pixel centre          u_i = (i - (nu-1)/2) du + det_off_u   (same for v),
+ *   one ray per pixel centre.  All lengths in mm, angles in radians. */
+typedef struct {
+    int nx, ny, nz;
+    double hx, hy, hz;
+    double vol_off[3];
+    int nu, nv;
+    double du, dv, det_off_u, det_off_v;
+    double sad, sdd;
+    int n_proj;
+    const double *angles_rad; /* n_proj angles; NULL => 2*pi*a/n_proj (L251); copied at create */
+    int bc_xy, bc_z;          /* TV boundary rule: CBCT_BC_ZERO / CBCT_BC_REFLECT; the paper uses
+                                 ZERO in x,y and REFLECT in z (L161) */
+    int max_levels;           /* multi-grid levels to provision (>= 1); level l has every volume and
+                                 detector dimension divided by 2^l, so all must be divisible */
+} cbct_geometry_desc;
+
+/* Validates the description, uploads per-view tables and allocates all scratch for
+ * `max_levels` levels.  *out is NULL on failure. */
+cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out);
+void cbct_geometry_destroy(cbct_geometry *g);
+
+/* Device bytes the handle allocated (scratch + tables). */
+unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g);
+
+/* A1: d_proj = P d_vol.  (P f)[a,jv,iu] = sum over voxels of (length in mm of the segment
+ * source -> pixel centre inside the voxel) * f[voxel]: Eq. 1 (L91) on a piecewise-constant
+ * volume, the exact radiological path of "a ray-tracing algorithm, such as Siddon's"
+ * (L187, L243).  `level` selects the multi-grid level (0 = the described geometry); sizes of
+ * the buffers are the level's.  Overwrites d_proj. */
+cbct_status cbct_forward_project(const cbct_geometry *g, int level, const float *d_vol,
+                                 float *d_proj, void *cuda_stream);
+
+/* A3: d_vol = P^T d_proj with the SAME coefficients a(ray, voxel) as cbct_forward_project
+ * (exact matrix transpose; L187 "sum_theta P^T (P f - Y)").  Voxel-driven gather, no
+ * atomics, fixed summation order.  Overwrites d_vol (no accumulate). */
+cbct_status cbct_back_project(const cbct_geometry *g, int level, const float *d_proj,
+                              float *d_vol, void *cuda_stream);
+
+/* A5: Lhat = c_norm * max_v [P^T (P 1)]_v with c_norm = 2 N_vox / (N_view N_pix): an upper
+ * bound of the largest eigenvalue of the normalised data-term Hessian (reading S5).
+ * Synchronises the stream. */
+cbct_status cbct_step_bound(const cbct_geometry *g, int level, double *lhat, void *cuda_stream);
+
+/* ROF sub-solver parameters (L155-L159): smoothed TV |grad f|_delta = sqrt(|grad f|^2 + delta^2)
+ * (reading S6); at most max_inner accepted descent steps; at most max_backtracks shrinks of
+ * the trial step per descent step; Armijo constant c, shrink factor alpha, relative-decrease
+ * stop epsilon.  Paper values: c = 0.01, alpha = 0.6, epsilon = 1e-3 (L159). */
+typedef struct {
+    double eps_delta;
+    int max_inner, max_backtracks;
+    double armijo_c, shrink_alpha, rel_tol;
+} cbct_tv_params;
+
+typedef struct {
+    int inner_iters; /* accepted descent steps */
+    int trials;      /* trial energies evaluated */
+    double e_first;  /* E_ROF[g] */
+    double e_last;   /* E_ROF[returned f] */
+} cbct_tv_report;
+
+/* A6 (+A7 when nonneg != 0): d_f ~ argmin_f mean|grad f|_delta + (1/(2 w)) mean (f - g)^2
+ * (Algorithm A1 step 2, L148; E_ROF L155 with beta = 1/w), by gradient descent with the Armijo
+ * rule Eq. 5 (L157) started at f = g with initial trial step w (readings S8, S10); forward
+ * differences in physical units with the handle's boundary rules (L161).  If nonneg, the
+ * returned volume is max(f, 0) (step 3, L149).  weight_w == 0 copies g to f.
+ * d_g and d_f must not alias.  report may be NULL (then the call does not synchronise). */
+cbct_status cbct_tv_prox(const cbct_geometry *g, int level, const float *d_g, float *d_f,
+                         double weight_w, int nonneg, const cbct_tv_params *params,
+                         cbct_tv_report *report, void *cuda_stream);
+
+/* A9 helper: *e1 = mean_v |grad f|_delta.  Synchronises the stream. */
+cbct_status cbct_tv_energy(const cbct_geometry *g, int level, const float *d_f, double eps_delta,
+                           double *e1, void *cuda_stream);
+
+/* A8 grid transfers (L215-L223; readings S12, S13).  `level` is the FINE level of the pair.
+ *   restrict: fine volume -> 2x2x2 mean on level+1.   bin: fine projections -> 2x2 mean.
+ *   prolong : coarse volume (level+1) -> fine, cell-centred trilinear (3/4, 1/4); a missing
+ *             neighbour is 0 under BC_ZERO and the edge value under BC_REFLECT. */
+cbct_status cbct_restrict_volume(const cbct_geometry *g, int level, const float *d_fine,
+                                 float *d_coarse, void *cuda_stream);
+cbct_status cbct_bin_projections(const cbct_geometry *g, int level, const float *d_fine,
+                                 float *d_coarse, void *cuda_stream);
+cbct_status cbct_prolong_volume(const cbct_geometry *g, int level, const float *d_coarse,
+                                float *d_fine, void *cuda_stream);
+
+/* Algorithm A1 (L137-L151) with the multi-grid driver (L215-L223), normalised form (S5):
+ *   per level: Lhat (cbct_step_bound), tau = step / Lhat, w = tau * tv_weight;
+ *   per iteration: T = P f - y; E2 = mean T^2; g = f - tau c_norm P^T T;
+ *                  f = TVprox_w(g); f = max(f, 0) if nonneg.
+ * Levels run n_levels-1 (coarsest) ... 0; iters_per_level[] is ordered coarsest -> finest.
+ * Coarse data are 2x2-binned; the volume moves up by cbct_prolong_volume.
+ * d_vol_inout: finest-level volume; the initial guess if use_initial (restricted down to
+ * the coarsest level first), else ignored on entry; the result on return. */
+typedef struct {
+    double tv_weight; /* lambda = 1/mu of Eq. 2 (L97) */
+    double step;      /* relative gradient step in (0, 2); 1 = 1/Lhat */
+    int n_levels;     /* <= max_levels of the handle */
+    const int *iters_per_level;
+    int nonneg, use_initial;
+    cbct_tv_params tv;
+} cbct_fbs_params;
+
+typedef struct {
+    int n_iters_total;
+    double *objective;   /* caller-owned HOST array of sum(iters) doubles or NULL:
+                            objective[it] = tv_weight*E1(f) + E2(f) of the f entering iteration it */
+    double *step_abs;    /* caller-owned HOST array of n_levels doubles or NULL: tau per level */
+    int inner_total, trials_total; /* summed over all TV-prox calls */
+    float ms_total;      /* device time of the whole call (CUDA events on the stream) */
+} cbct_fbs_report;
+
+cbct_status cbct_fbs_reconstruct(const cbct_geometry *g, const float *d_proj_y, float *d_vol_inout,
+                                 const cbct_fbs_params *params, cbct_fbs_report *report,
+                                 void *cuda_stream);
+
+/* The same call on HOST buffers: copies h_proj_y to the device, reconstructs, copies the
+ * volume back (and reads h_vol_inout first if use_initial).  The handle owns the device
+ * staging buffers.  Pinned host memory makes the copies asynchronous but is not required.
+ * Synchronises the stream. */
+cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_proj_y,
+                                      float *h_vol_inout, const cbct_fbs_params *params,
+                                      cbct_fbs_report *report, void *cuda_stream);
+
+/* Kernel launches issued by this handle since create (for the bench's gpu_launches). */
+unsigned long long cbct_launch_count(const cbct_geometry *g);
+
+/* Device milliseconds per stage accumulated by cbct_fbs_reconstruct when profiling is
+ * switched on (CUDA events around every stage; adds synchronisation, so timings taken with
+ * it on are for attribution only).  Order: forward, back, tv_prox, monitor, transfers. */
+cbct_status cbct_set_stage_timing(cbct_geometry *g, int enable);
+cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[5]);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char *cbct_last_error(void);
+const char *cbct_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBCT_H */

@@ -1,0 +1,125 @@
+// cbct_internal.cuh -- shared declarations of the CUDA product path (libcbct).
+// Nothing here is used by, or uses, the CPU oracle under oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <vector>
+#include "../../include/cbct.h"
+
+// One entry per (view, detector column iu): everything about the ray fan of that column
+// that does not depend on the detector row.  Computed in fp64 on the host at create
+// (Eq. 1, L374 Eq. A2), rounded once to fp32, and read by BOTH projectors so
+// that P and P^T evaluate bit-identical ray positions.
+//
+// "Index coordinates": axis a measured in voxels from grid plane n_a/2 (integer division),
+// so voxel i spans [i - n/2, i + 1 - n/2) and grid planes sit on integers.
+// The ray is driven along x when it crosses at least as many x-planes as y-planes
+// (drive = 0: slab = x index, in-plane minor axis = y), else along y (drive = 1).
+// Along the driving coordinate D (index units):
+//     minor(D) = a0 + D * m,        |m| <= 1
+//     z(D)     = sz + v * q * (D - sd)        (v = detector row coordinate in mm)
+//     length of the ray inside one slab (mm) = L(u,v) * inv_dd,  L = sqrt(c_l + v^2)
+struct __align__(16) RayU {
+    float a0, m, inv_m, q;
+    float sd, inv_dd, c_l;
+    int drive;
+};
+
+// Per-view constants of the voxel -> detector map (Eq. A6) used by the
+// back-projector to bound the set of rays that can cross a voxel.
+struct __align__(16) ViewC {
+    float c, s;        // cos, sin of the view angle
+    float dn, du;      // half extents of a voxel along e_n and e_u (mm)
+};
+
+struct LevelParams {
+    int nx, ny, nz, nu, nv, np;
+    int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
+    float hx, hy, hz;
+    float x0, y0, z0;          // centre of voxel 0 in mm
+    float u0, du, v0, dv;      // centre of pixel 0 and pitch in mm
+    float inv_du, inv_dv;
+    float sz;                  // source z in index coordinates
+    float sad, sdd;
+    int bc_xy, bc_z;
+};
+
+struct Level {
+    LevelParams p;
+    double hx, hy, hz, du, dv;
+    size_t nvox, nray;
+    RayU *d_rayu = nullptr;     // [np][nu]
+    ViewC *d_view = nullptr;    // [np]
+    // scratch (all fp32 unless noted)
+    float *d_volT = nullptr;    // volume with x and y swapped: [k][i][j]
+    float *d_T = nullptr;       // residual scaled by L(u,v): what P^T consumes
+    float *d_g = nullptr;       // g of Algorithm A1
+    float *d_d = nullptr;       // descent direction of the ROF sub-solver
+    float *d_f2 = nullptr;      // second volume (ping-pong / level volume)
+    float *d_f = nullptr;       // level volume for levels > 0 and for the host entry point
+    float *d_y = nullptr;       // binned data for levels > 0; staging for level 0 host entry
+};
+
+struct cbct_geometry {
+    cbct_geometry_desc desc;
+    std::vector<double> angles;
+    std::vector<Level> levels;
+    double *d_partials = nullptr;   // fp64 block partials, 4 rows of partials_stride
+    int partials_stride = 0;        // >= the block count of every reducing kernel on every level
+    double *d_scalars = nullptr;    // reduced scalars on the device
+    double *h_scalars = nullptr;    // pinned host mirror
+    double *d_objective = nullptr;  // per-iteration E1, E2 pairs
+    int objective_cap = 0;
+    unsigned long long device_bytes = 0;
+    mutable unsigned long long launches = 0;
+    int stage_timing = 0;
+    mutable float stage_ms[5] = {0, 0, 0, 0, 0};
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    int sm_count = 148;
+};
+
+constexpr int kScalars = 16;
+
+// error plumbing (geometry.cu)
+cbct_status cbct_fail(cbct_status st, const char *fmt, ...);
+#define CBCT_CUDA(expr)                                                                         \
+    do {                                                                                        \
+        cudaError_t e__ = (expr);                                                               \
+        if (e__ != cudaSuccess)                                                                 \
+            return cbct_fail(e__ == cudaErrorMemoryAllocation ? CBCT_ERR_OOM : CBCT_ERR_CUDA,   \
+                             "%s: %s", #expr, cudaGetErrorString(e__));                         \
+    } while (0)
+#define CBCT_LAUNCH_CHECK(g)                                                                    \
+    do {                                                                                        \
+        (g)->launches++;                                                                        \
+        cudaError_t e__ = cudaGetLastError();                                                   \
+        if (e__ != cudaSuccess)                                                                 \
+            return cbct_fail(CBCT_ERR_CUDA, "kernel launch: %s", cudaGetErrorString(e__));      \
+    } while (0)
+
+static inline const Level *get_level(const cbct_geometry *g, int level)
+{
+    if (!g || level < 0 || level >= (int)g->levels.size()) return nullptr;
+    return &g->levels[level];
+}
+
+// internal launchers (asynchronous on `st`)
+// forward.cu : mode 0: out = P vol.  mode 1: out = L * (P vol - y), *d_sum_sq = sum (P vol - y)^2.
+//              mode 2: out = L * (P vol)
+cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
+                           float *d_out, int mode, double *d_sum_sq, cudaStream_t st);
+// back.cu : scaled != 0: d_in already holds L*T.  upd: out = f - coef * P^T in (f may be NULL: out = P^T in)
+cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
+                        const float *d_f, float coef, float *d_out, cudaStream_t st);
+// tv.cu
+cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
+                        int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,
+                        cudaStream_t st);
+cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float *d_f, double delta,
+                             double *d_out, cudaStream_t st);
+// transfer.cu
+cbct_status launch_restrict(const cbct_geometry *g, const Level &fine, const float *d_fine, float *d_coarse, cudaStream_t st);
+cbct_status launch_bin(const cbct_geometry *g, const Level &fine, const float *d_fine, float *d_coarse, cudaStream_t st);
+cbct_status launch_prolong(const cbct_geometry *g, const Level &fine, const float *d_coarse, float *d_fine, cudaStream_t st);
+cbct_status launch_max(const cbct_geometry *g, const float *d_x, size_t n, double *d_out, cudaStream_t st);
+cbct_status launch_fill(const cbct_geometry *g, float *d_x, size_t n, float val, cudaStream_t st);

@@ -1,0 +1,199 @@
+// fbs.cu -- A4/A5/A9 and the drivers: Algorithm A1 inside the
+// coarse-to-fine multi-grid loop (L215-L223), in the normalised discrete form of DESIGN.md
+// reading S5:
+//   E2 = mean_{view,pixel} (P f - y)^2,  c_norm = 2 N_vox / (N_view N_pix),
+//   step 1 (L147): g = f - tau c_norm P^T (P f - y)
+//   step 2 (L148): f = TVprox_w(g),  w = tau * tv_weight
+//   step 3 (L149): f = max(f, 0)
+//   tau = step / Lhat,  Lhat = c_norm max_v [P^T (P 1)]_v   (row-sum bound, once per level)
+// Every stage is a kernel of this library; the host only sequences launches.
+#include <math.h>
+#include "cbct_internal.cuh"
+
+namespace {
+
+struct StageTimer {
+    const cbct_geometry *g;
+    cudaStream_t st;
+    int slot;
+    bool on;
+    StageTimer(const cbct_geometry *g_, cudaStream_t st_, int slot_) : g(g_), st(st_), slot(slot_), on(g_->stage_timing != 0)
+    {
+        if (on) cudaEventRecord(g->ev[2], st);
+    }
+    ~StageTimer()
+    {
+        if (!on) return;
+        cudaEventRecord(g->ev[3], st);
+        cudaEventSynchronize(g->ev[3]);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, g->ev[2], g->ev[3]);
+        g->stage_ms[slot] += ms;
+    }
+};
+
+// Lhat of one level; leaves the result in h_scalars[9] and returns it.  Synchronises.
+cbct_status step_bound_level(const cbct_geometry *g, const Level &L, double *lhat, cudaStream_t st)
+{
+    cbct_status s;
+    if ((s = launch_fill(g, L.d_g, L.nvox, 1.0f, st)) != CBCT_OK) return s;
+    if ((s = launch_forward(g, L, L.d_g, nullptr, L.d_T, 2, nullptr, st)) != CBCT_OK) return s;   // L * (P 1)
+    if ((s = launch_back(g, L, L.d_T, 1, nullptr, 0.0f, L.d_d, st)) != CBCT_OK) return s;
+    if ((s = launch_max(g, L.d_d, L.nvox, g->d_scalars + 9, st)) != CBCT_OK) return s;
+    CBCT_CUDA(cudaMemcpyAsync(g->h_scalars + 9, g->d_scalars + 9, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    const double c_norm = 2.0 * (double)L.nvox / (double)L.nray;
+    *lhat = c_norm * g->h_scalars[9];
+    return CBCT_OK;
+}
+
+cbct_status check_params(const cbct_geometry *g, const cbct_fbs_params *p)
+{
+    if (!g || !p) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: NULL handle or params");
+    if (p->n_levels < 1 || p->n_levels > (int)g->levels.size())
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: n_levels = %d but the handle provisions %d",
+                         p->n_levels, (int)g->levels.size());
+    if (!p->iters_per_level) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: iters_per_level is NULL");
+    long total = 0;
+    for (int l = 0; l < p->n_levels; ++l) {
+        if (p->iters_per_level[l] < 0) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: negative iteration count");
+        total += p->iters_per_level[l];
+    }
+    if (total > g->objective_cap)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: more than %d iterations in one call", g->objective_cap);
+    if (!(p->tv_weight >= 0.0) || !(p->step > 0.0 && p->step < 2.0))
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: need tv_weight >= 0 and 0 < step < 2");
+    if (p->tv.max_inner < 0 || p->tv.max_backtracks < 0 || !(p->tv.shrink_alpha > 0.0 && p->tv.shrink_alpha < 1.0))
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: bad TV parameters");
+    return CBCT_OK;
+}
+
+// The whole reconstruction on device buffers (level-0 sized d_y, d_vol).
+cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, const cbct_fbs_params *p,
+                       cbct_fbs_report *rep, cudaStream_t st)
+{
+    cbct_status s;
+    const int nl = p->n_levels;
+    const bool want_obj = rep && rep->objective;
+    CBCT_CUDA(cudaEventRecord(g->ev[0], st));
+
+    // data pyramid: y_l = 2x2 mean of y_{l-1}  (S12)
+    {
+        StageTimer t(g, st, 4);
+        for (int l = 1; l < nl; ++l) {
+            const float *src = (l == 1) ? d_y : g->levels[l - 1].d_y;
+            if ((s = launch_bin(g, g->levels[l - 1], src, g->levels[l].d_y, st)) != CBCT_OK) return s;
+        }
+        // initial volume on the coarsest level
+        if (p->use_initial) {
+            for (int l = 1; l < nl; ++l) {
+                const float *src = (l == 1) ? d_vol : g->levels[l - 1].d_f;
+                if ((s = launch_restrict(g, g->levels[l - 1], src, g->levels[l].d_f, st)) != CBCT_OK) return s;
+            }
+        } else {
+            float *dst = (nl == 1) ? d_vol : g->levels[nl - 1].d_f;
+            if ((s = launch_fill(g, dst, g->levels[nl - 1].nvox, 0.0f, st)) != CBCT_OK) return s;
+        }
+    }
+
+    int done = 0, inner_total = 0, trials_total = 0;
+    for (int l = nl - 1; l >= 0; --l) {
+        const Level &L = g->levels[l];
+        float *f = (l == 0) ? d_vol : L.d_f;
+        const float *y = (l == 0) ? d_y : L.d_y;
+        const int n_it = p->iters_per_level[nl - 1 - l];
+        double lhat = 0.0;
+        {
+            StageTimer t(g, st, 3);
+            if ((s = step_bound_level(g, L, &lhat, st)) != CBCT_OK) return s;
+        }
+        if (!(lhat > 0.0)) return cbct_fail(CBCT_ERR_GEOMETRY, "level %d: no ray crosses the volume (Lhat = %g)", l, lhat);
+        const double c_norm = 2.0 * (double)L.nvox / (double)L.nray;
+        const double tau = p->step / lhat, w = tau * p->tv_weight;
+        if (rep && rep->step_abs) rep->step_abs[nl - 1 - l] = tau;
+        for (int it = 0; it < n_it; ++it, ++done) {
+            {
+                StageTimer t(g, st, 0);
+                if ((s = launch_forward(g, L, f, y, L.d_T, 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
+            }
+            if (want_obj) {
+                StageTimer t(g, st, 3);
+                if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, g->d_objective + 2 * done, st)) != CBCT_OK) return s;
+            }
+            {
+                StageTimer t(g, st, 1);
+                if ((s = launch_back(g, L, L.d_T, 1, f, (float)(tau * c_norm), L.d_g, st)) != CBCT_OK) return s;
+            }
+            {
+                StageTimer t(g, st, 2);
+                cbct_tv_report tr;
+                if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st)) != CBCT_OK) return s;
+                inner_total += tr.inner_iters;
+                trials_total += tr.trials;
+            }
+        }
+        if (l > 0) {
+            StageTimer t(g, st, 4);
+            float *fine = (l == 1) ? d_vol : g->levels[l - 1].d_f;
+            if ((s = launch_prolong(g, g->levels[l - 1], L.d_f, fine, st)) != CBCT_OK) return s;
+        }
+    }
+    CBCT_CUDA(cudaEventRecord(g->ev[1], st));
+    if (rep) {
+        rep->n_iters_total = done;
+        rep->inner_total = inner_total;
+        rep->trials_total = trials_total;
+        CBCT_CUDA(cudaEventSynchronize(g->ev[1]));
+        CBCT_CUDA(cudaEventElapsedTime(&rep->ms_total, g->ev[0], g->ev[1]));
+        if (want_obj && done > 0) {
+            std::vector<double> h(2 * (size_t)done);
+            CBCT_CUDA(cudaMemcpyAsync(h.data(), g->d_objective, sizeof(double) * 2 * done, cudaMemcpyDeviceToHost, st));
+            CBCT_CUDA(cudaStreamSynchronize(st));
+            int idx = 0;
+            for (int l = nl - 1; l >= 0; --l) {
+                const Level &L = g->levels[l];
+                for (int it = 0; it < p->iters_per_level[nl - 1 - l]; ++it, ++idx)
+                    rep->objective[idx] = p->tv_weight * h[2 * idx] / (double)L.nvox + h[2 * idx + 1] / (double)L.nray;
+            }
+        }
+    }
+    return CBCT_OK;
+}
+
+}  // namespace
+
+extern "C" cbct_status cbct_step_bound(const cbct_geometry *g, int level, double *lhat, void *cuda_stream)
+{
+    const Level *L = get_level(g, level);
+    if (!L || !lhat) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_step_bound: bad handle, level or NULL");
+    return step_bound_level(g, *L, lhat, (cudaStream_t)cuda_stream);
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *g, const float *d_proj_y, float *d_vol_inout,
+                                            const cbct_fbs_params *params, cbct_fbs_report *report,
+                                            void *cuda_stream)
+{
+    cbct_status s = check_params(g, params);
+    if (s != CBCT_OK) return s;
+    if (!d_proj_y || !d_vol_inout) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: NULL buffer");
+    return fbs_device(g, d_proj_y, d_vol_inout, params, report, (cudaStream_t)cuda_stream);
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_proj_y,
+                                                 float *h_vol_inout, const cbct_fbs_params *params,
+                                                 cbct_fbs_report *report, void *cuda_stream)
+{
+    cbct_status s = check_params(g, params);
+    if (s != CBCT_OK) return s;
+    if (!h_proj_y || !h_vol_inout) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct_host: NULL buffer");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const Level &L0 = g->levels[0];
+    CBCT_CUDA(cudaMemcpyAsync(L0.d_y, h_proj_y, L0.nray * sizeof(float), cudaMemcpyHostToDevice, st));
+    if (params->use_initial)
+        CBCT_CUDA(cudaMemcpyAsync(L0.d_f, h_vol_inout, L0.nvox * sizeof(float), cudaMemcpyHostToDevice, st));
+    s = fbs_device(g, L0.d_y, L0.d_f, params, report, st);
+    if (s != CBCT_OK) return s;
+    CBCT_CUDA(cudaMemcpyAsync(h_vol_inout, L0.d_f, L0.nvox * sizeof(float), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
