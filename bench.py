@@ -1,0 +1,377 @@
+#!/usr/bin/env python
+"""bench.py -- FBS iterations/s of the CUDA path on BASELINE.json's metric configuration.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config3]
+
+One "step" = one pass of the whole hot path (SURVEY.md section 8(a) rows A1-A7, A9's E2): one
+finest-level forward-backward-splitting iteration -- forward projection + residual + E2,
+exact-transpose back-projection + gradient step, TV-prox (Armijo gradient descent), clip -- on
+config 3 of BASELINE.json (256^3 volume, 40 views of 512x384; synthetic torso phantom, Poisson
+noise), started from the volume the two coarser multi-grid levels hand to the finest one.
+The multi-grid driver (A8) is timed as the full reconstruction ("recon_seconds").
+
+Prints ONE JSON line (rank 0).  Under torchrun every rank reconstructs its own independent problem
+(same geometry, own noise seed): no data-path collective, "scaling": "weak".
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same
+workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1001_0599_b200 import inputs as I  # noqa: E402
+
+METRIC = "fbs_iterations_per_second"
+UNIT = "iter/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.lines, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+            self.thread.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.lines:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def workload(name: str):
+    k = {"config1": 1, "config2": 2, "config3": 3, "config4": 4}[name]
+    cfg = I.config(k)
+    return k, cfg
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of our arm; the whole of --impl reference)
+# ---------------------------------------------------------------------------------------------
+
+def oracle_sample(cfg, y, views: int, z_div: int):
+    """The oracle's cost of one finest-level FBS iteration, from a bounded sample at FULL resolution:
+    P and P^T on `views` of the workload's views (their cost is a sum over views, so the full
+    operator is n_proj/views times the sample) and one TV-prox call on a slab of nz/z_div slices
+    of g = f - tau c_norm P^T(P f - y) built from those views (full call = z_div times the slab)."""
+    from oracle import cbct_oracle as orc
+    orc.build()
+    g = cfg.geom
+    sel = (np.arange(views) * g.n_proj // views + g.n_proj // (2 * views)) % g.n_proj
+    gs = g.replace(n_proj=views, angles=g.angles_rad()[sel])
+    f = I.paint(cfg.ellipsoids, g).astype(np.float64) * 0.9
+    t0 = time.perf_counter()
+    T = orc.forward(gs, f) - y[sel]
+    t1 = time.perf_counter()
+    b = orc.back(gs, T)
+    t2 = time.perf_counter()
+    c_norm = 2.0 * f.size / T.size
+    tau = cfg.fbs.step / (c_norm * 2.0e5 * views / g.n_proj)      # order of magnitude of 1/Lhat; timing only
+    nzs = max(4, g.nz // z_div)
+    k0 = (g.nz - nzs) // 2
+    gz = g.replace(nz=nzs)
+    gg = (f - tau * c_norm * b)[k0:k0 + nzs]
+    t3 = time.perf_counter()
+    _, rep = orc.tv_prox(gz, gg, tau * cfg.fbs.tv_weight, cfg.fbs)
+    t4 = time.perf_counter()
+    sec_full = (t1 - t0) * g.n_proj / views + (t2 - t1) * g.n_proj / views + (t4 - t3) * g.nz / nzs
+    return {"seconds_full_iteration": sec_full, "sample_seconds": t4 - t0 - (t3 - t2), "threads": orc.threads(),
+            "parts_s": {"P": (t1 - t0) * g.n_proj / views, "PT": (t2 - t1) * g.n_proj / views,
+                        "tv_prox": (t4 - t3) * g.nz / nzs, "tv_inner": rep.inner_iters},
+            "sample": f"oracle P and P^T on {views} of {g.n_proj} views at full resolution ({g.nx}x{g.ny}x{g.nz}, "
+                      f"{g.nu}x{g.nv}) scaled x{g.n_proj / views:.0f}, plus one oracle TV-prox call on a "
+                      f"{nzs}-slice slab scaled x{g.nz / nzs:.0f}; sum = one finest-level FBS iteration"}
+
+
+def cpu_baseline(cfg, y, budget: str = "default"):
+    views, z_div = (2, 4) if budget == "default" else (1, 16)
+    r = oracle_sample(cfg, y, views, z_div)
+    return {"value": 1.0 / r["seconds_full_iteration"], "unit": UNIT, "cores": r["threads"], "kind": "oracle",
+            "sample": r["sample"], "sample_seconds": round(r["sample_seconds"], 3),
+            "full_iteration_seconds_by_part": {k: round(v, 3) for k, v in r["parts_s"].items()},
+            "extrapolated": True}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    k, cfg = workload(args.workload)
+    y = I.make_projections(cfg)
+    times = []
+    base = None
+    for i in range(args.warmup + args.steps):
+        base = cpu_baseline(cfg, y, "small")
+        if i >= args.warmup:
+            times.append(1.0 / base["value"])
+    sec = float(np.mean(times))
+    g = cfg.geom
+    line = {"impl": "reference", "metric": METRIC, "value": 1.0 / sec, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config{k}: {g.nx}x{g.ny}x{g.nz} voxels, {g.n_proj} views of {g.nu}x{g.nv}, "
+                                   "one finest-level FBS iteration (scaled up from a bounded full-resolution sample)"},
+            "cpu_baseline": {"value": 1.0 / sec, "unit": UNIT, "kind": "oracle", "cores": base["cores"],
+                             "sample": base["sample"]},
+            "e2e": {"value": 1.0 / sec, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1001_0599_b200 import cbct
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_peak, sm_max_mhz, peak_src = _peaks()
+
+    k, cfg = workload(args.workload)
+    g = cfg.geom
+    cfg.seed += 1000 * rank                       # every rank: same phantom, own noise realisation
+    y_host = I.make_projections(cfg)
+    n_levels = len(cfg.fbs.iters_per_level)
+    fbs = cfg.fbs
+    stream = torch.cuda.Stream()
+    nvox, nray = int(np.prod(g.vol_shape)), int(np.prod(g.proj_shape))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms: float) -> float:
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    with torch.cuda.stream(stream), cbct.geometry_create(g, max_levels=n_levels) as h:
+        y = torch.from_numpy(y_host).cuda()
+        f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+        one = I.FbsSetup(**{**fbs.__dict__, "iters_per_level": (1,)})
+
+        # the volume the coarser levels hand to the finest level (untimed set-up)
+        if n_levels > 1:
+            pre = I.FbsSetup(**{**fbs.__dict__, "iters_per_level": tuple(fbs.iters_per_level[:-1]) + (0,)})
+            h.fbs_reconstruct(y, f, pre, objective=False)
+        S = h.count_samples()
+        h.step_bound()
+        f_start = f.clone()
+
+        def step_device():
+            return h.fbs_reconstruct(y, f, one, use_initial=True, objective=False, stream=stream)
+
+        for _ in range(args.warmup):
+            step_device()
+        # ---- timed region: K device-resident steps ------------------------------------------
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = h.launch_count
+        inner = trials = 0
+        barrier()
+        with ClockSampler(local) as clk:
+            ev0.record(stream)
+            for _ in range(args.steps):
+                r = step_device()
+                inner += r.inner_total
+                trials += r.trials_total
+            ev1.record(stream)
+            barrier()
+        ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+        launches = h.launch_count - l0
+        clocks = clk.summary()
+
+        # ---- e2e: the same step through the HOST entry point, copies inside the timed region -
+        y_pin = torch.from_numpy(y_host).pin_memory()
+        f_pin = f.cpu().pin_memory()
+        for _ in range(max(1, min(args.warmup, 2))):
+            h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
+        barrier()
+        ev0.record(stream)
+        for _ in range(args.steps):
+            h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
+        ev1.record(stream)
+        barrier()
+        ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
+
+        # ---- per-kernel attribution (CUDA events on the library's stream, synchronising) ----
+        f.copy_(f_start)
+        h.set_stage_timing(True)
+        for _ in range(args.steps):
+            step_device()
+        stages = h.stage_ms()
+        h.set_stage_timing(False)
+
+        # ---- whole reconstruction: all levels, all iterations (rank 0 reports) ---------------
+        recon = None
+        if not args.no_recon:
+            f.zero_()
+            barrier()
+            rr = h.fbs_reconstruct(y, f, fbs, objective=False, stream=stream)
+            t0 = time.perf_counter()
+            vol_host = np.zeros(g.vol_shape, dtype=np.float32)
+            hr = h.fbs_reconstruct_host(y_host, vol_host, fbs, stream=stream)
+            wall = time.perf_counter() - t0
+            truth = I.paint(cfg.ellipsoids, g)
+            recon = {"recon_seconds": rr.ms_total / 1e3, "recon_seconds_host_buffers_wall": wall,
+                     "iterations": int(rr.n_iters_total), "levels": n_levels,
+                     "tv_inner_total": int(rr.inner_total), "tv_trials_total": int(rr.trials_total),
+                     "rel_error_vs_phantom": float(np.linalg.norm(vol_host - truth) / np.linalg.norm(truth))}
+            del hr
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    K = args.steps
+    sec_step = ms_total / 1e3 / K
+    per = {name: {"ms_per_step": ms / K, "launches_per_step": c / K, "ms_per_launch": (ms / c if c else None)}
+           for name, (ms, c) in stages.items()}
+    # kernel rooflines: P and P^T are ALU/gather bound -- reported as GUPS and as the
+    # fraction of the fp32 issue peak their algorithmic flops reach; the TV passes are HBM bound.
+    fp32_peak = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12            # TFLOP/s, FMA = 2
+    FLOP_FWD, FLOP_BACK = 36.0, 52.0                              # algorithmic flops per ray-voxel sample
+    kern = {}
+    if per["forward"]["ms_per_launch"]:
+        t = per["forward"]["ms_per_launch"] / 1e3
+        kern["forward"] = {"bound": "alu", "gups": S / t / 1e9, "achieved": S * FLOP_FWD / t / 1e12, "peak": fp32_peak,
+                           "unit": "TFLOP/s", "frac": S * FLOP_FWD / t / 1e12 / fp32_peak}
+    if per["back"]["ms_per_launch"]:
+        t = per["back"]["ms_per_launch"] / 1e3
+        kern["back"] = {"bound": "alu", "gups": S / t / 1e9, "achieved": S * FLOP_BACK / t / 1e12, "peak": fp32_peak,
+                        "unit": "TFLOP/s", "frac": S * FLOP_BACK / t / 1e12 / fp32_peak}
+    for name, bpv in (("tv_grad", 12.0), ("tv_trial", 12.0), ("tv_update", 12.0)):
+        if per[name]["ms_per_launch"]:
+            t = per[name]["ms_per_launch"] / 1e3
+            kern[name] = {"bound": "hbm", "achieved": bpv * nvox / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                          "frac": bpv * nvox / t / 1e9 / hbm_peak}
+    dominant = max((n for n in kern), key=lambda n: per[n]["ms_per_step"])
+    roof = dict(kern[dominant])
+    roof.update({"kernel": dominant, "traffic": None, "peak_source": peak_src,
+                 "share_of_step": per[dominant]["ms_per_step"] / sum(v["ms_per_step"] for v in per.values())})
+
+    base = cpu_baseline(cfg, y_host)
+    line = {
+        "metric": METRIC, "value": world * K / (ms_total / 1e3), "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": args.warmup, "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"config{k} ({cfg.name}): {g.nx}x{g.ny}x{g.nz} fp32 voxels at {g.hx} mm, {g.n_proj} views "
+                               f"of {g.nu}x{g.nv} at {g.du} mm, one finest-level FBS iteration per step after "
+                               f"{n_levels - 1} coarser multi-grid levels",
+                   "tv_weight": fbs.tv_weight, "step": fbs.step, "levels": n_levels,
+                   "iters_per_level": list(fbs.iters_per_level),
+                   "l2": "working set (5 volumes + 2 projection stacks = %.0f MiB) exceeds the 126 MB L2; no flush"
+                         % ((5 * nvox + 2 * nray) * 4 / 2 ** 20),
+                   "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
+        "clocks": clocks,
+        "e2e": {"value": world * K / (ms_e2e / 1e3), "unit": UNIT, "h2d_bytes_per_step": 4 * (nray + nvox),
+                "d2h_bytes_per_step": 4 * nvox, "ms_per_step": ms_e2e / K},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "kernels": kern,
+        "stage_ms_per_step": {n: round(v["ms_per_step"], 4) for n, v in per.items()},
+        "projector_gups": {"samples_per_projection": int(S),
+                           "forward": kern.get("forward", {}).get("gups"), "back": kern.get("back", {}).get("gups")},
+        "tv_inner_per_step": inner / K, "tv_trials_per_step": trials / K,
+        "cpu_baseline": base,
+    }
+    if recon:
+        line["reconstruction"] = recon
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--no-recon", action="store_true", help="skip the whole-reconstruction timing")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

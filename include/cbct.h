@@ -86,9 +86,15 @@ cbct_status cbct_forward_project(const cbct_geometry *g, int level, const float 
 cbct_status cbct_back_project(const cbct_geometry *g, int level, const float *d_proj,
                               float *d_vol, void *cuda_stream);
 
+/* S = number of (ray, voxel) pairs with a(ray, voxel) > 0 at `level`: the "ray-voxel samples" one
+ * forward (or back) projection processes -- the unit of the GUPS metric.  Synchronises the stream. */
+cbct_status cbct_count_samples(const cbct_geometry *g, int level, unsigned long long *count,
+                               void *cuda_stream);
+
 /* A5: Lhat = c_norm * max_v [P^T (P 1)]_v with c_norm = 2 N_vox / (N_view N_pix): an upper
- * bound of the largest eigenvalue of the normalised data-term Hessian (reading S5).
- * Synchronises the stream. */
+ * bound of the largest eigenvalue of the normalised data-term Hessian (reading S5).  It depends on
+ * the geometry only: the first call per level evaluates it (one P, one P^T, one max-reduction;
+ * synchronises the stream), later calls and cbct_fbs_reconstruct reuse the stored value. */
 cbct_status cbct_step_bound(const cbct_geometry *g, int level, double *lhat, void *cuda_stream);
 
 /* ROF sub-solver parameters (L155-L159): smoothed TV |grad f|_delta = sqrt(|grad f|^2 + delta^2)
@@ -174,11 +180,18 @@ cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_pro
 /* Kernel launches issued by this handle since create (for the bench's gpu_launches). */
 unsigned long long cbct_launch_count(const cbct_geometry *g);
 
-/* Device milliseconds per stage accumulated by cbct_fbs_reconstruct when profiling is
- * switched on (CUDA events around every stage; adds synchronisation, so timings taken with
- * it on are for attribution only).  Order: forward, back, tv_prox, monitor, transfers. */
+/* Per-kernel attribution.  When switched on, every launch of the kernels below is bracketed by
+ * CUDA events on the library's stream and its device time accumulated (this adds one
+ * synchronisation per launch, so timings of whole calls taken with it on are for attribution only).
+ * Slots: 0 volume transpose (forward projector's x<->y copy), 1 forward projector kernel,
+ * 2 back-projector kernel, 3 TV gradient pass, 4 TV trial-energy pass, 5 TV update / clip pass,
+ * 6 reduction finalisers + objective monitor, 7 grid transfers, fills, max.
+ * cbct_get_stage_ms returns the accumulated milliseconds and launch-group counts since the last
+ * cbct_set_stage_timing call. */
+#define CBCT_N_STAGES 8
 cbct_status cbct_set_stage_timing(cbct_geometry *g, int enable);
-cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[5]);
+cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[CBCT_N_STAGES],
+                              unsigned long long out_calls[CBCT_N_STAGES]);
 
 /* Thread-local message of the last failing call on this thread ("" if none). */
 const char *cbct_last_error(void);

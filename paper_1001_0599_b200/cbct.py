@@ -28,7 +28,7 @@ STATUS_NAMES = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_GEOMETRY",
 # every symbol include/cbct.h declares
 EXPORTS = [
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_device_bytes",
-    "cbct_forward_project", "cbct_back_project", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
+    "cbct_forward_project", "cbct_back_project", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
     "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_last_error", "cbct_version",
@@ -114,6 +114,7 @@ def load_library():
     lib.cbct_geometry_device_bytes.restype = C.c_ulonglong
     lib.cbct_forward_project.argtypes = [vp, ip, vp, vp, vp]
     lib.cbct_back_project.argtypes = [vp, ip, vp, vp, vp]
+    lib.cbct_count_samples.argtypes = [vp, ip, C.POINTER(C.c_ulonglong), vp]
     lib.cbct_step_bound.argtypes = [vp, ip, C.POINTER(dp), vp]
     lib.cbct_tv_prox.argtypes = [vp, ip, vp, vp, dp, ip, C.POINTER(_TvParams), C.POINTER(_TvReport), vp]
     lib.cbct_tv_energy.argtypes = [vp, ip, vp, dp, C.POINTER(dp), vp]
@@ -125,7 +126,7 @@ def load_library():
     lib.cbct_launch_count.argtypes = [vp]
     lib.cbct_launch_count.restype = C.c_ulonglong
     lib.cbct_set_stage_timing.argtypes = [vp, ip]
-    lib.cbct_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    lib.cbct_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_ulonglong)]
     lib.cbct_last_error.restype = C.c_char_p
     lib.cbct_version.restype = C.c_char_p
     for name in EXPORTS:
@@ -233,6 +234,11 @@ class Geometry:
                                                 _dev(vol, self._nvox(level), "vol"), _stream_ptr(stream)))
         return vol
 
+    def count_samples(self, level: int = 0, stream=None) -> int:
+        out = C.c_ulonglong()
+        _check(load_library().cbct_count_samples(self._h, level, C.byref(out), _stream_ptr(stream)))
+        return int(out.value)
+
     def step_bound(self, level: int = 0, stream=None) -> float:
         out = C.c_double()
         _check(load_library().cbct_step_bound(self._h, level, C.byref(out), _stream_ptr(stream)))
@@ -319,10 +325,14 @@ class Geometry:
     def set_stage_timing(self, enable: bool):
         _check(load_library().cbct_set_stage_timing(self._h, int(bool(enable))))
 
+    STAGES = ("transpose", "forward", "back", "tv_grad", "tv_trial", "tv_update", "reduce", "transfer")
+
     def stage_ms(self):
-        out = (C.c_float * 5)()
-        _check(load_library().cbct_get_stage_ms(self._h, out))
-        return dict(zip(("forward", "back", "tv_prox", "monitor", "transfers"), [float(x) for x in out]))
+        """{stage: (milliseconds, launch groups)} accumulated since set_stage_timing."""
+        ms = (C.c_float * len(self.STAGES))()
+        calls = (C.c_ulonglong * len(self.STAGES))()
+        _check(load_library().cbct_get_stage_ms(self._h, ms, calls))
+        return {k: (float(m), int(c)) for k, m, c in zip(self.STAGES, ms, calls)}
 
 
 def geometry_create(desc, max_levels: int = 1) -> Geometry:

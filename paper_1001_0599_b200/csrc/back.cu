@@ -90,6 +90,7 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
     const LevelParams &P = L.p;
     const float *src = d_in;
     if (!scaled) {
+        StageTimer t(g, st, ST_TRANSFER);
         dim3 b(128), gr((P.nu + 127) / 128, P.nv, P.np);
         scale_by_L_kernel<<<gr, b, 0, st>>>(P, L.d_rayu, d_in, L.d_T);
         CBCT_LAUNCH_CHECK(g);
@@ -97,6 +98,7 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
     }
     dim3 b(BK_BX, BK_BY, BK_BZ);
     dim3 gr((P.nx + BK_BX - 1) / BK_BX, (P.ny + BK_BY - 1) / BK_BY, (P.nz + BK_BZ - 1) / BK_BZ);
+    StageTimer t(g, st, ST_BACK);
     back_kernel<<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;

@@ -58,6 +58,7 @@ struct Level {
     float *d_f2 = nullptr;      // second volume (ping-pong / level volume)
     float *d_f = nullptr;       // level volume for levels > 0 and for the host entry point
     float *d_y = nullptr;       // binned data for levels > 0; staging for level 0 host entry
+    mutable double lhat = -1.0; // A5 step bound: a property of the geometry alone, computed on first use
 };
 
 struct cbct_geometry {
@@ -73,12 +74,38 @@ struct cbct_geometry {
     unsigned long long device_bytes = 0;
     mutable unsigned long long launches = 0;
     int stage_timing = 0;
-    mutable float stage_ms[5] = {0, 0, 0, 0, 0};
+    mutable float stage_ms[CBCT_N_STAGES] = {0};
+    mutable unsigned long long stage_calls[CBCT_N_STAGES] = {0};
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     int sm_count = 148;
 };
 
 constexpr int kScalars = 16;
+
+// Attribution of device time to one kernel (or a short fixed group): CUDA events around the
+// launches on the library's stream, only when cbct_set_stage_timing switched it on (it adds a
+// synchronisation per stage, so whole-call timings are taken with it off).
+enum { ST_TRANSPOSE = 0, ST_FORWARD, ST_BACK, ST_TV_GRAD, ST_TV_TRIAL, ST_TV_UPDATE, ST_REDUCE, ST_TRANSFER };
+struct StageTimer {
+    const cbct_geometry *g;
+    cudaStream_t st;
+    int slot;
+    bool on;
+    StageTimer(const cbct_geometry *g_, cudaStream_t st_, int slot_) : g(g_), st(st_), slot(slot_), on(g_->stage_timing != 0)
+    {
+        if (on) cudaEventRecord(g->ev[2], st);
+    }
+    ~StageTimer()
+    {
+        if (!on) return;
+        cudaEventRecord(g->ev[3], st);
+        cudaEventSynchronize(g->ev[3]);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, g->ev[2], g->ev[3]);
+        g->stage_ms[slot] += ms;
+        g->stage_calls[slot] += 1;
+    }
+};
 
 // error plumbing (geometry.cu)
 cbct_status cbct_fail(cbct_status st, const char *fmt, ...);
@@ -105,7 +132,7 @@ static inline const Level *get_level(const cbct_geometry *g, int level)
 
 // internal launchers (asynchronous on `st`)
 // forward.cu : mode 0: out = P vol.  mode 1: out = L * (P vol - y), *d_sum_sq = sum (P vol - y)^2.
-//              mode 2: out = L * (P vol)
+//              mode 2: out = L * (P vol).  mode 3: *d_sum_sq = number of (ray, voxel) pairs, no volume read
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
                            float *d_out, int mode, double *d_sum_sq, cudaStream_t st);
 // back.cu : scaled != 0: d_in already holds L*T.  upd: out = f - coef * P^T in (f may be NULL: out = P^T in)

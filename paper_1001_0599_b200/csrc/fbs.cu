@@ -12,30 +12,11 @@
 
 namespace {
 
-struct StageTimer {
-    const cbct_geometry *g;
-    cudaStream_t st;
-    int slot;
-    bool on;
-    StageTimer(const cbct_geometry *g_, cudaStream_t st_, int slot_) : g(g_), st(st_), slot(slot_), on(g_->stage_timing != 0)
-    {
-        if (on) cudaEventRecord(g->ev[2], st);
-    }
-    ~StageTimer()
-    {
-        if (!on) return;
-        cudaEventRecord(g->ev[3], st);
-        cudaEventSynchronize(g->ev[3]);
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, g->ev[2], g->ev[3]);
-        g->stage_ms[slot] += ms;
-    }
-};
-
-// Lhat of one level; leaves the result in h_scalars[9] and returns it.  Synchronises.
+// Lhat of one level (cached in the handle after the first evaluation: it depends on the geometry only).
 cbct_status step_bound_level(const cbct_geometry *g, const Level &L, double *lhat, cudaStream_t st)
 {
     cbct_status s;
+    if (L.lhat > 0.0) { *lhat = L.lhat; return CBCT_OK; }
     if ((s = launch_fill(g, L.d_g, L.nvox, 1.0f, st)) != CBCT_OK) return s;
     if ((s = launch_forward(g, L, L.d_g, nullptr, L.d_T, 2, nullptr, st)) != CBCT_OK) return s;   // L * (P 1)
     if ((s = launch_back(g, L, L.d_T, 1, nullptr, 0.0f, L.d_d, st)) != CBCT_OK) return s;
@@ -44,6 +25,7 @@ cbct_status step_bound_level(const cbct_geometry *g, const Level &L, double *lha
     CBCT_CUDA(cudaStreamSynchronize(st));
     const double c_norm = 2.0 * (double)L.nvox / (double)L.nray;
     *lhat = c_norm * g->h_scalars[9];
+    if (*lhat > 0.0) L.lhat = *lhat;
     return CBCT_OK;
 }
 
@@ -79,7 +61,6 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
 
     // data pyramid: y_l = 2x2 mean of y_{l-1}  (S12)
     {
-        StageTimer t(g, st, 4);
         for (int l = 1; l < nl; ++l) {
             const float *src = (l == 1) ? d_y : g->levels[l - 1].d_y;
             if ((s = launch_bin(g, g->levels[l - 1], src, g->levels[l].d_y, st)) != CBCT_OK) return s;
@@ -104,7 +85,6 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         const int n_it = p->iters_per_level[nl - 1 - l];
         double lhat = 0.0;
         {
-            StageTimer t(g, st, 3);
             if ((s = step_bound_level(g, L, &lhat, st)) != CBCT_OK) return s;
         }
         if (!(lhat > 0.0)) return cbct_fail(CBCT_ERR_GEOMETRY, "level %d: no ray crosses the volume (Lhat = %g)", l, lhat);
@@ -113,19 +93,15 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         if (rep && rep->step_abs) rep->step_abs[nl - 1 - l] = tau;
         for (int it = 0; it < n_it; ++it, ++done) {
             {
-                StageTimer t(g, st, 0);
                 if ((s = launch_forward(g, L, f, y, L.d_T, 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
             }
             if (want_obj) {
-                StageTimer t(g, st, 3);
                 if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, g->d_objective + 2 * done, st)) != CBCT_OK) return s;
             }
             {
-                StageTimer t(g, st, 1);
                 if ((s = launch_back(g, L, L.d_T, 1, f, (float)(tau * c_norm), L.d_g, st)) != CBCT_OK) return s;
             }
             {
-                StageTimer t(g, st, 2);
                 cbct_tv_report tr;
                 if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st)) != CBCT_OK) return s;
                 inner_total += tr.inner_iters;
@@ -133,7 +109,6 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
             }
         }
         if (l > 0) {
-            StageTimer t(g, st, 4);
             float *fine = (l == 1) ? d_vol : g->levels[l - 1].d_f;
             if ((s = launch_prolong(g, g->levels[l - 1], L.d_f, fine, st)) != CBCT_OK) return s;
         }

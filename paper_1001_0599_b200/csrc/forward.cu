@@ -70,6 +70,7 @@ forward_kernel(const LevelParams P, const float *__restrict__ vol, const float *
             } else if (rz.za < zlo || rz.za >= zhi) dhi = dlo - 1.0f;
         }
         float acc = 0.0f;
+        int cnt = 0;
         if (dhi > dlo) {
             const int s_lo = max(0, (int)floorf(dlo) + cd), s_hi = min(nd, (int)ceilf(dhi) + cd);
             float d0 = (float)(s_lo - cd);
@@ -85,22 +86,27 @@ forward_kernel(const LevelParams P, const float *__restrict__ vol, const float *
                 const float wa = fminf(sy, sz), wb = fmaxf(sy, sz) - wa, wc = 1.0f - fmaxf(sy, sz);
                 const int j0 = (int)fy0 + cm, j1 = (int)fy1 + cm, k0 = (int)fz0 + P.cz, k1 = (int)fz1 + P.cz;
                 const float *__restrict__ row = base + (size_t)s * nm;
-                if (wa > 0.0f && (unsigned)j0 < (unsigned)nm && (unsigned)k0 < (unsigned)P.nz)
-                    acc = fmaf(wa, __ldg(row + k0 * kstride + j0), acc);
+                if (wa > 0.0f && (unsigned)j0 < (unsigned)nm && (unsigned)k0 < (unsigned)P.nz) {
+                    if (MODE == 3) ++cnt; else acc = fmaf(wa, __ldg(row + k0 * kstride + j0), acc);
+                }
                 if (wb > 0.0f) {
                     const int jb = sy < sz ? j1 : j0, kb = sy < sz ? k0 : k1;
-                    if ((unsigned)jb < (unsigned)nm && (unsigned)kb < (unsigned)P.nz)
-                        acc = fmaf(wb, __ldg(row + kb * kstride + jb), acc);
+                    if ((unsigned)jb < (unsigned)nm && (unsigned)kb < (unsigned)P.nz) {
+                        if (MODE == 3) ++cnt; else acc = fmaf(wb, __ldg(row + kb * kstride + jb), acc);
+                    }
                 }
-                if (wc > 0.0f && (unsigned)j1 < (unsigned)nm && (unsigned)k1 < (unsigned)P.nz)
-                    acc = fmaf(wc, __ldg(row + k1 * kstride + j1), acc);
+                if (wc > 0.0f && (unsigned)j1 < (unsigned)nm && (unsigned)k1 < (unsigned)P.nz) {
+                    if (MODE == 3) ++cnt; else acc = fmaf(wc, __ldg(row + k1 * kstride + j1), acc);
+                }
                 y0 = y1; z0 = z1;
             }
         }
         const float Lr = ray_len_L(r, v);
         const float pr = acc * (Lr * r.inv_dd);
         const size_t o = ((size_t)a * P.nv + iv) * P.nu + iu;
-        if (MODE == 0) {
+        if (MODE == 3) {
+            sq = (double)cnt;
+        } else if (MODE == 0) {
             out[o] = pr;
         } else if (MODE == 2) {
             out[o] = pr * Lr;          // L * (P f): input of the transpose without a residual
@@ -110,7 +116,7 @@ forward_kernel(const LevelParams P, const float *__restrict__ vol, const float *
             sq = (double)T * (double)T;
         }
     }
-    if (MODE == 1) {
+    if (MODE == 1 || MODE == 3) {
         double s = block_sum(sq, slot);
         if (threadIdx.x == 0 && threadIdx.y == 0)
             partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
@@ -122,20 +128,32 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
 {
     const LevelParams &P = L.p;
     dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.ny + 31) / 32, P.nz);
-    transpose_xy_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_volT, P.nx, P.ny);
-    CBCT_LAUNCH_CHECK(g);
+    if (mode != 3) {
+        StageTimer t(g, st, ST_TRANSPOSE);
+        transpose_xy_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_volT, P.nx, P.ny);
+        CBCT_LAUNCH_CHECK(g);
+    }
     dim3 b(FWD_BX, FWD_BY), gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.np);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
     if (mode == 0) {
+        StageTimer t(g, st, ST_FORWARD);
         forward_kernel<0><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, d_out, nullptr);
         CBCT_LAUNCH_CHECK(g);
     } else if (mode == 2) {
+        StageTimer t(g, st, ST_FORWARD);
         forward_kernel<2><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, d_out, nullptr);
         CBCT_LAUNCH_CHECK(g);
     } else {
         if (nblk > (size_t)g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
-        forward_kernel<1><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, d_y, d_out, g->d_partials);
-        CBCT_LAUNCH_CHECK(g);
+        {
+            StageTimer t(g, st, ST_FORWARD);
+            if (mode == 3)
+                forward_kernel<3><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, nullptr, g->d_partials);
+            else
+                forward_kernel<1><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, d_y, d_out, g->d_partials);
+            CBCT_LAUNCH_CHECK(g);
+        }
+        StageTimer t(g, st, ST_REDUCE);
         finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
         CBCT_LAUNCH_CHECK(g);
     }
@@ -148,4 +166,18 @@ extern "C" cbct_status cbct_forward_project(const cbct_geometry *g, int level, c
     const Level *L = get_level(g, level);
     if (!L || !d_vol || !d_proj) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_forward_project: bad handle, level or NULL buffer");
     return launch_forward(g, *L, d_vol, nullptr, d_proj, 0, nullptr, (cudaStream_t)cuda_stream);
+}
+
+extern "C" cbct_status cbct_count_samples(const cbct_geometry *g, int level, unsigned long long *count,
+                                          void *cuda_stream)
+{
+    const Level *L = get_level(g, level);
+    if (!L || !count) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_count_samples: bad handle, level or NULL");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cbct_status s = launch_forward(g, *L, nullptr, nullptr, nullptr, 3, g->d_scalars + 10, st);
+    if (s != CBCT_OK) return s;
+    CBCT_CUDA(cudaMemcpyAsync(g->h_scalars + 10, g->d_scalars + 10, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    *count = (unsigned long long)(g->h_scalars[10] + 0.5);
+    return CBCT_OK;
 }

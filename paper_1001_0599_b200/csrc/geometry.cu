@@ -227,13 +227,17 @@ extern "C" cbct_status cbct_set_stage_timing(cbct_geometry *g, int enable)
 {
     if (!g) return cbct_fail(CBCT_ERR_INVALID_ARG, "NULL handle");
     g->stage_timing = enable ? 1 : 0;
-    for (int i = 0; i < 5; ++i) g->stage_ms[i] = 0.f;
+    for (int i = 0; i < CBCT_N_STAGES; ++i) { g->stage_ms[i] = 0.f; g->stage_calls[i] = 0; }
     return CBCT_OK;
 }
 
-extern "C" cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[5])
+extern "C" cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[CBCT_N_STAGES],
+                                         unsigned long long out_calls[CBCT_N_STAGES])
 {
     if (!g || !out_ms) return cbct_fail(CBCT_ERR_INVALID_ARG, "NULL argument");
-    for (int i = 0; i < 5; ++i) out_ms[i] = g->stage_ms[i];
+    for (int i = 0; i < CBCT_N_STAGES; ++i) {
+        out_ms[i] = g->stage_ms[i];
+        if (out_calls) out_calls[i] = g->stage_calls[i];
+    }
     return CBCT_OK;
 }

@@ -77,6 +77,7 @@ cbct_status launch_restrict(const cbct_geometry *g, const Level &fine, const flo
 {
     const int cx = fine.p.nx / 2, cy = fine.p.ny / 2, cz = fine.p.nz / 2;
     dim3 b(32, 8), gr((cx + 31) / 32, (cy + 7) / 8, cz);
+    StageTimer t(g, st, ST_TRANSFER);
     restrict_kernel<<<gr, b, 0, st>>>(cx, cy, cz, d_fine, d_coarse);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
@@ -86,6 +87,7 @@ cbct_status launch_bin(const cbct_geometry *g, const Level &fine, const float *d
 {
     const int cu = fine.p.nu / 2, cv = fine.p.nv / 2;
     dim3 b(32, 8), gr((cu + 31) / 32, (cv + 7) / 8, fine.p.np);
+    StageTimer t(g, st, ST_TRANSFER);
     bin_kernel<<<gr, b, 0, st>>>(cu, cv, d_fine, d_coarse);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
@@ -95,6 +97,7 @@ cbct_status launch_prolong(const cbct_geometry *g, const Level &fine, const floa
 {
     const int cx = fine.p.nx / 2, cy = fine.p.ny / 2, cz = fine.p.nz / 2;
     dim3 b(32, 8), gr((fine.p.nx + 31) / 32, (fine.p.ny + 7) / 8, fine.p.nz);
+    StageTimer t(g, st, ST_TRANSFER);
     prolong_kernel<<<gr, b, 0, st>>>(cx, cy, cz, fine.p.bc_xy == CBCT_BC_ZERO, fine.p.bc_z == CBCT_BC_ZERO, d_coarse, d_fine);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
@@ -103,6 +106,7 @@ cbct_status launch_prolong(const cbct_geometry *g, const Level &fine, const floa
 cbct_status launch_max(const cbct_geometry *g, const float *d_x, size_t n, double *d_out, cudaStream_t st)
 {
     const int blocks = 1024 < g->partials_stride ? 1024 : g->partials_stride;
+    StageTimer t(g, st, ST_TRANSFER);
     max_kernel<<<blocks, 256, 0, st>>>(n, d_x, g->d_partials);
     CBCT_LAUNCH_CHECK(g);
     finalize_max_kernel<<<1, 256, 0, st>>>(g->d_partials, blocks, d_out);
@@ -112,6 +116,7 @@ cbct_status launch_max(const cbct_geometry *g, const float *d_x, size_t n, doubl
 
 cbct_status launch_fill(const cbct_geometry *g, float *d_x, size_t n, float val, cudaStream_t st)
 {
+    StageTimer t(g, st, ST_TRANSFER);
     fill_kernel<<<g->sm_count * 8, 256, 0, st>>>(n, val, d_x);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;

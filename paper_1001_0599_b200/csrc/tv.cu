@@ -133,6 +133,7 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
     dim3 gr = tv_grid(D), b(TV_BX, TV_BY, TV_BZ);
     const int nblk = gr.x * gr.y * gr.z;
     if (nblk > g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
+    StageTimer t(g, st, ST_REDUCE);
     tv_pass_kernel<false, false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, nullptr, 0.f, (float)(delta * delta),
                                                   nullptr, g->d_partials, g->partials_stride);
     CBCT_LAUNCH_CHECK(g);
@@ -152,6 +153,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     const size_t n = L.nvox;
     const int cp_blocks = g->sm_count * 8;
     if (w <= 0.0) {
+        StageTimer t(g, st, ST_TV_UPDATE);
         clip_copy_kernel<<<cp_blocks, 256, 0, st>>>(n, d_g, nonneg, d_f);
         CBCT_LAUNCH_CHECK(g);
         if (rep) *rep = r;
@@ -171,11 +173,17 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     double E0 = 0.0;
     bool have_E0 = false;
     for (int it = 0; it < tp.max_inner; ++it) {
-        tv_pass_kernel<true, false><<<gr, b, 0, st>>>(D, cur, nullptr, d_g, nullptr, (float)beta, delta2, L.d_d,
-                                                     g->d_partials, S);
-        CBCT_LAUNCH_CHECK(g);
-        finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 3, S, ds);
-        CBCT_LAUNCH_CHECK(g);
+        {
+            StageTimer t(g, st, ST_TV_GRAD);
+            tv_pass_kernel<true, false><<<gr, b, 0, st>>>(D, cur, nullptr, d_g, nullptr, (float)beta, delta2, L.d_d,
+                                                         g->d_partials, S);
+            CBCT_LAUNCH_CHECK(g);
+        }
+        {
+            StageTimer t(g, st, ST_REDUCE);
+            finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 3, S, ds);
+            CBCT_LAUNCH_CHECK(g);
+        }
         CBCT_CUDA(cudaMemcpyAsync(hs, ds, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
         CBCT_CUDA(cudaStreamSynchronize(st));
         if (!have_E0) { E0 = hs[0] / N + 0.5 * beta * hs[1] / N; r.e_first = r.e_last = E0; have_E0 = true; }
@@ -185,11 +193,17 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         for (int bt = 0; bt <= tp.max_backtracks; ++bt) {
             hs[4] = lam;
             CBCT_CUDA(cudaMemcpyAsync(ds + 4, hs + 4, sizeof(double), cudaMemcpyHostToDevice, st));
-            tv_pass_kernel<false, true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, ds + 4, (float)beta, delta2, nullptr,
-                                                         g->d_partials, S);
-            CBCT_LAUNCH_CHECK(g);
-            finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 2, S, ds);
-            CBCT_LAUNCH_CHECK(g);
+            {
+                StageTimer t(g, st, ST_TV_TRIAL);
+                tv_pass_kernel<false, true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, ds + 4, (float)beta, delta2, nullptr,
+                                                             g->d_partials, S);
+                CBCT_LAUNCH_CHECK(g);
+            }
+            {
+                StageTimer t(g, st, ST_REDUCE);
+                finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 2, S, ds);
+                CBCT_LAUNCH_CHECK(g);
+            }
             CBCT_CUDA(cudaMemcpyAsync(hs, ds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
             CBCT_CUDA(cudaStreamSynchronize(st));
             Enew = hs[0] / N + 0.5 * beta * hs[1] / N;
@@ -200,8 +214,11 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         if (!accepted) break;
         float *nxt = bufs[which];
         which ^= 1;
-        tv_update_kernel<<<cp_blocks, 256, 0, st>>>(n, cur, L.d_d, ds + 4, 0, nxt);
-        CBCT_LAUNCH_CHECK(g);
+        {
+            StageTimer t(g, st, ST_TV_UPDATE);
+            tv_update_kernel<<<cp_blocks, 256, 0, st>>>(n, cur, L.d_d, ds + 4, 0, nxt);
+            CBCT_LAUNCH_CHECK(g);
+        }
         cur = nxt;
         ++r.inner_iters;
         const double rel = fabs(Enew - E0) / E0;
@@ -211,6 +228,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     }
     // result to d_f, with the non-negativity truncation
     if (cur != d_f || nonneg) {
+        StageTimer t(g, st, ST_TV_UPDATE);
         clip_copy_kernel<<<cp_blocks, 256, 0, st>>>(n, cur, nonneg, d_f);
         CBCT_LAUNCH_CHECK(g);
     }
