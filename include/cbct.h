@@ -62,12 +62,19 @@ typedef struct {
                                  ZERO in x,y and REFLECT in z (L161) */
     int max_levels;           /* multi-grid levels to provision (>= 1); level l has every volume and
                                  detector dimension divided by 2^l, so all must be divisible */
+    int no_symmetry;          /* 0 (default): when the in-plane grid is square, centred and even-sized and
+                                 the views come in quarter-turn quadruples (angles[a + n_proj/4] = angles[a]
+                                 + pi/2), both projectors compute each weight once for the four quarter-turn
+                                 images of a ray.  1: always use the generic one-view-at-a-time kernels. */
 } cbct_geometry_desc;
 
 /* Validates the description, uploads per-view tables and allocates all scratch for
  * `max_levels` levels.  *out is NULL on failure. */
 cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out);
 void cbct_geometry_destroy(cbct_geometry *g);
+
+/* Views per thread the projectors of `level` handle by quarter-turn symmetry: 4 or 1 (0: bad level). */
+int cbct_geometry_symmetry(const cbct_geometry *g, int level);
 
 /* Device bytes the handle allocated (scratch + tables). */
 unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g);

@@ -27,7 +27,7 @@ STATUS_NAMES = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_GEOMETRY",
 
 # every symbol include/cbct.h declares
 EXPORTS = [
-    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_device_bytes",
+    "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_symmetry", "cbct_geometry_device_bytes",
     "cbct_forward_project", "cbct_back_project", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
@@ -49,7 +49,7 @@ class _Desc(C.Structure):
                 ("du", C.c_double), ("dv", C.c_double), ("det_off_u", C.c_double), ("det_off_v", C.c_double),
                 ("sad", C.c_double), ("sdd", C.c_double),
                 ("n_proj", C.c_int), ("angles_rad", C.POINTER(C.c_double)),
-                ("bc_xy", C.c_int), ("bc_z", C.c_int), ("max_levels", C.c_int)]
+                ("bc_xy", C.c_int), ("bc_z", C.c_int), ("max_levels", C.c_int), ("no_symmetry", C.c_int)]
 
 
 class _TvParams(C.Structure):
@@ -110,6 +110,7 @@ def load_library():
     lib.cbct_geometry_create.argtypes = [C.POINTER(_Desc), C.POINTER(vp)]
     lib.cbct_geometry_destroy.argtypes = [vp]
     lib.cbct_geometry_destroy.restype = None
+    lib.cbct_geometry_symmetry.argtypes = [vp, ip]
     lib.cbct_geometry_device_bytes.argtypes = [vp]
     lib.cbct_geometry_device_bytes.restype = C.c_ulonglong
     lib.cbct_forward_project.argtypes = [vp, ip, vp, vp, vp]
@@ -165,7 +166,7 @@ class Geometry:
     `desc` is any object with the attributes of `inputs.Geometry`.
     """
 
-    def __init__(self, desc, max_levels: int = 1):
+    def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False):
         lib = load_library()
         self._h = C.c_void_p()
         self.desc = desc
@@ -181,6 +182,7 @@ class Geometry:
         ang = np.ascontiguousarray(desc.angles_rad(), dtype=np.float64)
         d.angles_rad = ang.ctypes.data_as(C.POINTER(C.c_double))
         d.bc_xy, d.bc_z, d.max_levels = desc.bc_xy, desc.bc_z, self.max_levels
+        d.no_symmetry = int(bool(no_symmetry))
         _check(lib.cbct_geometry_create(C.byref(d), C.byref(self._h)))
 
     def close(self):
@@ -214,6 +216,10 @@ class Geometry:
 
     def _nray(self, level):
         return int(np.prod(self.proj_shape(level)))
+
+    @property
+    def symmetry(self) -> int:
+        return int(load_library().cbct_geometry_symmetry(self._h, 0))
 
     @property
     def device_bytes(self) -> int:
@@ -335,8 +341,8 @@ class Geometry:
         return {k: (float(m), int(c)) for k, m, c in zip(self.STAGES, ms, calls)}
 
 
-def geometry_create(desc, max_levels: int = 1) -> Geometry:
-    return Geometry(desc, max_levels)
+def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False) -> Geometry:
+    return Geometry(desc, max_levels, no_symmetry)
 
 
 def version() -> str:

@@ -5,18 +5,26 @@
 // ray-driven scatter because threads would collide on voxels and evaluates the continuum
 // adjoint Eq. 6 instead; here each thread owns voxels and enumerates, per view, every
 // detector ray whose slab segment can cross them: the pixel range comes from the voxel ->
-// detector map of Eq. A6 (L401-L406) applied to the voxel's extent, and each candidate's
-// length is the overlap of three intervals in the slab parameter s in [0,1] -- the same
-// fp32 expressions, on the same table entries, as the forward projector's split.
-// No atomics, fixed order (views ascending, rows, columns) => deterministic.
+// detector map of Eq. A6 (L401-L406) applied to the voxel's extent (to first order, with
+// inflated half extents, so one reciprocal serves both detector axes), and each candidate's
+// length is the overlap of three intervals in the slab parameter t in [0,1] -- the same
+// fp32 crossing parameters, from the same table entries, as the forward projector's
+// (ray.cuh).  No atomics, fixed order (views ascending, columns, rows) => deterministic.
 //
 // Input is T scaled by L(u,v) (ray length source -> pixel), so the per-candidate weight is
 // overlap * inv_dd(view, iu).
+//
+// Rotation symmetry (R == 4, see forward.cu): a thread owns the four quarter-turn images
+// w_0..w_3 of a voxel of the first quadrant.  For a base view t and the image w_s, the
+// weights a(ray(t; iu, iv), w_s) are also those of the pairs (view t + 90 r, voxel w_{s+r}),
+// so each weight is computed once and applied to four accumulators with ONE 16-byte load
+// from the interleaved residual stack T4[base view][iv][iu][r].
 #include "cbct_internal.cuh"
 #include "ray.cuh"
 #include "reduce.cuh"
 
-// d_out[ray] = d_in[ray] * L(u,v)
+// d_out = d_in * L(u,v) in the d_T layout (plain for R == 1, quarter-turn interleaved for R == 4)
+template <int R>
 __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ rayu,
                                   const float *__restrict__ in, float *__restrict__ out)
 {
@@ -25,63 +33,106 @@ __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ 
     if (iu >= P.nu) return;
     const RayU r = load_rayu(rayu, a * P.nu + iu);
     const float v = fmaf((float)iv, P.dv, P.v0);
-    const size_t o = ((size_t)a * P.nv + iv) * P.nu + iu;
-    out[o] = __ldg(in + o) * ray_len_L(r, v);
+    const float Lr = ray_len_L(r, v);
+    const size_t plane = (size_t)P.nv * P.nu, pix = (size_t)iv * P.nu + iu;
+    float res[R];
+#pragma unroll
+    for (int q = 0; q < R; ++q) res[q] = __ldg(in + (size_t)(a + q * P.nbase) * plane + pix) * Lr;
+    if (R == 4) reinterpret_cast<float4 *>(out)[(size_t)a * plane + pix] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+    else out[(size_t)a * plane + pix] = res[0];
 }
 
-constexpr int BK_BX = 32, BK_BY = 4, BK_BZ = 2;
+constexpr int BK_BX = 32, BK_BY = 8;
 
-__global__ void __launch_bounds__(BK_BX *BK_BY *BK_BZ)
+template <int R>
+__global__ void __launch_bounds__(BK_BX *BK_BY)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
             const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
 {
     const int i = blockIdx.x * BK_BX + threadIdx.x;
     const int j = blockIdx.y * BK_BY + threadIdx.y;
-    const int k = blockIdx.z * BK_BZ + threadIdx.z;
-    if (i >= P.nx || j >= P.ny || k >= P.nz) return;
-    const float xc = fmaf((float)i, P.hx, P.x0), yc = fmaf((float)j, P.hy, P.y0), zc = fmaf((float)k, P.hz, P.z0);
+    const int k = blockIdx.z;
+    const int ni = R == 4 ? P.nx / 2 : P.nx, nj = R == 4 ? P.ny / 2 : P.ny;
+    if (i >= ni || j >= nj) return;
+    const float zc = fmaf((float)k, P.hz, P.z0);
     const float zlo_mm = zc - 0.5f * P.hz, zhi_mm = zc + 0.5f * P.hz;
-    // index-coordinate box of the voxel
-    const float bx = (float)(i - P.cx), by = (float)(j - P.cy), bz = (float)(k - P.cz);
-    float acc = 0.0f;
-    for (int a = 0; a < P.np; ++a) {
+    const float bz = (float)(k - P.cz), bz1 = bz + 1.0f;
+    // the R quarter-turn images of the voxel: (i,j), (n-1-j, i), (n-1-i, n-1-j), (j, n-1-i)
+    int vi[R], vj[R];
+    vi[0] = i; vj[0] = j;
+    if (R == 4) {
+        const int n1 = P.nx - 1;
+        vi[1 % R] = n1 - j; vj[1 % R] = i;
+        vi[2 % R] = n1 - i; vj[2 % R] = n1 - j;
+        vi[3 % R] = j;      vj[3 % R] = n1 - i;
+    }
+    float acc[R];
+#pragma unroll
+    for (int q = 0; q < R; ++q) acc[q] = 0.0f;
+    const size_t plane = (size_t)P.nv * P.nu;
+    for (int a = 0; a < P.nbase; ++a) {
         const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);   // c, s, dn, du
-        const float rn = fmaf(xc, vw.x, fmaf(yc, vw.y, P.sad));   // (X - S).e_n  > 0
-        const float ru = fmaf(xc, vw.y, -yc * vw.x);               // (X - S).e_u
-        // bounds of u* = sdd ru/rn and v* = sdd z/rn over the voxel (Eq. A6), conservative
-        const float inv_near = P.sdd / (rn - vw.z), inv_far = P.sdd / (rn + vw.z);
-        const float ul = ru - vw.w, uh = ru + vw.w;
-        const float u_lo = ul * (ul < 0.0f ? inv_near : inv_far), u_hi = uh * (uh > 0.0f ? inv_near : inv_far);
-        const float v_lo = zlo_mm * (zlo_mm < 0.0f ? inv_near : inv_far), v_hi = zhi_mm * (zhi_mm > 0.0f ? inv_near : inv_far);
-        const int iu_lo = max(0, (int)ceilf((u_lo - P.u0) * P.inv_du - 0.01f));
-        const int iu_hi = min(P.nu - 1, (int)floorf((u_hi - P.u0) * P.inv_du + 0.01f));
-        const int iv_lo = max(0, (int)ceilf((v_lo - P.v0) * P.inv_dv - 0.01f));
-        const int iv_hi = min(P.nv - 1, (int)floorf((v_hi - P.v0) * P.inv_dv + 0.01f));
-        if (iu_lo > iu_hi || iv_lo > iv_hi) continue;
-        const float *__restrict__ Ta = TL + (size_t)a * P.nv * P.nu;
-        for (int iu = iu_lo; iu <= iu_hi; ++iu) {
-            const RayU r = load_rayu(rayu, a * P.nu + iu);
-            const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;   // slab coordinate, minor plane
-            // in-plane: s-interval where minor(s) = y0 + s m lies in [mn, mn+1)
-            const float y0 = fmaf(d0, r.m, r.a0);
-            const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
-            const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
-            if (!(s_hi > s_lo)) continue;
-            float col = 0.0f;
-            for (int iv = iv_lo; iv <= iv_hi; ++iv) {
-                const float v = fmaf((float)iv, P.dv, P.v0);
-                const RayZ rz = ray_z(r, v, P.sz);
-                const float z0 = fmaf(d0, rz.mz, rz.za);
-                const float q1 = (bz - z0) * rz.inv_mz, q2 = (bz + 1.0f - z0) * rz.inv_mz;
-                const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
-                const float w = hi - lo;
-                if (w > 0.0f) col = fmaf(w, __ldg(Ta + (size_t)iv * P.nu + iu), col);
+        const float *__restrict__ Ta = TL + (size_t)a * plane * R;
+#pragma unroll
+        for (int sg = 0; sg < R; ++sg) {
+            const float xc = fmaf((float)vi[sg], P.hx, P.x0), yc = fmaf((float)vj[sg], P.hy, P.y0);
+            const float bx = (float)(vi[sg] - P.cx), by = (float)(vj[sg] - P.cy);
+            const float rn = fmaf(xc, vw.x, fmaf(yc, vw.y, P.sad));   // (X - S).e_n  > 0
+            const float ru = fmaf(xc, vw.y, -yc * vw.x);               // (X - S).e_u
+            // shadow of the voxel on the detector (Eq. A6): u* = sdd ru/rn, v* = sdd z/rn, to first
+            // order in the voxel's half extents dn, du (inflated in the table), plus 0.02 pixel
+            float rinv;
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(rn));
+            const float mag = P.sdd * rinv, tn = ru * rinv, e = vw.z * rinv;
+            const float uc = mag * ru, W = mag * fmaf(fabsf(tn), vw.z, vw.w);
+            const float v_lo = zlo_mm * mag * (zlo_mm < 0.0f ? 1.0f + e : 1.0f - e);
+            const float v_hi = zhi_mm * mag * (zhi_mm > 0.0f ? 1.0f + e : 1.0f - e);
+            const int iu_lo = max(0, __float2int_ru((uc - W - P.u0) * P.inv_du - 0.02f));
+            const int iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
+            const int iv_lo = max(0, __float2int_ru((v_lo - P.v0) * P.inv_dv - 0.02f));
+            const int iv_hi = min(P.nv - 1, __float2int_rd((v_hi - P.v0) * P.inv_dv + 0.02f));
+            if (iv_lo > iv_hi) continue;
+            for (int iu = iu_lo; iu <= iu_hi; ++iu) {
+                const RayU r = load_rayu(rayu, a * P.nu + iu);
+                const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;   // slab coordinate, minor plane
+                // in-plane: t-interval where minor(t) = y0 + t m lies in [mn, mn+1)
+                const float y0 = fmaf(d0, r.m, r.a0);
+                const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
+                const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
+                if (!(s_hi > s_lo)) continue;
+                float col[R];
+#pragma unroll
+                for (int q = 0; q < R; ++q) col[q] = 0.0f;
+                for (int iv = iv_lo; iv <= iv_hi; ++iv) {
+                    const float v = fmaf((float)iv, P.dv, P.v0);
+                    const RayZ rz = ray_z(r, v, P.sz);
+                    const float z0 = fmaf(d0, rz.mz, rz.za);
+                    const float q1 = (bz - z0) * rz.inv_mz, q2 = (bz1 - z0) * rz.inv_mz;
+                    const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
+                    const float w = hi - lo;
+                    if (w > 0.0f) {
+                        if (R == 4) {
+                            const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + (size_t)iv * P.nu + iu);
+                            col[0] = fmaf(w, t.x, col[0]);
+                            col[1 % R] = fmaf(w, t.y, col[1 % R]);
+                            col[2 % R] = fmaf(w, t.z, col[2 % R]);
+                            col[3 % R] = fmaf(w, t.w, col[3 % R]);
+                        } else {
+                            col[0] = fmaf(w, __ldg(Ta + (size_t)iv * P.nu + iu), col[0]);
+                        }
+                    }
+                }
+                // weights of image sg under base view a serve the pairs (view a + r nbase, image sg + r)
+#pragma unroll
+                for (int q = 0; q < R; ++q) acc[(sg + q) % R] = fmaf(col[q], r.inv_dd, acc[(sg + q) % R]);
             }
-            acc = fmaf(col, r.inv_dd, acc);
         }
     }
-    const size_t o = ((size_t)k * P.ny + j) * P.nx + i;
-    out[o] = f ? fmaf(-coef, acc, __ldg(f + o)) : acc;
+#pragma unroll
+    for (int q = 0; q < R; ++q) {
+        const size_t o = ((size_t)k * P.ny + vj[q]) * P.nx + vi[q];
+        out[o] = f ? fmaf(-coef, acc[q], __ldg(f + o)) : acc[q];
+    }
 }
 
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
@@ -91,15 +142,21 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
     const float *src = d_in;
     if (!scaled) {
         StageTimer t(g, st, ST_TRANSFER);
-        dim3 b(128), gr((P.nu + 127) / 128, P.nv, P.np);
-        scale_by_L_kernel<<<gr, b, 0, st>>>(P, L.d_rayu, d_in, L.d_T);
+        dim3 b(128), gr((P.nu + 127) / 128, P.nv, P.nbase);
+        if (P.nsym == 4) scale_by_L_kernel<4><<<gr, b, 0, st>>>(P, L.d_rayu, d_in, L.d_T);
+        else scale_by_L_kernel<1><<<gr, b, 0, st>>>(P, L.d_rayu, d_in, L.d_T);
         CBCT_LAUNCH_CHECK(g);
         src = L.d_T;
     }
-    dim3 b(BK_BX, BK_BY, BK_BZ);
-    dim3 gr((P.nx + BK_BX - 1) / BK_BX, (P.ny + BK_BY - 1) / BK_BY, (P.nz + BK_BZ - 1) / BK_BZ);
     StageTimer t(g, st, ST_BACK);
-    back_kernel<<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    dim3 b(BK_BX, BK_BY);
+    if (P.nsym == 4) {
+        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, (P.ny / 2 + BK_BY - 1) / BK_BY, P.nz);
+        back_kernel<4><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    } else {
+        dim3 gr((P.nx + BK_BX - 1) / BK_BX, (P.ny + BK_BY - 1) / BK_BY, P.nz);
+        back_kernel<1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    }
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }

@@ -29,11 +29,20 @@ struct __align__(16) RayU {
 // back-projector to bound the set of rays that can cross a voxel.
 struct __align__(16) ViewC {
     float c, s;        // cos, sin of the view angle
-    float dn, du;      // half extents of a voxel along e_n and e_u (mm)
+    float dn, du;      // half extents of a voxel along e_n and e_u (mm), slightly inflated
 };
+
+// Padding (voxels) of the staged volume copies on the minor in-plane axis and on z: the forward
+// projector walks a ray only through slabs where it is within half a voxel of the volume, so
+// every cell it can touch -- including the one-cell slack of its incremental cell tracking
+// -- lies inside the zero-filled margin and no load needs a bounds test.
+constexpr int PAD_M = 4, PAD_Z = 4;
 
 struct LevelParams {
     int nx, ny, nz, nu, nv, np;
+    int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
+    int nxP, nyP;              // padded row lengths of the staged copies A ([k][j][i]) and B ([k][i][j])
+    int offB;                  // element offset of copy B inside d_stage
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
     float hx, hy, hz;
     float x0, y0, z0;          // centre of voxel 0 in mm
@@ -51,8 +60,10 @@ struct Level {
     RayU *d_rayu = nullptr;     // [np][nu]
     ViewC *d_view = nullptr;    // [np]
     // scratch (all fp32 unless noted)
-    float *d_volT = nullptr;    // volume with x and y swapped: [k][i][j]
-    float *d_T = nullptr;       // residual scaled by L(u,v): what P^T consumes
+    float *d_stage = nullptr;   // zero-padded copies of the volume: A = [k+PZ][j][i+PM], B = [k+PZ][i][j+PM]
+    size_t stage_elems = 0;
+    float *d_T = nullptr;       // residual scaled by L(u,v): what P^T consumes; [np][nv][nu], or
+                                // [nbase][nv][nu][4] (the four quarter-turn views interleaved) when nsym == 4
     float *d_g = nullptr;       // g of Algorithm A1
     float *d_d = nullptr;       // descent direction of the ROF sub-solver
     float *d_f2 = nullptr;      // second volume (ping-pong / level volume)
@@ -73,6 +84,7 @@ struct cbct_geometry {
     int objective_cap = 0;
     unsigned long long device_bytes = 0;
     mutable unsigned long long launches = 0;
+    int allow_symmetry = 1;
     int stage_timing = 0;
     mutable float stage_ms[CBCT_N_STAGES] = {0};
     mutable unsigned long long stage_calls[CBCT_N_STAGES] = {0};
@@ -131,11 +143,14 @@ static inline const Level *get_level(const cbct_geometry *g, int level)
 }
 
 // internal launchers (asynchronous on `st`)
-// forward.cu : mode 0: out = P vol.  mode 1: out = L * (P vol - y), *d_sum_sq = sum (P vol - y)^2.
-//              mode 2: out = L * (P vol).  mode 3: *d_sum_sq = number of (ray, voxel) pairs, no volume read
+// forward.cu : mode 0: out = P vol (plain layout).
+//              mode 1: out = L * (P vol - y) in the d_T layout, *d_sum_sq = sum (P vol - y)^2.
+//              mode 2: out = L * (P vol) in the d_T layout.
+//              mode 3: *d_sum_sq = number of (ray, voxel) pairs, no volume read
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
                            float *d_out, int mode, double *d_sum_sq, cudaStream_t st);
-// back.cu : scaled != 0: d_in already holds L*T.  upd: out = f - coef * P^T in (f may be NULL: out = P^T in)
+// back.cu : scaled != 0: d_in already holds L*T in the d_T layout; else plain layout, unscaled.
+//           out = f - coef * P^T in (f may be NULL: out = P^T in)
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
                         const float *d_f, float coef, float *d_out, cudaStream_t st);
 // tv.cu

@@ -1,158 +1,256 @@
-// forward.cu -- A1/A2: cone-beam forward projector, one thread per detector ray.
+// forward.cu -- A1/A2: cone-beam forward projector, one thread per detector ray (or per group
+// of four rays related by quarter turns of the gantry).
 //
 // (P f)[ray] = sum_voxels len(ray ∩ voxel) f[voxel]   (Eq. 1 on piecewise-
 // constant voxels; "a ray-tracing algorithm, such as Siddon's", L187, L243).
 //
-// Instead of Siddon's data-dependent merge of three crossing lists, the ray is cut into
-// unit slabs of its DRIVING axis (the in-plane axis along which it crosses more planes).
-// Inside one slab it crosses at most one plane of the other in-plane axis and at most one
-// z-plane (checked at create), so it touches at most three voxels whose lengths follow in
-// closed form from the two crossing parameters.  The lengths are the exact radiological
-// path -- the same numbers as Siddon's up to rounding -- but every thread of a warp runs
-// the same loop with the same trip structure, and neighbouring rays read neighbouring
-// addresses: x-driven rays read the [k][i][j] copy of the volume, y-driven rays the
-// [k][j][i] original, so the minor in-plane index is always the fastest one in memory.
+// Instead of Siddon's data-dependent merge of three crossing lists, the ray is cut into unit
+// slabs of its DRIVING axis (the in-plane axis along which it crosses more planes).  Inside one
+// slab it crosses at most one plane of the other in-plane axis and at most one z-plane (checked
+// at create), so it touches at most three voxels whose lengths follow in closed form from the
+// two crossing parameters sy, sz in [0,1]:  min(sy,sz), |sy-sz|, 1-max(sy,sz).  These are the
+// exact radiological path -- Siddon's numbers up to rounding -- but every thread of a warp runs
+// the same branch-free loop, and neighbouring rays read neighbouring addresses.
+//
+// Memory: the volume is staged once per projection into two zero-padded copies, A = [k][j][i]
+// and B = [k][i][j], so that the minor in-plane index is the fastest one whichever axis drives
+// the ray, and so that no load needs a bounds test (cbct_internal.cuh, PAD_M / PAD_Z).  The cell
+// of the ray is tracked incrementally (the next plane on each axis and a linear offset), so the
+// loop holds no floor, no integer multiply and no branch.
+//
+// Rotation symmetry (nsym == 4): on a square, centred in-plane grid with views at angles
+// t, t+90, t+180, t+270 degrees, the ray (t + 90 r, iu, iv) is the ray (t, iu, iv) turned by
+// r quarter turns, and a quarter turn maps voxel (i,j) to (n-1-j, i).  One thread then walks
+// the base ray once and applies its weights to the four turned copies of the cell: the crossing
+// arithmetic is shared, only the three loads and FMAs are per view.
 #include "cbct_internal.cuh"
 #include "ray.cuh"
 #include "reduce.cuh"
 
-// [k][j][i] -> [k][i][j], 32x32 tiles through shared memory
-__global__ void transpose_xy_kernel(const float *__restrict__ in, float *__restrict__ out, int nx, int ny)
+// vol [k][j][i] -> A[(k+PZ)][j][i+PM] and B[(k+PZ)][i][j+PM]; 32x32 tiles through shared memory.
+// The margins of both copies were zeroed at create and are never written.
+__global__ void stage_volume_kernel(const float *__restrict__ in, float *__restrict__ stage, int nx, int ny,
+                                    int nxP, int nyP, int offB)
 {
     __shared__ float tile[32][33];
-    const size_t slice = (size_t)blockIdx.z * nx * ny;
-    int i = blockIdx.x * 32 + threadIdx.x, j0 = blockIdx.y * 32;
+    const int k = blockIdx.z;
+    const size_t slice = (size_t)k * nx * ny;
+    const size_t sliceA = (size_t)(k + PAD_Z) * ny * nxP, sliceB = (size_t)offB + (size_t)(k + PAD_Z) * nx * nyP;
+    const int i = blockIdx.x * 32 + threadIdx.x, j0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        int j = j0 + r;
-        if (i < nx && j < ny) tile[r][threadIdx.x] = __ldg(in + slice + (size_t)j * nx + i);
+        const int j = j0 + r;
+        if (i < nx && j < ny) {
+            const float v = __ldg(in + slice + (size_t)j * nx + i);
+            tile[r][threadIdx.x] = v;
+            stage[sliceA + (size_t)j * nxP + i + PAD_M] = v;
+        }
     }
     __syncthreads();
-    int j = j0 + threadIdx.x, i0 = blockIdx.x * 32;
+    const int j = j0 + threadIdx.x, i0 = blockIdx.x * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        int ii = i0 + r;
-        if (ii < nx && j < ny) out[slice + (size_t)ii * ny + j] = tile[threadIdx.x][r];
+        const int ii = i0 + r;
+        if (ii < nx && j < ny) stage[sliceB + (size_t)ii * nyP + j + PAD_M] = tile[threadIdx.x][r];
     }
 }
 
 constexpr int FWD_BX = 32, FWD_BY = 8;
 
-template <int MODE>
+// R = rays per thread (1, or 4 by rotation symmetry).  MODE as in launch_forward.
+template <int R, int MODE>
 __global__ void __launch_bounds__(FWD_BX *FWD_BY)
-forward_kernel(const LevelParams P, const float *__restrict__ vol, const float *__restrict__ volT,
-               const RayU *__restrict__ rayu, const float *__restrict__ y, float *__restrict__ out,
-               double *__restrict__ partials)
+forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
+               const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials)
 {
     __shared__ double slot[32];
     const int iu = blockIdx.x * FWD_BX + threadIdx.x;
     const int iv = blockIdx.y * FWD_BY + threadIdx.y;
-    const int a = blockIdx.z;
+    const int a = blockIdx.z;                  // base view
     double sq = 0.0;
     if (iu < P.nu && iv < P.nv) {
         const RayU r = load_rayu(rayu, a * P.nu + iu);
         const float v = fmaf((float)iv, P.dv, P.v0);
         const RayZ rz = ray_z(r, v, P.sz);
-        // driving axis: nd slabs, minor axis: nm voxels; memory index (k*nd + slab)*nm + minor
-        const float *__restrict__ base = r.drive ? vol : volT;
-        const int nd = r.drive ? P.ny : P.nx, nm = r.drive ? P.nx : P.ny;
+        // driving axis: nd slabs; minor axis: nm voxels in rows of nmP; cell (slab s, minor jm, k) of the
+        // copy whose rows run along the minor axis sits at (k + PZ) kstride + s nmP + jm + PM
+        const int nd = r.drive ? P.ny : P.nx, nm = r.drive ? P.nx : P.ny, nmP = r.drive ? P.nxP : P.nyP;
         const int cd = r.drive ? P.cy : P.cx, cm = r.drive ? P.cx : P.cy;
-        // slab range in which the ray can be inside the minor and z extents (conservative)
+        const int kstride = nd * nmP;
+        // slabs in which the ray comes within half a voxel of the volume
         float dlo = (float)(-cd), dhi = (float)(nd - cd);
         {
-            float mlo = (float)(-cm), mhi = (float)(nm - cm);
-            if (r.m != 0.0f) {
-                float t1 = (mlo - r.a0) * r.inv_m, t2 = (mhi - r.a0) * r.inv_m;
-                dlo = fmaxf(dlo, fminf(t1, t2) - 1.0f); dhi = fminf(dhi, fmaxf(t1, t2) + 1.0f);
-            } else if (r.a0 < mlo || r.a0 >= mhi) dhi = dlo - 1.0f;
-            float zlo = (float)(-P.cz), zhi = (float)(P.nz - P.cz);
-            if (rz.mz != 0.0f) {
-                float t1 = (zlo - rz.za) * rz.inv_mz, t2 = (zhi - rz.za) * rz.inv_mz;
-                dlo = fmaxf(dlo, fminf(t1, t2) - 1.0f); dhi = fminf(dhi, fmaxf(t1, t2) + 1.0f);
-            } else if (rz.za < zlo || rz.za >= zhi) dhi = dlo - 1.0f;
+            const float t1 = ((float)(-cm) - 0.5f - r.a0) * r.inv_m, t2 = ((float)(nm - cm) + 0.5f - r.a0) * r.inv_m;
+            dlo = fmaxf(dlo, fminf(t1, t2)); dhi = fminf(dhi, fmaxf(t1, t2));
+            const float t3 = ((float)(-P.cz) - 0.5f - rz.za) * rz.inv_mz, t4 = ((float)(P.nz - P.cz) + 0.5f - rz.za) * rz.inv_mz;
+            dlo = fmaxf(dlo, fminf(t3, t4)); dhi = fminf(dhi, fmaxf(t3, t4));
         }
-        float acc = 0.0f;
-        int cnt = 0;
+        float acc[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) acc[q] = 0.0f;
         if (dhi > dlo) {
             const int s_lo = max(0, (int)floorf(dlo) + cd), s_hi = min(nd, (int)ceilf(dhi) + cd);
-            float d0 = (float)(s_lo - cd);
-            float y0 = fmaf(d0, r.m, r.a0), z0 = fmaf(d0, rz.mz, rz.za);
-            const size_t kstride = (size_t)nd * nm;
+            float d = (float)(s_lo - cd);
+            float y0 = fmaf(d, r.m, r.a0), z0 = fmaf(d, rz.mz, rz.za);
+            const float fy = floorf(y0), fz = floorf(z0);
+            const bool posy = r.m >= 0.0f, posz = rz.mz >= 0.0f;
+            float nexty = posy ? fy + 1.0f : fy, nextz = posz ? fz + 1.0f : fz;
+            const float sgny = posy ? 1.0f : -1.0f, sgnz = posz ? 1.0f : -1.0f;
+            const int dj = posy ? 1 : -1, dk = posz ? kstride : -kstride;
+            const int jm = (int)fy + cm, kk = (int)fz + P.cz + PAD_Z;
+            // per-view offsets of the current cell, their slab step and their minor-axis step
+            int o[R], drow[R], dcol[R];
+            const int cb = r.drive ? 0 : P.offB;       // copy whose rows run along this ray's minor axis
+            if (R == 1) {
+                o[0] = cb + kk * kstride + s_lo * nmP + jm + PAD_M;
+                drow[0] = nmP; dcol[0] = dj;
+            } else {
+                // quarter turns (square grid, nd == nm == n, both copies of equal shape):
+                //   drive x: r0 B(s, jm)  r1 A(s, n-1-jm)    r2 B(n-1-s, n-1-jm)  r3 A(n-1-s, jm)
+                //   drive y: r0 A(s, jm)  r1 B(n-1-s, jm)    r2 A(n-1-s, n-1-jm)  r3 B(s, n-1-jm)
+                const int co = r.drive ? P.offB : 0;
+                const int zf = kk * kstride + PAD_M;
+                const int rf = s_lo * nmP, rb = (nd - 1 - s_lo) * nmP, cf = jm, cr = nm - 1 - jm;
+                o[0 % R] = cb + zf + rf + cf;                       drow[0 % R] = nmP;  dcol[0 % R] = dj;
+                o[2 % R] = cb + zf + rb + cr;                       drow[2 % R] = -nmP; dcol[2 % R] = -dj;
+                o[1 % R] = co + zf + (r.drive ? rb + cf : rf + cr); drow[1 % R] = r.drive ? -nmP : nmP; dcol[1 % R] = r.drive ? dj : -dj;
+                o[3 % R] = co + zf + (r.drive ? rf + cr : rb + cf); drow[3 % R] = r.drive ? nmP : -nmP; dcol[3 % R] = r.drive ? -dj : dj;
+            }
             for (int s = s_lo; s < s_hi; ++s) {
-                const float d1 = (float)(s + 1 - cd);
-                const float y1 = fmaf(d1, r.m, r.a0), z1 = fmaf(d1, rz.mz, rz.za);
-                const float fy0 = floorf(y0), fy1 = floorf(y1), fz0 = floorf(z0), fz1 = floorf(z1);
-                float sy = 1.0f, sz = 1.0f;
-                if (fy0 != fy1) sy = __saturatef((fmaxf(fy0, fy1) - y0) * r.inv_m);
-                if (fz0 != fz1) sz = __saturatef((fmaxf(fz0, fz1) - z0) * rz.inv_mz);
-                const float wa = fminf(sy, sz), wb = fmaxf(sy, sz) - wa, wc = 1.0f - fmaxf(sy, sz);
-                const int j0 = (int)fy0 + cm, j1 = (int)fy1 + cm, k0 = (int)fz0 + P.cz, k1 = (int)fz1 + P.cz;
-                const float *__restrict__ row = base + (size_t)s * nm;
-                if (wa > 0.0f && (unsigned)j0 < (unsigned)nm && (unsigned)k0 < (unsigned)P.nz) {
-                    if (MODE == 3) ++cnt; else acc = fmaf(wa, __ldg(row + k0 * kstride + j0), acc);
+                const float sy = __saturatef((nexty - y0) * r.inv_m);
+                const float sz = __saturatef((nextz - z0) * rz.inv_mz);
+                const float wa = fminf(sy, sz), mx = fmaxf(sy, sz);
+                const float wb = mx - wa, wc = 1.0f - mx;
+                const bool cy = sy < 1.0f, cz = sz < 1.0f, yfirst = sy < sz;
+                const int zc = cz ? dk : 0;
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    const int ob = o[q] + (yfirst ? dcol[q] : dk);
+                    const int oc = o[q] + (cy ? dcol[q] : 0) + zc;
+                    const float va = __ldg(stage + o[q]), vb = __ldg(stage + ob), vc = __ldg(stage + oc);
+                    acc[q] = fmaf(wa, va, acc[q]);
+                    acc[q] = fmaf(wb, vb, acc[q]);
+                    acc[q] = fmaf(wc, vc, acc[q]);
+                    o[q] = oc + drow[q];
                 }
-                if (wb > 0.0f) {
-                    const int jb = sy < sz ? j1 : j0, kb = sy < sz ? k0 : k1;
-                    if ((unsigned)jb < (unsigned)nm && (unsigned)kb < (unsigned)P.nz) {
-                        if (MODE == 3) ++cnt; else acc = fmaf(wb, __ldg(row + kb * kstride + jb), acc);
-                    }
-                }
-                if (wc > 0.0f && (unsigned)j1 < (unsigned)nm && (unsigned)k1 < (unsigned)P.nz) {
-                    if (MODE == 3) ++cnt; else acc = fmaf(wc, __ldg(row + k1 * kstride + j1), acc);
-                }
-                y0 = y1; z0 = z1;
+                if (cy) nexty += sgny;
+                if (cz) nextz += sgnz;
+                d += 1.0f;
+                y0 = fmaf(d, r.m, r.a0);
+                z0 = fmaf(d, rz.mz, rz.za);
             }
         }
         const float Lr = ray_len_L(r, v);
-        const float pr = acc * (Lr * r.inv_dd);
-        const size_t o = ((size_t)a * P.nv + iv) * P.nu + iu;
-        if (MODE == 3) {
-            sq = (double)cnt;
-        } else if (MODE == 0) {
-            out[o] = pr;
-        } else if (MODE == 2) {
-            out[o] = pr * Lr;          // L * (P f): input of the transpose without a residual
-        } else {
-            const float T = pr - __ldg(y + o);
-            out[o] = T * Lr;           // what the transpose consumes (see back.cu)
-            sq = (double)T * (double)T;
+        const float scale = Lr * r.inv_dd;
+        const size_t plane = (size_t)P.nv * P.nu, pix = (size_t)iv * P.nu + iu;
+        float res[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const float pr = acc[q] * scale;
+            const size_t o1 = (size_t)(a + q * P.nbase) * plane + pix;
+            if (MODE == 0) {
+                out[o1] = pr;
+            } else if (MODE == 2) {
+                res[q] = pr * Lr;                  // L * (P f): input of the transpose without a residual
+            } else {
+                const float T = pr - __ldg(y + o1);
+                res[q] = T * Lr;                   // what the transpose consumes (see back.cu)
+                sq += (double)T * (double)T;
+            }
+        }
+        if (MODE != 0) {
+            if (R == 4) {
+                reinterpret_cast<float4 *>(out)[(size_t)a * plane + pix] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+            } else {
+                out[(size_t)a * plane + pix] = res[0];
+            }
         }
     }
-    if (MODE == 1 || MODE == 3) {
+    if (MODE == 1) {
         double s = block_sum(sq, slot);
         if (threadIdx.x == 0 && threadIdx.y == 0)
             partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
     }
 }
 
+// S = number of (ray, voxel) pairs with positive length, by the same slab decomposition with the
+// cell taken from floor() and tested against the true volume bounds.  Not on the hot path.
+__global__ void __launch_bounds__(FWD_BX *FWD_BY)
+count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double *__restrict__ partials)
+{
+    __shared__ double slot[32];
+    const int iu = blockIdx.x * FWD_BX + threadIdx.x;
+    const int iv = blockIdx.y * FWD_BY + threadIdx.y;
+    const int a = blockIdx.z;
+    int cnt = 0;
+    if (iu < P.nu && iv < P.nv) {
+        const RayU r = load_rayu(rayu, a * P.nu + iu);
+        const float v = fmaf((float)iv, P.dv, P.v0);
+        const RayZ rz = ray_z(r, v, P.sz);
+        const int nd = r.drive ? P.ny : P.nx, nm = r.drive ? P.nx : P.ny;
+        const int cd = r.drive ? P.cy : P.cx, cm = r.drive ? P.cx : P.cy;
+        for (int s = 0; s < nd; ++s) {
+            const float d0 = (float)(s - cd), d1 = (float)(s + 1 - cd);
+            const float y0 = fmaf(d0, r.m, r.a0), z0 = fmaf(d0, rz.mz, rz.za);
+            const float y1 = fmaf(d1, r.m, r.a0), z1 = fmaf(d1, rz.mz, rz.za);
+            const float fy0 = floorf(y0), fy1 = floorf(y1), fz0 = floorf(z0), fz1 = floorf(z1);
+            float sy = 1.0f, sz = 1.0f;
+            if (fy0 != fy1) sy = __saturatef((fmaxf(fy0, fy1) - y0) * r.inv_m);
+            if (fz0 != fz1) sz = __saturatef((fmaxf(fz0, fz1) - z0) * rz.inv_mz);
+            const float wa = fminf(sy, sz), wb = fmaxf(sy, sz) - wa, wc = 1.0f - fmaxf(sy, sz);
+            const int j0 = (int)fy0 + cm, j1 = (int)fy1 + cm, k0 = (int)fz0 + P.cz, k1 = (int)fz1 + P.cz;
+            if (wa > 0.0f && (unsigned)j0 < (unsigned)nm && (unsigned)k0 < (unsigned)P.nz) ++cnt;
+            if (wb > 0.0f) {
+                const int jb = sy < sz ? j1 : j0, kb = sy < sz ? k0 : k1;
+                if ((unsigned)jb < (unsigned)nm && (unsigned)kb < (unsigned)P.nz) ++cnt;
+            }
+            if (wc > 0.0f && (unsigned)j1 < (unsigned)nm && (unsigned)k1 < (unsigned)P.nz) ++cnt;
+        }
+    }
+    double s = block_sum((double)cnt, slot);
+    if (threadIdx.x == 0 && threadIdx.y == 0)
+        partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
+}
+
+template <int R>
+static void launch_forward_mode(const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode, const float *stage,
+                                const RayU *rayu, const float *d_y, float *d_out, double *partials)
+{
+    if (mode == 0) forward_kernel<R, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
+    else if (mode == 2) forward_kernel<R, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
+    else forward_kernel<R, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, partials);
+}
+
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
                            float *d_out, int mode, double *d_sum_sq, cudaStream_t st)
 {
     const LevelParams &P = L.p;
-    dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.ny + 31) / 32, P.nz);
-    if (mode != 3) {
+    dim3 b(FWD_BX, FWD_BY);
+    if (mode == 3) {
+        dim3 gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.np);
+        const size_t nblk = (size_t)gr.x * gr.y * gr.z;
+        if (nblk > (size_t)g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
+        count_samples_kernel<<<gr, b, 0, st>>>(P, L.d_rayu, g->d_partials);
+        CBCT_LAUNCH_CHECK(g);
+        finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
+        CBCT_LAUNCH_CHECK(g);
+        return CBCT_OK;
+    }
+    {
         StageTimer t(g, st, ST_TRANSPOSE);
-        transpose_xy_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_volT, P.nx, P.ny);
+        dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.ny + 31) / 32, P.nz);
+        stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nxP, P.nyP, P.offB);
         CBCT_LAUNCH_CHECK(g);
     }
-    dim3 b(FWD_BX, FWD_BY), gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.np);
+    dim3 gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.nbase);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
-    if (mode == 0) {
+    if (mode == 1 && nblk > (size_t)g->partials_stride)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
+    {
         StageTimer t(g, st, ST_FORWARD);
-        forward_kernel<0><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, d_out, nullptr);
+        if (P.nsym == 4) launch_forward_mode<4>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
+        else launch_forward_mode<1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
         CBCT_LAUNCH_CHECK(g);
-    } else if (mode == 2) {
-        StageTimer t(g, st, ST_FORWARD);
-        forward_kernel<2><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, d_out, nullptr);
-        CBCT_LAUNCH_CHECK(g);
-    } else {
-        if (nblk > (size_t)g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
-        {
-            StageTimer t(g, st, ST_FORWARD);
-            if (mode == 3)
-                forward_kernel<3><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, nullptr, nullptr, g->d_partials);
-            else
-                forward_kernel<1><<<gr, b, 0, st>>>(P, d_vol, L.d_volT, L.d_rayu, d_y, d_out, g->d_partials);
-            CBCT_LAUNCH_CHECK(g);
-        }
+    }
+    if (mode == 1) {
         StageTimer t(g, st, ST_REDUCE);
         finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
         CBCT_LAUNCH_CHECK(g);

@@ -53,8 +53,10 @@ static cbct_status build_tables(const cbct_geometry *g, Level &L, std::vector<Ra
         const double syi = (-d.sad * s - d.vol_off[1]) / L.hy + shy;
         ViewC vc;
         vc.c = (float)c; vc.s = (float)s;
-        vc.dn = (float)(0.5 * (fabs(c) * L.hx + fabs(s) * L.hy));
-        vc.du = (float)(0.5 * (fabs(s) * L.hx + fabs(c) * L.hy));
+        // half extents of a voxel along e_n and e_u, inflated so that the first-order bounds of
+        // back.cu on the voxel's shadow are conservative
+        vc.dn = (float)(1.01 * 0.5 * (fabs(c) * L.hx + fabs(s) * L.hy));
+        vc.du = (float)(1.003 * 0.5 * (fabs(s) * L.hx + fabs(c) * L.hy));
         views[a] = vc;
         for (int iu = 0; iu < p.nu; ++iu) {
             const double u = (iu - 0.5 * (p.nu - 1)) * L.du + d.det_off_u;
@@ -111,7 +113,7 @@ static void free_all(cbct_geometry *g)
 {
     if (!g) return;
     for (Level &L : g->levels) {
-        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_volT); cudaFree(L.d_T);
+        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_stage); cudaFree(L.d_T);
         cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_y);
     }
     cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective);
@@ -144,6 +146,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     cbct_geometry *g = new (std::nothrow) cbct_geometry();
     if (!g) return cbct_fail(CBCT_ERR_OOM, "host allocation failed");
     g->desc = *desc;
+    g->allow_symmetry = desc->no_symmetry ? 0 : 1;
     g->sm_count = prop.multiProcessorCount;
     g->angles.resize(desc->n_proj);
     for (int a = 0; a < desc->n_proj; ++a)
@@ -173,6 +176,26 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.bc_xy = desc->bc_xy; p.bc_z = desc->bc_z;
         L.nvox = (size_t)p.nx * p.ny * p.nz;
         L.nray = (size_t)p.nu * p.nv * p.np;
+        // staged copies A [nz+2PZ][ny][nx+2PM] and B [nz+2PZ][nx][ny+2PM]
+        p.nxP = p.nx + 2 * PAD_M; p.nyP = p.ny + 2 * PAD_M;
+        {
+            const size_t sizeA = (size_t)(p.nz + 2 * PAD_Z) * p.ny * p.nxP, sizeB = (size_t)(p.nz + 2 * PAD_Z) * p.nx * p.nyP;
+            const size_t offB = (sizeA + 31) / 32 * 32;
+            L.stage_elems = offB + sizeB;
+            if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copies exceed 2^31 elements"); }
+            p.offB = (int)offB;
+        }
+        // quarter-turn symmetry: square centred in-plane grid, views a and a + np/4 a quarter turn apart
+        p.nsym = 1;
+        if (g->allow_symmetry && p.nx == p.ny && p.nx % 2 == 0 && L.hx == L.hy && desc->vol_off[0] == 0.0 &&
+            desc->vol_off[1] == 0.0 && p.np % 4 == 0) {
+            bool ok = true;
+            const int nb = p.np / 4;
+            for (int a = 0; a + nb < p.np && ok; ++a)
+                ok = fabs(g->angles[a + nb] - g->angles[a] - 0.5 * M_PI) < 1e-12;
+            if (ok) p.nsym = 4;
+        }
+        p.nbase = p.np / p.nsym;
 
         std::vector<RayU> rays;
         std::vector<ViewC> views;
@@ -181,7 +204,8 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
 #define TRY(x) do { st = (x); if (st != CBCT_OK) { free_all(g); return st; } } while (0)
         TRY(dev_alloc(g, &L.d_rayu, rays.size()));
         TRY(dev_alloc(g, &L.d_view, views.size()));
-        TRY(dev_alloc(g, &L.d_volT, L.nvox));
+        TRY(dev_alloc(g, &L.d_stage, L.stage_elems));
+        if (cudaMemset(L.d_stage, 0, L.stage_elems * sizeof(float)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the staged volume failed"); }
         TRY(dev_alloc(g, &L.d_T, L.nray));
         TRY(dev_alloc(g, &L.d_g, L.nvox));
         TRY(dev_alloc(g, &L.d_d, L.nvox));
@@ -218,6 +242,12 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     tls_error[0] = 0;
     *out = g;
     return CBCT_OK;
+}
+
+extern "C" int cbct_geometry_symmetry(const cbct_geometry *g, int level)
+{
+    const Level *L = get_level(g, level);
+    return L ? L->p.nsym : 0;
 }
 
 extern "C" unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g) { return g ? g->device_bytes : 0ULL; }

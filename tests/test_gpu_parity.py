@@ -58,18 +58,26 @@ def geoms():
     # 64^3 at config-2 sampling, 9 views
     out["cube64"] = I.Geometry(nx=64, ny=64, nz=64, hx=2.0, hy=2.0, hz=2.0, nu=128, nv=96, du=1.55, dv=1.55,
                                sad=1000.0, sdd=1500.0, n_proj=9)
+    # quarter-turn symmetric (square centred in-plane grid, 16 views), odd nz / nv, off-centre in z and v
+    out["sym48"] = I.Geometry(nx=48, ny=48, nz=21, hx=1.5, hy=1.5, hz=2.0, nu=80, nv=37, du=1.4, dv=1.7,
+                              sad=600.0, sdd=900.0, n_proj=16, vol_off=(0.0, 0.0, 1.3), det_off_u=0.9,
+                              det_off_v=-2.1,
+                              angles=np.deg2rad(11.0) + 2 * np.pi * np.arange(16) / 16)
     return out
 
 
 GEOMS = geoms()
+# every geometry through the generic kernels; the symmetric ones also through the quarter-turn kernels
+CASES = [(n, True) for n in GEOMS] + [(n, False) for n in ("config1", "aniso", "sym48")]
 
 
-@pytest.mark.parametrize("name", list(GEOMS))
-def test_forward_projector_matches_oracle(torch, cbct, orc, name):
+@pytest.mark.parametrize("name,generic", CASES)
+def test_forward_projector_matches_oracle(torch, cbct, orc, name, generic):
     g = GEOMS[name]
     f = I.uniform_volume(g, 11)
     want = orc.forward(g, f)
-    with cbct.geometry_create(g) as h:
+    with cbct.geometry_create(g, no_symmetry=generic) as h:
+        assert h.symmetry == (1 if generic or name not in ("config1", "aniso", "sym48") else 4)
         p = torch.empty(g.proj_shape, device="cuda", dtype=torch.float32)
         h.forward_project(dev(torch, f), p)
         got = p.cpu().numpy()
@@ -80,12 +88,12 @@ def test_forward_projector_matches_oracle(torch, cbct, orc, name):
     assert np.array_equal(got == 0.0, want == 0.0) or np.abs(got[want == 0.0]).max() < 1e-6
 
 
-@pytest.mark.parametrize("name", list(GEOMS))
-def test_back_projector_matches_oracle(torch, cbct, orc, name):
+@pytest.mark.parametrize("name,generic", CASES)
+def test_back_projector_matches_oracle(torch, cbct, orc, name, generic):
     g = GEOMS[name]
     q = I.uniform_projections(g, 12)
     want = orc.back(g, q)
-    with cbct.geometry_create(g) as h:
+    with cbct.geometry_create(g, no_symmetry=generic) as h:
         b = torch.empty(g.vol_shape, device="cuda", dtype=torch.float32)
         h.back_project(dev(torch, q), b)
         got = b.cpu().numpy()
@@ -94,13 +102,13 @@ def test_back_projector_matches_oracle(torch, cbct, orc, name):
     assert np.abs(got - want).max() <= 1e-4 * np.abs(want).max()
 
 
-@pytest.mark.parametrize("name", list(GEOMS))
-def test_adjoint_identity_on_device(torch, cbct, name):
+@pytest.mark.parametrize("name,generic", CASES)
+def test_adjoint_identity_on_device(torch, cbct, name, generic):
     """<P f, q> = <f, P^T q> to 1e-5 relative (north_star), dot products in fp64 on the host."""
     g = GEOMS[name]
     f = I.uniform_volume(g, 21)
     q = I.uniform_projections(g, 22) - 0.3
-    with cbct.geometry_create(g) as h:
+    with cbct.geometry_create(g, no_symmetry=generic) as h:
         p = torch.empty(g.proj_shape, device="cuda", dtype=torch.float32)
         b = torch.empty(g.vol_shape, device="cuda", dtype=torch.float32)
         h.forward_project(dev(torch, f), p)
@@ -110,8 +118,9 @@ def test_adjoint_identity_on_device(torch, cbct, name):
     assert abs(lhs - rhs) <= 1e-5 * abs(lhs), (lhs, rhs)
 
 
-def test_projectors_are_bitwise_deterministic(torch, cbct):
-    g = GEOMS["ragged"]
+@pytest.mark.parametrize("name", ["ragged", "sym48"])
+def test_projectors_are_bitwise_deterministic(torch, cbct, name):
+    g = GEOMS[name]
     f, q = dev(torch, I.uniform_volume(g, 31)), dev(torch, I.uniform_projections(g, 32))
     outs = []
     for _ in range(2):
@@ -309,8 +318,8 @@ def test_error_paths(torch, cbct):
             h.fbs_reconstruct(y, f, I.FbsSetup(step=2.5))
         with pytest.raises(ValueError):
             h.forward_project(f[:4], y)
-        with pytest.raises(cbct.CbctError):
-            h.forward_project(f, y, level=1)
+        with pytest.raises((ValueError, cbct.CbctError)):
+            h.forward_project(f, y, level=1)                                  # level not provisioned
     # voxels too flat in z for the cone angle: the driving-axis traversal refuses, loudly
     flat = I.Geometry(nx=16, ny=16, nz=64, hx=4.0, hy=4.0, hz=0.05, nu=16, nv=64, du=4.0, dv=4.0, sad=100.0,
                       sdd=150.0, n_proj=4)
