@@ -18,7 +18,7 @@
 // w_0..w_3 of a voxel of the first quadrant.  For a base view t and the image w_s, the
 // weights a(ray(t; iu, iv), w_s) are also those of the pairs (view t + 90 r, voxel w_{s+r}),
 // so each weight is computed once and applied to four accumulators with ONE 16-byte load
-// from the interleaved residual stack T4[base view][iv][iu][r].
+// from the interleaved residual stack T4[base view][iu][iv][r] (detector rows fastest, matching the lanes).
 #include "cbct_internal.cuh"
 #include "ray.cuh"
 #include "reduce.cuh"
@@ -38,22 +38,25 @@ __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ 
     float res[R];
 #pragma unroll
     for (int q = 0; q < R; ++q) res[q] = __ldg(in + (size_t)(a + q * P.nbase) * plane + pix) * Lr;
-    if (R == 4) reinterpret_cast<float4 *>(out)[(size_t)a * plane + pix] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
-    else out[(size_t)a * plane + pix] = res[0];
+    const size_t ot = ((size_t)a * P.nu + iu) * P.nv + iv;          // d_T layout: detector rows fastest
+    if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+    else out[ot] = res[0];
 }
 
-constexpr int BK_BX = 32, BK_BY = 8;
+constexpr int BK_BZ = 32, BK_BX = 8;       // block: 32 consecutive k (lanes) x 8 consecutive i
 
 template <int R>
-__global__ void __launch_bounds__(BK_BX *BK_BY)
+__global__ void __launch_bounds__(BK_BZ *BK_BX)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
             const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
 {
-    const int i = blockIdx.x * BK_BX + threadIdx.x;
-    const int j = blockIdx.y * BK_BY + threadIdx.y;
-    const int k = blockIdx.z;
-    const int ni = R == 4 ? P.nx / 2 : P.nx, nj = R == 4 ? P.ny / 2 : P.ny;
-    if (i >= ni || j >= nj) return;
+    // lanes run along z: a warp shares (i,j), hence the whole in-plane part of every candidate test
+    // (uniform branches, broadcast table loads), and its lanes read consecutive detector rows
+    const int k = blockIdx.z * BK_BZ + threadIdx.x;
+    const int i = blockIdx.x * BK_BX + threadIdx.y;
+    const int j = blockIdx.y;
+    const int ni = R == 4 ? P.nx / 2 : P.nx;
+    if (i >= ni || k >= P.nz) return;
     const float zc = fmaf((float)k, P.hz, P.z0);
     const float zlo_mm = zc - 0.5f * P.hz, zhi_mm = zc + 0.5f * P.hz;
     const float bz = (float)(k - P.cz), bz1 = bz + 1.0f;
@@ -112,13 +115,13 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
                     const float w = hi - lo;
                     if (w > 0.0f) {
                         if (R == 4) {
-                            const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + (size_t)iv * P.nu + iu);
+                            const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + (size_t)iu * P.nv + iv);
                             col[0] = fmaf(w, t.x, col[0]);
                             col[1 % R] = fmaf(w, t.y, col[1 % R]);
                             col[2 % R] = fmaf(w, t.z, col[2 % R]);
                             col[3 % R] = fmaf(w, t.w, col[3 % R]);
                         } else {
-                            col[0] = fmaf(w, __ldg(Ta + (size_t)iv * P.nu + iu), col[0]);
+                            col[0] = fmaf(w, __ldg(Ta + (size_t)iu * P.nv + iv), col[0]);
                         }
                     }
                 }
@@ -149,12 +152,12 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
         src = L.d_T;
     }
     StageTimer t(g, st, ST_BACK);
-    dim3 b(BK_BX, BK_BY);
+    dim3 b(BK_BZ, BK_BX);
     if (P.nsym == 4) {
-        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, (P.ny / 2 + BK_BY - 1) / BK_BY, P.nz);
+        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, P.ny / 2, (P.nz + BK_BZ - 1) / BK_BZ);
         back_kernel<4><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
     } else {
-        dim3 gr((P.nx + BK_BX - 1) / BK_BX, (P.ny + BK_BY - 1) / BK_BY, P.nz);
+        dim3 gr((P.nx + BK_BX - 1) / BK_BX, P.ny, (P.nz + BK_BZ - 1) / BK_BZ);
         back_kernel<1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
     }
     CBCT_LAUNCH_CHECK(g);

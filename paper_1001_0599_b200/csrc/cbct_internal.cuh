@@ -41,8 +41,8 @@ constexpr int PAD_M = 4, PAD_Z = 4;
 struct LevelParams {
     int nx, ny, nz, nu, nv, np;
     int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
-    int nxP, nyP;              // padded row lengths of the staged copies A ([k][j][i]) and B ([k][i][j])
-    int offB;                  // element offset of copy B inside d_stage
+    int nyP, nzP;              // padded extents of the staged volume [i + PM][j + PM][k + PZ] (k fastest)
+    int istride, jstride;      // its element strides along i and j (nyP * nzP, nzP)
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
     float hx, hy, hz;
     float x0, y0, z0;          // centre of voxel 0 in mm
@@ -60,10 +60,11 @@ struct Level {
     RayU *d_rayu = nullptr;     // [np][nu]
     ViewC *d_view = nullptr;    // [np]
     // scratch (all fp32 unless noted)
-    float *d_stage = nullptr;   // zero-padded copies of the volume: A = [k+PZ][j][i+PM], B = [k+PZ][i][j+PM]
+    float *d_stage = nullptr;   // zero-padded, z-fastest copy of the volume: [i+PM][j+PM][k+PZ]
     size_t stage_elems = 0;
-    float *d_T = nullptr;       // residual scaled by L(u,v): what P^T consumes; [np][nv][nu], or
-                                // [nbase][nv][nu][4] (the four quarter-turn views interleaved) when nsym == 4
+    float *d_T = nullptr;       // residual scaled by L(u,v): what P^T consumes; detector rows fastest:
+                                // [np][nu][nv], or [nbase][nu][nv][4] (the four quarter-turn views
+                                // interleaved) when nsym == 4
     float *d_g = nullptr;       // g of Algorithm A1
     float *d_d = nullptr;       // descent direction of the ROF sub-solver
     float *d_f2 = nullptr;      // second volume (ping-pong / level volume)

@@ -10,71 +10,67 @@
 // at create), so it touches at most three voxels whose lengths follow in closed form from the
 // two crossing parameters sy, sz in [0,1]:  min(sy,sz), |sy-sz|, 1-max(sy,sz).  These are the
 // exact radiological path -- Siddon's numbers up to rounding -- but every thread of a warp runs
-// the same branch-free loop, and neighbouring rays read neighbouring addresses.
+// the same branch-free loop.
 //
-// Memory: the volume is staged once per projection into two zero-padded copies, A = [k][j][i]
-// and B = [k][i][j], so that the minor in-plane index is the fastest one whichever axis drives
-// the ray, and so that no load needs a bounds test (cbct_internal.cuh, PAD_M / PAD_Z).  The cell
-// of the ray is tracked incrementally (the next plane on each axis and a linear offset), so the
-// loop holds no floor, no integer multiply and no branch.
+// Memory: the volume is staged once per projection into a zero-padded copy with z FASTEST,
+// [i][j][k], and the 32 lanes of a warp are 32 consecutive detector ROWS of one detector column.
+// All lanes then share the in-plane path (same slab, same minor cell, same in-plane crossing) and
+// differ only in z, where their cells are consecutive: every load of the warp falls in one or two
+// 128-byte lines whatever the view angle, one copy serves both driving axes and all quarter turns
+// (it stays L2-resident), and no load needs a bounds test (cbct_internal.cuh, PAD_M / PAD_Z).  The
+// cell of the ray is tracked incrementally (the next plane on each axis and a linear offset), so
+// the loop holds no floor, no integer multiply and no divergent branch.
 //
 // Rotation symmetry (nsym == 4): on a square, centred in-plane grid with views at angles
 // t, t+90, t+180, t+270 degrees, the ray (t + 90 r, iu, iv) is the ray (t, iu, iv) turned by
 // r quarter turns, and a quarter turn maps voxel (i,j) to (n-1-j, i).  One thread then walks
 // the base ray once and applies its weights to the four turned copies of the cell: the crossing
-// arithmetic is shared, only the three loads and FMAs are per view.
+// arithmetic is shared, only the loads and FMAs are per view.
 #include "cbct_internal.cuh"
 #include "ray.cuh"
 #include "reduce.cuh"
 
-// vol [k][j][i] -> A[(k+PZ)][j][i+PM] and B[(k+PZ)][i][j+PM]; 32x32 tiles through shared memory.
-// The margins of both copies were zeroed at create and are never written.
-__global__ void stage_volume_kernel(const float *__restrict__ in, float *__restrict__ stage, int nx, int ny,
-                                    int nxP, int nyP, int offB)
+// vol [k][j][i] -> stage[i+PM][j+PM][k+PZ]: per j, a 32x32 (k,i) tile through shared memory.
+// The margins of the staged copy were zeroed at create and are never written.
+__global__ void stage_volume_kernel(const float *__restrict__ in, float *__restrict__ stage, int nx, int ny, int nz,
+                                    int istride, int jstride)
 {
     __shared__ float tile[32][33];
-    const int k = blockIdx.z;
-    const size_t slice = (size_t)k * nx * ny;
-    const size_t sliceA = (size_t)(k + PAD_Z) * ny * nxP, sliceB = (size_t)offB + (size_t)(k + PAD_Z) * nx * nyP;
-    const int i = blockIdx.x * 32 + threadIdx.x, j0 = blockIdx.y * 32;
+    const int j = blockIdx.z;
+    const int i = blockIdx.x * 32 + threadIdx.x, k0 = blockIdx.y * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
-        const int j = j0 + r;
-        if (i < nx && j < ny) {
-            const float v = __ldg(in + slice + (size_t)j * nx + i);
-            tile[r][threadIdx.x] = v;
-            stage[sliceA + (size_t)j * nxP + i + PAD_M] = v;
-        }
+        const int k = k0 + r;
+        if (i < nx && k < nz) tile[r][threadIdx.x] = __ldg(in + ((size_t)k * ny + j) * nx + i);
     }
     __syncthreads();
-    const int j = j0 + threadIdx.x, i0 = blockIdx.x * 32;
+    const int k = k0 + threadIdx.x, i0 = blockIdx.x * 32;
     for (int r = threadIdx.y; r < 32; r += blockDim.y) {
         const int ii = i0 + r;
-        if (ii < nx && j < ny) stage[sliceB + (size_t)ii * nyP + j + PAD_M] = tile[threadIdx.x][r];
+        if (ii < nx && k < nz)
+            stage[(size_t)(ii + PAD_M) * istride + (size_t)(j + PAD_M) * jstride + k + PAD_Z] = tile[threadIdx.x][r];
     }
 }
 
-constexpr int FWD_BX = 32, FWD_BY = 8;
+constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x 8 detector columns
 
 // R = rays per thread (1, or 4 by rotation symmetry).  MODE as in launch_forward.
 template <int R, int MODE>
-__global__ void __launch_bounds__(FWD_BX *FWD_BY)
+__global__ void __launch_bounds__(FWD_BV *FWD_BU)
 forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials)
 {
     __shared__ double slot[32];
-    const int iu = blockIdx.x * FWD_BX + threadIdx.x;
-    const int iv = blockIdx.y * FWD_BY + threadIdx.y;
+    const int iv = blockIdx.y * FWD_BV + threadIdx.x;
+    const int iu = blockIdx.x * FWD_BU + threadIdx.y;
     const int a = blockIdx.z;                  // base view
     double sq = 0.0;
     if (iu < P.nu && iv < P.nv) {
         const RayU r = load_rayu(rayu, a * P.nu + iu);
         const float v = fmaf((float)iv, P.dv, P.v0);
         const RayZ rz = ray_z(r, v, P.sz);
-        // driving axis: nd slabs; minor axis: nm voxels in rows of nmP; cell (slab s, minor jm, k) of the
-        // copy whose rows run along the minor axis sits at (k + PZ) kstride + s nmP + jm + PM
-        const int nd = r.drive ? P.ny : P.nx, nm = r.drive ? P.nx : P.ny, nmP = r.drive ? P.nxP : P.nyP;
+        // driving axis: nd slabs; minor axis: nm voxels
+        const int nd = r.drive ? P.ny : P.nx, nm = r.drive ? P.nx : P.ny;
         const int cd = r.drive ? P.cy : P.cx, cm = r.drive ? P.cx : P.cy;
-        const int kstride = nd * nmP;
         // slabs in which the ray comes within half a voxel of the volume
         float dlo = (float)(-cd), dhi = (float)(nd - cd);
         {
@@ -94,25 +90,22 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             const bool posy = r.m >= 0.0f, posz = rz.mz >= 0.0f;
             float nexty = posy ? fy + 1.0f : fy, nextz = posz ? fz + 1.0f : fz;
             const float sgny = posy ? 1.0f : -1.0f, sgnz = posz ? 1.0f : -1.0f;
-            const int dj = posy ? 1 : -1, dk = posz ? kstride : -kstride;
+            const int dj = posy ? 1 : -1, dk = posz ? 1 : -1;
             const int jm = (int)fy + cm, kk = (int)fz + P.cz + PAD_Z;
-            // per-view offsets of the current cell, their slab step and their minor-axis step
+            // the current cell in (i,j), its slab step and its minor-axis step; a quarter turn maps
+            // a position (i,j) -> (n-1-j, i) and a step (di,dj) -> (-dj, di)
+            int ci = r.drive ? jm : s_lo, cj = r.drive ? s_lo : jm;
+            int si = r.drive ? 0 : 1, sj = r.drive ? 1 : 0;
+            int mi = r.drive ? dj : 0, mj = r.drive ? 0 : dj;
             int o[R], drow[R], dcol[R];
-            const int cb = r.drive ? 0 : P.offB;       // copy whose rows run along this ray's minor axis
-            if (R == 1) {
-                o[0] = cb + kk * kstride + s_lo * nmP + jm + PAD_M;
-                drow[0] = nmP; dcol[0] = dj;
-            } else {
-                // quarter turns (square grid, nd == nm == n, both copies of equal shape):
-                //   drive x: r0 B(s, jm)  r1 A(s, n-1-jm)    r2 B(n-1-s, n-1-jm)  r3 A(n-1-s, jm)
-                //   drive y: r0 A(s, jm)  r1 B(n-1-s, jm)    r2 A(n-1-s, n-1-jm)  r3 B(s, n-1-jm)
-                const int co = r.drive ? P.offB : 0;
-                const int zf = kk * kstride + PAD_M;
-                const int rf = s_lo * nmP, rb = (nd - 1 - s_lo) * nmP, cf = jm, cr = nm - 1 - jm;
-                o[0 % R] = cb + zf + rf + cf;                       drow[0 % R] = nmP;  dcol[0 % R] = dj;
-                o[2 % R] = cb + zf + rb + cr;                       drow[2 % R] = -nmP; dcol[2 % R] = -dj;
-                o[1 % R] = co + zf + (r.drive ? rb + cf : rf + cr); drow[1 % R] = r.drive ? -nmP : nmP; dcol[1 % R] = r.drive ? dj : -dj;
-                o[3 % R] = co + zf + (r.drive ? rf + cr : rb + cf); drow[3 % R] = r.drive ? nmP : -nmP; dcol[3 % R] = r.drive ? -dj : dj;
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                o[q] = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride + kk;
+                drow[q] = si * P.istride + sj * P.jstride;
+                dcol[q] = mi * P.istride + mj * P.jstride;
+                int t = ci; ci = P.nx - 1 - cj; cj = t;
+                t = si; si = -sj; sj = t;
+                t = mi; mi = -mj; mj = t;
             }
             for (int s = s_lo; s < s_hi; ++s) {
                 const float sy = __saturatef((nexty - y0) * r.inv_m);
@@ -125,7 +118,10 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
                 for (int q = 0; q < R; ++q) {
                     const int ob = o[q] + (yfirst ? dcol[q] : dk);
                     const int oc = o[q] + (cy ? dcol[q] : 0) + zc;
-                    const float va = __ldg(stage + o[q]), vb = __ldg(stage + ob), vc = __ldg(stage + oc);
+                    const float va = __ldg(stage + o[q]);
+                    float vb = 0.0f, vc = 0.0f;
+                    if (wb > 0.0f) vb = __ldg(stage + ob);
+                    if (wc > 0.0f) vc = __ldg(stage + oc);
                     acc[q] = fmaf(wa, va, acc[q]);
                     acc[q] = fmaf(wb, vb, acc[q]);
                     acc[q] = fmaf(wc, vc, acc[q]);
@@ -156,12 +152,10 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
                 sq += (double)T * (double)T;
             }
         }
-        if (MODE != 0) {
-            if (R == 4) {
-                reinterpret_cast<float4 *>(out)[(size_t)a * plane + pix] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
-            } else {
-                out[(size_t)a * plane + pix] = res[0];
-            }
+        if (MODE != 0) {                           // d_T layout: [base view][iu][iv] (x4 interleaved)
+            const size_t ot = ((size_t)a * P.nu + iu) * P.nv + iv;
+            if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+            else out[ot] = res[0];
         }
     }
     if (MODE == 1) {
@@ -170,6 +164,8 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
     }
 }
+
+constexpr int FWD_BX = 32, FWD_BY = 8;      // count_samples_kernel block
 
 // S = number of (ray, voxel) pairs with positive length, by the same slab decomposition with the
 // cell taken from floor() and tested against the true volume bounds.  Not on the hot path.
@@ -236,11 +232,12 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     }
     {
         StageTimer t(g, st, ST_TRANSPOSE);
-        dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.ny + 31) / 32, P.nz);
-        stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nxP, P.nyP, P.offB);
+        dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.nz + 31) / 32, P.ny);
+        stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nz, P.istride, P.jstride);
         CBCT_LAUNCH_CHECK(g);
     }
-    dim3 gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.nbase);
+    b = dim3(FWD_BV, FWD_BU);
+    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, (P.nv + FWD_BV - 1) / FWD_BV, P.nbase);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
     if (mode == 1 && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");

@@ -176,15 +176,11 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.bc_xy = desc->bc_xy; p.bc_z = desc->bc_z;
         L.nvox = (size_t)p.nx * p.ny * p.nz;
         L.nray = (size_t)p.nu * p.nv * p.np;
-        // staged copies A [nz+2PZ][ny][nx+2PM] and B [nz+2PZ][nx][ny+2PM]
-        p.nxP = p.nx + 2 * PAD_M; p.nyP = p.ny + 2 * PAD_M;
-        {
-            const size_t sizeA = (size_t)(p.nz + 2 * PAD_Z) * p.ny * p.nxP, sizeB = (size_t)(p.nz + 2 * PAD_Z) * p.nx * p.nyP;
-            const size_t offB = (sizeA + 31) / 32 * 32;
-            L.stage_elems = offB + sizeB;
-            if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copies exceed 2^31 elements"); }
-            p.offB = (int)offB;
-        }
+        // staged copy [nx+2PM][ny+2PM][nz+2PZ], z fastest
+        p.nyP = p.ny + 2 * PAD_M; p.nzP = p.nz + 2 * PAD_Z;
+        p.jstride = p.nzP; p.istride = p.nyP * p.nzP;
+        L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP;
+        if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }
         // quarter-turn symmetry: square centred in-plane grid, views a and a + np/4 a quarter turn apart
         p.nsym = 1;
         if (g->allow_symmetry && p.nx == p.ny && p.nx % 2 == 0 && L.hx == L.hy && desc->vol_off[0] == 0.0 &&
