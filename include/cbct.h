@@ -65,7 +65,9 @@ typedef struct {
     int no_symmetry;          /* 0 (default): when the in-plane grid is square, centred and even-sized and
                                  the views come in quarter-turn quadruples (angles[a + n_proj/4] = angles[a]
                                  + pi/2), both projectors compute each weight once for the four quarter-turn
-                                 images of a ray.  1: always use the generic one-view-at-a-time kernels. */
+                                 images of a ray; when the volume is centred in z and the detector in v
+                                 (even nz, nv) also for the mirror image z -> -z.
+                                 1: always use the generic one-ray-at-a-time kernels. */
 } cbct_geometry_desc;
 
 /* Validates the description, uploads per-view tables and allocates all scratch for
@@ -73,7 +75,8 @@ typedef struct {
 cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct_geometry **out);
 void cbct_geometry_destroy(cbct_geometry *g);
 
-/* Views per thread the projectors of `level` handle by quarter-turn symmetry: 4 or 1 (0: bad level). */
+/* Rays (voxels) per thread the projectors of `level` handle with one weight computation: 4 by
+ * quarter-turn symmetry, times 2 by the mirror symmetry z -> -z; 8, 4, 2 or 1 (0: bad level). */
 int cbct_geometry_symmetry(const cbct_geometry *g, int level);
 
 /* Device bytes the handle allocated (scratch + tables). */

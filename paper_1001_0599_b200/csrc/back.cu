@@ -19,6 +19,10 @@
 // weights a(ray(t; iu, iv), w_s) are also those of the pairs (view t + 90 r, voxel w_{s+r}),
 // so each weight is computed once and applied to four accumulators with ONE 16-byte load
 // from the interleaved residual stack T4[base view][iu][iv][r] (detector rows fastest, matching the lanes).
+//
+// Mirror symmetry (M == 2): with the volume centred in z and the detector in v, the weight of
+// (ray (iu, iv), voxel k) is also that of (ray (iu, nv-1-iv), voxel nz-1-k): the thread owns
+// both voxels and adds a second load per weight.
 #include "cbct_internal.cuh"
 #include "ray.cuh"
 #include "reduce.cuh"
@@ -45,7 +49,7 @@ __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ 
 
 constexpr int BK_BZ = 32, BK_BX = 8;       // block: 32 consecutive k (lanes) x 8 consecutive i
 
-template <int R>
+template <int R, int M>
 __global__ void __launch_bounds__(BK_BZ *BK_BX)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
             const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
@@ -56,7 +60,7 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
     const int i = blockIdx.x * BK_BX + threadIdx.y;
     const int j = blockIdx.y;
     const int ni = R == 4 ? P.nx / 2 : P.nx;
-    if (i >= ni || k >= P.nz) return;
+    if (i >= ni || k >= P.nz / M) return;           // M == 2: the upper half are the mirror images nz-1-k
     const float zc = fmaf((float)k, P.hz, P.z0);
     const float zlo_mm = zc - 0.5f * P.hz, zhi_mm = zc + 0.5f * P.hz;
     const float bz = (float)(k - P.cz), bz1 = bz + 1.0f;
@@ -69,9 +73,9 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
         vi[2 % R] = n1 - i; vj[2 % R] = n1 - j;
         vi[3 % R] = j;      vj[3 % R] = n1 - i;
     }
-    float acc[R];
+    float acc[R * M];
 #pragma unroll
-    for (int q = 0; q < R; ++q) acc[q] = 0.0f;
+    for (int q = 0; q < R * M; ++q) acc[q] = 0.0f;
     const size_t plane = (size_t)P.nv * P.nu;
     for (int a = 0; a < P.nbase; ++a) {
         const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);   // c, s, dn, du
@@ -103,9 +107,9 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
                 const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
                 const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
                 if (!(s_hi > s_lo)) continue;
-                float col[R];
+                float col[R * M];
 #pragma unroll
-                for (int q = 0; q < R; ++q) col[q] = 0.0f;
+                for (int q = 0; q < R * M; ++q) col[q] = 0.0f;
                 for (int iv = iv_lo; iv <= iv_hi; ++iv) {
                     const float v = fmaf((float)iv, P.dv, P.v0);
                     const RayZ rz = ray_z(r, v, P.sz);
@@ -114,28 +118,37 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
                     const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
                     const float w = hi - lo;
                     if (w > 0.0f) {
-                        if (R == 4) {
-                            const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + (size_t)iu * P.nv + iv);
-                            col[0] = fmaf(w, t.x, col[0]);
-                            col[1 % R] = fmaf(w, t.y, col[1 % R]);
-                            col[2 % R] = fmaf(w, t.z, col[2 % R]);
-                            col[3 % R] = fmaf(w, t.w, col[3 % R]);
-                        } else {
-                            col[0] = fmaf(w, __ldg(Ta + (size_t)iu * P.nv + iv), col[0]);
+#pragma unroll
+                        for (int mm = 0; mm < M; ++mm) {        // the mirror voxel sees the mirror row with the same weight
+                            const size_t ot = (size_t)iu * P.nv + (mm ? P.nv - 1 - iv : iv);
+                            if (R == 4) {
+                                const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + ot);
+                                col[mm * R] = fmaf(w, t.x, col[mm * R]);
+                                col[mm * R + 1 % R] = fmaf(w, t.y, col[mm * R + 1 % R]);
+                                col[mm * R + 2 % R] = fmaf(w, t.z, col[mm * R + 2 % R]);
+                                col[mm * R + 3 % R] = fmaf(w, t.w, col[mm * R + 3 % R]);
+                            } else {
+                                col[mm * R] = fmaf(w, __ldg(Ta + ot), col[mm * R]);
+                            }
                         }
                     }
                 }
                 // weights of image sg under base view a serve the pairs (view a + r nbase, image sg + r)
 #pragma unroll
-                for (int q = 0; q < R; ++q) acc[(sg + q) % R] = fmaf(col[q], r.inv_dd, acc[(sg + q) % R]);
+                for (int mm = 0; mm < M; ++mm)
+#pragma unroll
+                    for (int q = 0; q < R; ++q)
+                        acc[mm * R + (sg + q) % R] = fmaf(col[mm * R + q], r.inv_dd, acc[mm * R + (sg + q) % R]);
             }
         }
     }
 #pragma unroll
-    for (int q = 0; q < R; ++q) {
-        const size_t o = ((size_t)k * P.ny + vj[q]) * P.nx + vi[q];
-        out[o] = f ? fmaf(-coef, acc[q], __ldg(f + o)) : acc[q];
-    }
+    for (int mm = 0; mm < M; ++mm)
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            const size_t o = ((size_t)(mm ? P.nz - 1 - k : k) * P.ny + vj[q]) * P.nx + vi[q];
+            out[o] = f ? fmaf(-coef, acc[mm * R + q], __ldg(f + o)) : acc[mm * R + q];
+        }
 }
 
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
@@ -153,12 +166,15 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
     }
     StageTimer t(g, st, ST_BACK);
     dim3 b(BK_BZ, BK_BX);
+    const int nzh = P.nz / P.nmir;
     if (P.nsym == 4) {
-        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, P.ny / 2, (P.nz + BK_BZ - 1) / BK_BZ);
-        back_kernel<4><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, P.ny / 2, (nzh + BK_BZ - 1) / BK_BZ);
+        if (P.nmir == 2) back_kernel<4, 2><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+        else back_kernel<4, 1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
     } else {
-        dim3 gr((P.nx + BK_BX - 1) / BK_BX, P.ny, (P.nz + BK_BZ - 1) / BK_BZ);
-        back_kernel<1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+        dim3 gr((P.nx + BK_BX - 1) / BK_BX, P.ny, (nzh + BK_BZ - 1) / BK_BZ);
+        if (P.nmir == 2) back_kernel<1, 2><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+        else back_kernel<1, 1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
     }
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;

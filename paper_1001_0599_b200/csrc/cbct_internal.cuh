@@ -41,6 +41,7 @@ constexpr int PAD_M = 4, PAD_Z = 4;
 struct LevelParams {
     int nx, ny, nz, nu, nv, np;
     int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
+    int nmir;                  // 2 when the z-mirror image of every ray / voxel shares its weights, else 1
     int nyP, nzP;              // padded extents of the staged volume [i + PM][j + PM][k + PZ] (k fastest)
     int istride, jstride;      // its element strides along i and j (nyP * nzP, nzP)
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0

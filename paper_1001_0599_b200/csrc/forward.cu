@@ -21,6 +21,10 @@
 // cell of the ray is tracked incrementally (the next plane on each axis and a linear offset), so
 // the loop holds no floor, no integer multiply and no divergent branch.
 //
+// Mirror symmetry (nmir == 2): with the volume centred in z and the detector centred in v, the ray
+// (iu, nv-1-iv) is the mirror image z -> -z of the ray (iu, iv); the same thread walks it through
+// the cells nz-1-k with the same weights.
+//
 // Rotation symmetry (nsym == 4): on a square, centred in-plane grid with views at angles
 // t, t+90, t+180, t+270 degrees, the ray (t + 90 r, iu, iv) is the ray (t, iu, iv) turned by
 // r quarter turns, and a quarter turn maps voxel (i,j) to (n-1-j, i).  One thread then walks
@@ -53,8 +57,10 @@ __global__ void stage_volume_kernel(const float *__restrict__ in, float *__restr
 
 constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x 8 detector columns
 
-// R = rays per thread (1, or 4 by rotation symmetry).  MODE as in launch_forward.
-template <int R, int MODE>
+// R = quarter-turn views per thread (1 or 4), M = 2 when the thread also walks the mirror image
+// z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again.  MODE as in
+// launch_forward.
+template <int R, int M, int MODE>
 __global__ void __launch_bounds__(FWD_BV *FWD_BU)
 forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials)
@@ -63,8 +69,9 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
     const int iv = blockIdx.y * FWD_BV + threadIdx.x;
     const int iu = blockIdx.x * FWD_BU + threadIdx.y;
     const int a = blockIdx.z;                  // base view
+    const int nvh = M == 2 ? P.nv / 2 : P.nv;  // rows this grid walks; the others are their mirrors
     double sq = 0.0;
-    if (iu < P.nu && iv < P.nv) {
+    if (iu < P.nu && iv < nvh) {
         const RayU r = load_rayu(rayu, a * P.nu + iu);
         const float v = fmaf((float)iv, P.dv, P.v0);
         const RayZ rz = ray_z(r, v, P.sz);
@@ -79,9 +86,9 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             const float t3 = ((float)(-P.cz) - 0.5f - rz.za) * rz.inv_mz, t4 = ((float)(P.nz - P.cz) + 0.5f - rz.za) * rz.inv_mz;
             dlo = fmaxf(dlo, fminf(t3, t4)); dhi = fminf(dhi, fmaxf(t3, t4));
         }
-        float acc[R];
+        float acc[R * M];
 #pragma unroll
-        for (int q = 0; q < R; ++q) acc[q] = 0.0f;
+        for (int q = 0; q < R * M; ++q) acc[q] = 0.0f;
         if (dhi > dlo) {
             const int s_lo = max(0, (int)floorf(dlo) + cd), s_hi = min(nd, (int)ceilf(dhi) + cd);
             float d = (float)(s_lo - cd);
@@ -97,10 +104,13 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             int ci = r.drive ? jm : s_lo, cj = r.drive ? s_lo : jm;
             int si = r.drive ? 0 : 1, sj = r.drive ? 1 : 0;
             int mi = r.drive ? dj : 0, mj = r.drive ? 0 : dj;
-            int o[R], drow[R], dcol[R];
+            const float *p[R * M];
+            int drow[R], dcol[R];
 #pragma unroll
             for (int q = 0; q < R; ++q) {
-                o[q] = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride + kk;
+                const int o = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride;
+                p[q] = stage + o + kk;
+                if (M == 2) p[R + q] = stage + o + (P.nzP - 1 - kk);
                 drow[q] = si * P.istride + sj * P.jstride;
                 dcol[q] = mi * P.istride + mj * P.jstride;
                 int t = ci; ci = P.nx - 1 - cj; cj = t;
@@ -108,24 +118,40 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
                 t = mi; mi = -mj; mj = t;
             }
             for (int s = s_lo; s < s_hi; ++s) {
+                // crossing parameters of the next minor-axis plane and the next z-plane, clipped to the slab
                 const float sy = __saturatef((nexty - y0) * r.inv_m);
                 const float sz = __saturatef((nextz - z0) * rz.inv_mz);
-                const float wa = fminf(sy, sz), mx = fmaxf(sy, sz);
-                const float wb = mx - wa, wc = 1.0f - mx;
-                const bool cy = sy < 1.0f, cz = sz < 1.0f, yfirst = sy < sz;
+                const bool cy = sy < 1.0f, cz = sz < 1.0f;
+                const float lo = fminf(sy, sz);                          // first cell: [0, lo]
+                const float hi = (cy && cz) ? fmaxf(sy, sz) : lo;        // middle cell: [lo, hi]; last: [hi, 1]
+                const float wl = 1.0f - hi;
                 const int zc = cz ? dk : 0;
+                const float *pc[R * M];
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
-                    const int ob = o[q] + (yfirst ? dcol[q] : dk);
-                    const int oc = o[q] + (cy ? dcol[q] : 0) + zc;
-                    const float va = __ldg(stage + o[q]);
-                    float vb = 0.0f, vc = 0.0f;
-                    if (wb > 0.0f) vb = __ldg(stage + ob);
-                    if (wc > 0.0f) vc = __ldg(stage + oc);
-                    acc[q] = fmaf(wa, va, acc[q]);
-                    acc[q] = fmaf(wb, vb, acc[q]);
-                    acc[q] = fmaf(wc, vc, acc[q]);
-                    o[q] = oc + drow[q];
+                    const int dc = cy ? dcol[q] : 0;
+                    pc[q] = p[q] + (dc + zc);
+                    acc[q] = fmaf(lo, __ldg(p[q]), acc[q]);
+                    acc[q] = fmaf(wl, __ldg(pc[q]), acc[q]);
+                    if (M == 2) {
+                        pc[R + q] = p[R + q] + (dc - zc);
+                        acc[R + q] = fmaf(lo, __ldg(p[R + q]), acc[R + q]);
+                        acc[R + q] = fmaf(wl, __ldg(pc[R + q]), acc[R + q]);
+                    }
+                }
+                if (hi > lo) {      // both planes crossed inside this slab, at different parameters: a third cell
+                    const float wm = hi - lo;
+                    const bool yfirst = sy < sz;
+#pragma unroll
+                    for (int q = 0; q < R; ++q) {
+                        acc[q] = fmaf(wm, __ldg(p[q] + (yfirst ? dcol[q] : dk)), acc[q]);
+                        if (M == 2) acc[R + q] = fmaf(wm, __ldg(p[R + q] + (yfirst ? dcol[q] : -dk)), acc[R + q]);
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    p[q] = pc[q] + drow[q];
+                    if (M == 2) p[R + q] = pc[R + q] + drow[q];
                 }
                 if (cy) nexty += sgny;
                 if (cz) nextz += sgnz;
@@ -136,26 +162,31 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
         }
         const float Lr = ray_len_L(r, v);
         const float scale = Lr * r.inv_dd;
-        const size_t plane = (size_t)P.nv * P.nu, pix = (size_t)iv * P.nu + iu;
-        float res[R];
+        const size_t plane = (size_t)P.nv * P.nu;
 #pragma unroll
-        for (int q = 0; q < R; ++q) {
-            const float pr = acc[q] * scale;
-            const size_t o1 = (size_t)(a + q * P.nbase) * plane + pix;
-            if (MODE == 0) {
-                out[o1] = pr;
-            } else if (MODE == 2) {
-                res[q] = pr * Lr;                  // L * (P f): input of the transpose without a residual
-            } else {
-                const float T = pr - __ldg(y + o1);
-                res[q] = T * Lr;                   // what the transpose consumes (see back.cu)
-                sq += (double)T * (double)T;
+        for (int mm = 0; mm < M; ++mm) {
+            const int ivm = mm ? P.nv - 1 - iv : iv;
+            const size_t pix = (size_t)ivm * P.nu + iu;
+            float res[R];
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                const float pr = acc[mm * R + q] * scale;
+                const size_t o1 = (size_t)(a + q * P.nbase) * plane + pix;
+                if (MODE == 0) {
+                    out[o1] = pr;
+                } else if (MODE == 2) {
+                    res[q] = pr * Lr;                  // L * (P f): input of the transpose without a residual
+                } else {
+                    const float T = pr - __ldg(y + o1);
+                    res[q] = T * Lr;                   // what the transpose consumes (see back.cu)
+                    sq += (double)T * (double)T;
+                }
             }
-        }
-        if (MODE != 0) {                           // d_T layout: [base view][iu][iv] (x4 interleaved)
-            const size_t ot = ((size_t)a * P.nu + iu) * P.nv + iv;
-            if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
-            else out[ot] = res[0];
+            if (MODE != 0) {                           // d_T layout: [base view][iu][iv] (x4 interleaved)
+                const size_t ot = ((size_t)a * P.nu + iu) * P.nv + ivm;
+                if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+                else out[ot] = res[0];
+            }
         }
     }
     if (MODE == 1) {
@@ -206,13 +237,13 @@ count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double 
         partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
 }
 
-template <int R>
+template <int R, int M>
 static void launch_forward_mode(const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode, const float *stage,
                                 const RayU *rayu, const float *d_y, float *d_out, double *partials)
 {
-    if (mode == 0) forward_kernel<R, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
-    else if (mode == 2) forward_kernel<R, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
-    else forward_kernel<R, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, partials);
+    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
+    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
+    else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, partials);
 }
 
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
@@ -237,14 +268,16 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         CBCT_LAUNCH_CHECK(g);
     }
     b = dim3(FWD_BV, FWD_BU);
-    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, (P.nv + FWD_BV - 1) / FWD_BV, P.nbase);
+    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV, P.nbase);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
     if (mode == 1 && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
     {
         StageTimer t(g, st, ST_FORWARD);
-        if (P.nsym == 4) launch_forward_mode<4>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
-        else launch_forward_mode<1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
+        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
+        else if (P.nsym == 4) launch_forward_mode<4, 1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
+        else if (P.nmir == 2) launch_forward_mode<1, 2>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
+        else launch_forward_mode<1, 1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
         CBCT_LAUNCH_CHECK(g);
     }
     if (mode == 1) {

@@ -192,6 +192,8 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
             if (ok) p.nsym = 4;
         }
         p.nbase = p.np / p.nsym;
+        // mirror symmetry z -> -z: volume centred in z, detector centred in v, even sizes
+        p.nmir = (g->allow_symmetry && desc->vol_off[2] == 0.0 && desc->det_off_v == 0.0 && p.nz % 2 == 0 && p.nv % 2 == 0) ? 2 : 1;
 
         std::vector<RayU> rays;
         std::vector<ViewC> views;
@@ -243,7 +245,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
 extern "C" int cbct_geometry_symmetry(const cbct_geometry *g, int level)
 {
     const Level *L = get_level(g, level);
-    return L ? L->p.nsym : 0;
+    return L ? L->p.nsym * L->p.nmir : 0;
 }
 
 extern "C" unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g) { return g ? g->device_bytes : 0ULL; }
