@@ -61,7 +61,7 @@ constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x
 // z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again.  MODE as in
 // launch_forward.
 template <int R, int M, int MODE>
-__global__ void __launch_bounds__(FWD_BV *FWD_BU)
+__global__ void __launch_bounds__(FWD_BV *FWD_BU, 2)
 forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials)
 {
@@ -126,20 +126,20 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
                 const float hi = (cy && cz) ? fmaxf(sy, sz) : lo;        // middle cell: [lo, hi]; last: [hi, 1]
                 const float wl = 1.0f - hi;
                 const int zc = cz ? dk : 0;
+                // issue every load of the step before the first use: the loop is bound by load latency otherwise
                 const float *pc[R * M];
+                float va[R * M], vc[R * M];
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
                     const int dc = cy ? dcol[q] : 0;
                     pc[q] = p[q] + (dc + zc);
-                    acc[q] = fmaf(lo, __ldg(p[q]), acc[q]);
-                    acc[q] = fmaf(wl, __ldg(pc[q]), acc[q]);
-                    if (M == 2) {
-                        pc[R + q] = p[R + q] + (dc - zc);
-                        acc[R + q] = fmaf(lo, __ldg(p[R + q]), acc[R + q]);
-                        acc[R + q] = fmaf(wl, __ldg(pc[R + q]), acc[R + q]);
-                    }
+                    if (M == 2) pc[R + q] = p[R + q] + (dc - zc);
                 }
-                if (hi > lo) {      // both planes crossed inside this slab, at different parameters: a third cell
+#pragma unroll
+                for (int q = 0; q < R * M; ++q) { va[q] = __ldg(p[q]); vc[q] = __ldg(pc[q]); }
+#pragma unroll
+                for (int q = 0; q < R * M; ++q) acc[q] = fmaf(wl, vc[q], fmaf(lo, va[q], acc[q]));
+                if (hi > lo) {      // both planes crossed inside this slab, at different parameters (rare): a third cell
                     const float wm = hi - lo;
                     const bool yfirst = sy < sz;
 #pragma unroll
