@@ -243,6 +243,7 @@ def run_ours(args):
         inner = trials = 0
         barrier()
         with ClockSampler(local) as clk:
+            torch.cuda.profiler.start()        # cudaProfilerStart: `ncu --profile-from-start off` sees only the timed region
             ev0.record(stream)
             for _ in range(args.steps):
                 r = step_device()
@@ -250,6 +251,7 @@ def run_ours(args):
                 trials += r.trials_total
             ev1.record(stream)
             barrier()
+            torch.cuda.profiler.stop()
         ms_total = max_over_ranks(ev0.elapsed_time(ev1))
         launches = h.launch_count - l0
         clocks = clk.summary()
