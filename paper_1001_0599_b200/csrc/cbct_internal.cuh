@@ -81,6 +81,7 @@ struct cbct_geometry {
     double *d_partials = nullptr;   // fp64 block partials, 4 rows of partials_stride
     int partials_stride = 0;        // >= the block count of every reducing kernel on every level
     double *d_scalars = nullptr;    // reduced scalars on the device
+    unsigned int *d_counter = nullptr;  // ticket of the fused reductions (reduce.cuh); 0 between kernels
     double *h_scalars = nullptr;    // pinned host mirror
     double *d_objective = nullptr;  // per-iteration E1, E2 pairs
     int objective_cap = 0;

@@ -63,7 +63,8 @@ constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x
 template <int R, int M, int MODE>
 __global__ void __launch_bounds__(FWD_BV *FWD_BU, 2)
 forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
-               const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials)
+               const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
+               unsigned int *__restrict__ counter, double *__restrict__ sum_out)
 {
     __shared__ double slot[32];
     const int iv = blockIdx.y * FWD_BV + threadIdx.x;
@@ -189,10 +190,10 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             }
         }
     }
-    if (MODE == 1) {
-        double s = block_sum(sq, slot);
-        if (threadIdx.x == 0 && threadIdx.y == 0)
-            partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
+    if (MODE == 1) {        // E2 numerator: sum of squared residuals, second stage fused (reduce.cuh)
+        double s[1];
+        s[0] = block_sum(sq, slot);
+        publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
     }
 }
 
@@ -238,12 +239,13 @@ count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double 
 }
 
 template <int R, int M>
-static void launch_forward_mode(const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode, const float *stage,
-                                const RayU *rayu, const float *d_y, float *d_out, double *partials)
+static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode,
+                                const float *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq)
 {
-    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
-    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr);
-    else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, partials);
+    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
+    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
+    else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                   g->d_counter, d_sum_sq);
 }
 
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
@@ -274,15 +276,10 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
     {
         StageTimer t(g, st, ST_FORWARD);
-        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
-        else if (P.nsym == 4) launch_forward_mode<4, 1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
-        else if (P.nmir == 2) launch_forward_mode<1, 2>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
-        else launch_forward_mode<1, 1>(P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, g->d_partials);
-        CBCT_LAUNCH_CHECK(g);
-    }
-    if (mode == 1) {
-        StageTimer t(g, st, ST_REDUCE);
-        finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
+        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
+        else if (P.nsym == 4) launch_forward_mode<4, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
+        else if (P.nmir == 2) launch_forward_mode<1, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
+        else launch_forward_mode<1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
         CBCT_LAUNCH_CHECK(g);
     }
     return CBCT_OK;

@@ -116,7 +116,7 @@ static void free_all(cbct_geometry *g)
         cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_stage); cudaFree(L.d_T);
         cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_y);
     }
-    cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective);
+    cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter);
     if (g->h_scalars) cudaFreeHost(g->h_scalars);
     for (int i = 0; i < 4; ++i) if (g->ev[i]) cudaEventDestroy(g->ev[i]);
     delete g;
@@ -219,8 +219,10 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         size_t need = 1024;
         for (const Level &L : g->levels) {
             const LevelParams &p = L.p;
-            size_t fwd = (size_t)((p.nu + 31) / 32) * ((p.nv + 7) / 8) * p.np;
-            size_t tv = (size_t)((p.nx + 31) / 32) * ((p.ny + 3) / 4) * ((p.nz + 1) / 2);
+            size_t fwd = (size_t)((p.nu + 31) / 32) * ((p.nv + 7) / 8) * p.np;     // count_samples_kernel blocks
+            size_t fw2 = (size_t)((p.nu + 7) / 8) * ((p.nv + 31) / 32) * p.np;     // forward_kernel blocks (upper bound)
+            if (fw2 > fwd) fwd = fw2;
+            size_t tv = (size_t)((p.nx + 31) / 32) * ((p.ny + 15) / 16) * ((p.nz + 3) / 4);   // tv.cu blocks, shortest march
             if (fwd > need) need = fwd;
             if (tv > need) need = tv;
         }
@@ -228,6 +230,8 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     }
     TRY(dev_alloc(g, &g->d_partials, (size_t)4 * g->partials_stride));
     TRY(dev_alloc(g, &g->d_scalars, (size_t)kScalars));
+    TRY(dev_alloc(g, &g->d_counter, (size_t)1));
+    if (cudaMemset(g->d_counter, 0, sizeof(unsigned int)) != cudaSuccess || cudaMemset(g->d_scalars, 0, sizeof(double) * kScalars) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the reduction scalars failed"); }
     g->objective_cap = 4096;
     TRY(dev_alloc(g, &g->d_objective, (size_t)2 * g->objective_cap));
 #undef TRY

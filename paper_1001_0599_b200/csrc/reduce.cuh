@@ -74,3 +74,37 @@ static __global__ void finalize_max_kernel(const double *partials, int n, double
     double s = block_max(v, slot);
     if (threadIdx.x == 0) out[0] = s;
 }
+
+// Fused second stage ("last block done"): every block publishes `rows` partial sums (held by
+// thread 0 in vals[]), takes an INTEGER ticket, and the block that draws the last ticket adds all
+// partials -- thread t sums elements t, t+T, ... of each row, then the block tree -- and writes
+// out[0..rows).  Which block is last varies from run to run, the order of the additions does not:
+// the result depends on the launch shape only.  `counter` must be 0 at launch; the last block
+// resets it.  All threads of the block must call this (it synchronises).  `slot`: >= 32 doubles.
+template <int ROWS>
+__device__ __forceinline__ void publish_and_finalize(const double (&vals)[ROWS], int rows, double *partials, int stride,
+                                                     unsigned int *counter, double *out, double *slot)
+{
+    __shared__ int last_flag;
+    const int tid = (threadIdx.z * blockDim.y + threadIdx.y) * blockDim.x + threadIdx.x;
+    const int nthr = blockDim.x * blockDim.y * blockDim.z;
+    const unsigned int nblk = gridDim.x * gridDim.y * gridDim.z;
+    const unsigned int blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r)
+            if (r < rows) partials[(size_t)r * stride + blk] = vals[r];
+        __threadfence();
+        last_flag = (atomicAdd(counter, 1u) == nblk - 1u);
+    }
+    __syncthreads();
+    if (!last_flag) return;
+    __threadfence();
+    for (int r = 0; r < rows; ++r) {
+        double v = 0.0;
+        for (unsigned int i = tid; i < nblk; i += nthr) v += __ldcg(partials + (size_t)r * stride + i);
+        const double s = block_sum(v, slot);
+        if (tid == 0) out[r] = s;
+    }
+    if (tid == 0) *counter = 0u;
+}

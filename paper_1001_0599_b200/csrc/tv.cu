@@ -26,124 +26,371 @@ static TvDims tv_dims(const Level &L)
     return D;
 }
 
-// forward-difference gradient at (i,j,k) of the field  f - lam*d  (d may be NULL)
+// value of the field  u = f - lam*dir  (TRIAL) or u = f  at p[o]
 template <bool TRIAL>
-__device__ __forceinline__ float field(const float *__restrict__ f, const float *__restrict__ d, float lam, size_t o)
+__device__ __forceinline__ float field(const float *__restrict__ f, const float *__restrict__ dir, float lam, size_t o)
 {
-    return TRIAL ? fmaf(-lam, __ldg(d + o), __ldg(f + o)) : __ldg(f + o);
+    return TRIAL ? fmaf(-lam, __ldg(dir + o), __ldg(f + o)) : __ldg(f + o);
 }
 
-template <bool TRIAL>
-__device__ __forceinline__ void grad3(const TvDims &D, const float *__restrict__ f, const float *__restrict__ d,
-                                      float lam, int i, int j, int k, float &c, float &gx, float &gy, float &gz)
+__device__ __forceinline__ float rsqrt_ftz(float x)
 {
-    const size_t o = ((size_t)k * D.ny + j) * D.nx + i;
-    c = field<TRIAL>(f, d, lam, o);
-    const float xn = (i + 1 < D.nx) ? field<TRIAL>(f, d, lam, o + 1) : (D.zero_xy ? 0.0f : c);
-    const float yn = (j + 1 < D.ny) ? field<TRIAL>(f, d, lam, o + D.nx) : (D.zero_xy ? 0.0f : c);
-    const float zn = (k + 1 < D.nz) ? field<TRIAL>(f, d, lam, o + (size_t)D.nx * D.ny) : (D.zero_z ? 0.0f : c);
-    gx = (xn - c) * D.ihx; gy = (yn - c) * D.ihy; gz = (zn - c) * D.ihz;
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
 }
 
-constexpr int TV_BX = 32, TV_BY = 4, TV_BZ = 2;
+// |grad u|_delta = n2 * rsqrt(n2) (n2 >= delta^2 > 0, or exactly 0 on a flat field with delta = 0);
+// inv = 1/|grad u|_delta for p = grad u * inv.
+__device__ __forceinline__ float grad_norm(float gx, float gy, float gz, float delta2, float &inv)
+{
+    const float n2 = fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, delta2)));
+    inv = rsqrt_ftz(n2);
+    return n2 > 0.0f ? n2 * inv : 0.0f;
+}
 
-// partial sums, row 0: sum |grad f|_delta, row 1: sum (f-g)^2, row 2: sum d^2 (GRAD only)
-// GRAD: also writes d.   TRIAL: evaluates the field f - lam*dir instead of f.
-template <bool GRAD, bool TRIAL>
-__global__ void __launch_bounds__(TV_BX *TV_BY *TV_BZ)
-tv_pass_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
-               const float *__restrict__ g, const double *__restrict__ lam_ptr, float beta, float delta2,
-               float *__restrict__ d_out, double *__restrict__ partials, int stride)
+// Work decomposition of both passes: a WARP owns a tile of 32 (x, the lanes) x TV_R (y, in
+// registers) voxels and marches through `zc` slices, carrying u(.,.,k+1) and p_z(.,.,k-1) in
+// registers, so every voxel's value and p = grad u/|grad u| are computed ONCE per pass:
+//   u(i+1,j,k)   is a warp shuffle; the values lane 31 needs (column i0+32) are loaded together
+//                by lanes 0..TV_R and shuffled into place,
+//   u(i,j+1,k)   is the register of the next row (one extra value-only row per tile),
+//   p_y(i,j-1,k) is the previous row's register (one extra row j0-1, p_y only),
+//   p_x(i-1,j,k) is a warp shuffle; the TV_R values lane 0 needs (column i0-1) are computed
+//                together in lanes 0..TV_R-1 and shuffled into place.
+// No shared memory and no barrier inside the march.  Loads run two slices ahead of their use
+// (three register stages, rotated by unrolling the march by three).  Indices are clamped into the
+// grid instead of predicated: a clamped neighbour equals the voxel itself, so the boundary rule is
+// one multiplier (0 or 1) per axis, and ragged tiles compute on duplicates and mask their stores
+// and sums.  Energy terms: fp32 over the TV_R rows of a slice, then fp64 per thread over the
+// march, then the fixed-order block / grid reduction of reduce.cuh.
+constexpr int TV_R = 4, TV_WPB = 4;
+
+struct TvTile {
+    int lane, i0, j0, k0, k1, ks;
+    bool hy, hx;
+    float xm, bz;
+    unsigned ro[TV_R + 1];   // element offsets of rows j0 .. j0+TV_R inside a slice (clamped)
+    bool rv[TV_R];           // voxel (i, j0+r) exists
+    float ym[TV_R];          // multiplier of the y-neighbour of row r
+    unsigned hro;            // row j0-1, this lane's column (p_y only)
+    unsigned lco;            // lanes <= TV_R: voxel (i0-1, j0+lane) (p_x for lanes < TV_R; lane+1 is the y-neighbour)
+    float lym;
+    unsigned rco;            // lanes <= TV_R: voxel (i0+32, j0-1+lane) (value only)
+    size_t plane;
+};
+
+__device__ __forceinline__ TvTile tv_tile(const TvDims &D, int zc)
+{
+    TvTile T;
+    T.lane = threadIdx.x;
+    T.i0 = blockIdx.x * 32;
+    const int i = T.i0 + T.lane;
+    T.j0 = (blockIdx.y * TV_WPB + threadIdx.y) * TV_R;
+    T.k0 = blockIdx.z * zc;
+    T.k1 = min(T.k0 + zc, D.nz);
+    T.ks = T.k0 > 0 ? T.k0 - 1 : 0;
+    T.hy = T.j0 > 0;
+    T.hx = T.i0 > 0;
+    const float bxy = D.zero_xy ? 0.0f : 1.0f;      // out-of-grid neighbour = b * own value
+    T.bz = D.zero_z ? 0.0f : 1.0f;
+    T.xm = (i + 1 < D.nx) ? 1.0f : bxy;
+    const int ic = min(i, D.nx - 1);
+#pragma unroll
+    for (int r = 0; r <= TV_R; ++r) T.ro[r] = (unsigned)(min(T.j0 + r, D.ny - 1) * D.nx + ic);
+#pragma unroll
+    for (int r = 0; r < TV_R; ++r) {
+        T.rv[r] = i < D.nx && T.j0 + r < D.ny;
+        T.ym[r] = (T.j0 + r + 1 < D.ny) ? 1.0f : bxy;
+    }
+    T.hro = (unsigned)(min(max(T.j0 - 1, 0), D.ny - 1) * D.nx + ic);
+    const int lj = T.j0 + min(T.lane, TV_R);
+    T.lco = (unsigned)(min(lj, D.ny - 1) * D.nx + max(T.i0 - 1, 0));
+    T.lym = (lj + 1 < D.ny) ? 1.0f : bxy;
+    const int rj = min(max(T.j0 - 1 + min(T.lane, TV_R), 0), D.ny - 1);
+    T.rco = (unsigned)(rj * D.nx + min(T.i0 + 32, D.nx - 1));
+    T.plane = (size_t)D.nx * D.ny;
+    return T;
+}
+
+// u(i+1, row) for every lane: the next lane's value, lane 31 takes the right-column value held by
+// lane `src` (a clamped duplicate of its own value at the grid's edge)
+__device__ __forceinline__ float right_neighbour(float own, float rcol, int src, int lane)
+{
+    const float v = __shfl_down_sync(0xffffffffu, own, 1);
+    const float e = __shfl_sync(0xffffffffu, rcol, src);
+    return lane == 31 ? e : v;
+}
+
+// Gradient pass at u = f:  d = -div p + beta (f - g);  out[0] = sum |grad f|_delta,
+// out[1] = sum (f-g)^2, out[2] = sum d^2.  FIRST: f is g itself (first descent step): no g loads.
+template <bool FIRST>
+__global__ void __launch_bounds__(32 * TV_WPB)
+tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ g, float beta, float delta2,
+               float *__restrict__ d_out, int zc, double *__restrict__ partials, int stride,
+               unsigned int *__restrict__ counter, double *__restrict__ out)
 {
     __shared__ double slot[32];
-    const int i = blockIdx.x * TV_BX + threadIdx.x;
-    const int j = blockIdx.y * TV_BY + threadIdx.y;
-    const int k = blockIdx.z * TV_BZ + threadIdx.z;
-    const float lam = TRIAL ? (float)lam_ptr[0] : 0.0f;
+    const TvTile T = tv_tile(D, zc);
+    const float *pk = f + T.ks * T.plane;                                    // slice k
+    const float *p2 = f + min(T.ks + 1, D.nz - 1) * T.plane;                 // slice k+2 (after the first advance)
+    const float *pg = g + min(T.ks + 1, D.nz - 1) * T.plane;
+    float *pd = d_out + T.ks * T.plane;
+    // three stages: slice k, k+1, k+2
+    float A[TV_R + 1], B[TV_R + 1], C[TV_R + 1], GA[TV_R], GB[TV_R], GC[TV_R];
+    float hA, hB, hC = 0.0f, lA, lB, lC = 0.0f, rA, rB, rC = 0.0f;
+    float pzp[TV_R];
+#pragma unroll
+    for (int r = 0; r <= TV_R; ++r) { A[r] = __ldg(pk + T.ro[r]); B[r] = __ldg(p2 + T.ro[r]); C[r] = 0.0f; }
+#pragma unroll
+    for (int r = 0; r < TV_R; ++r) {
+        GA[r] = FIRST ? 0.0f : __ldg(g + T.ks * T.plane + T.ro[r]);
+        GB[r] = FIRST ? 0.0f : __ldg(pg + T.ro[r]);
+        GC[r] = 0.0f;
+        pzp[r] = 0.0f;
+    }
+    hA = __ldg(pk + T.hro); hB = __ldg(p2 + T.hro);
+    lA = __ldg(pk + T.lco); lB = __ldg(p2 + T.lco);
+    rA = __ldg(pk + T.rco); rB = __ldg(p2 + T.rco);
     double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
-    if (i < D.nx && j < D.ny && k < D.nz) {
-        float c, gx, gy, gz;
-        grad3<TRIAL>(D, f, dir, lam, i, j, k, c, gx, gy, gz);
-        const float nrm2 = fmaf(gx, gx, fmaf(gy, gy, fmaf(gz, gz, delta2)));
-        const float nrm = sqrtf(nrm2);
-        e_tv = nrm;
-        const size_t o = ((size_t)k * D.ny + j) * D.nx + i;
-        const float r = g ? c - __ldg(g + o) : 0.0f;
-        e_q = (double)r * r;
-        if (GRAD) {
-            const float inv = 1.0f / nrm;
-            float div = (gx * D.ihx + gy * D.ihy + gz * D.ihz) * inv;
-            float c2, ax, ay, az;
-            if (i > 0) {
-                grad3<false>(D, f, nullptr, 0.f, i - 1, j, k, c2, ax, ay, az);
-                div -= ax * D.ihx * rsqrtf(fmaf(ax, ax, fmaf(ay, ay, fmaf(az, az, delta2))));
-            }
-            if (j > 0) {
-                grad3<false>(D, f, nullptr, 0.f, i, j - 1, k, c2, ax, ay, az);
-                div -= ay * D.ihy * rsqrtf(fmaf(ax, ax, fmaf(ay, ay, fmaf(az, az, delta2))));
-            }
-            if (k > 0) {
-                grad3<false>(D, f, nullptr, 0.f, i, j, k - 1, c2, ax, ay, az);
-                div -= az * D.ihz * rsqrtf(fmaf(ax, ax, fmaf(ay, ay, fmaf(az, az, delta2))));
-            }
-            const float dd = fmaf(beta, r, -div);
-            d_out[o] = dd;
-            e_d = (double)dd * dd;
+
+    auto step = [&](int k, float (&c)[TV_R + 1], float (&cn)[TV_R + 1], float (&cnn)[TV_R + 1], float (&gc)[TV_R],
+                    float (&gnn)[TV_R], float hc, float hcn, float &hcnn, float lc, float lcn, float &lcnn, float rc,
+                    float &rcnn) {
+        // two slices ahead (clamped at the top of the grid: those values are never used)
+        if (k + 2 < D.nz) { p2 += T.plane; pg += T.plane; }
+#pragma unroll
+        for (int r = 0; r <= TV_R; ++r) cnn[r] = __ldg(p2 + T.ro[r]);
+        if (!FIRST) {
+#pragma unroll
+            for (int r = 0; r < TV_R; ++r) gnn[r] = __ldg(pg + T.ro[r]);
         }
+        hcnn = __ldg(p2 + T.hro); lcnn = __ldg(p2 + T.lco); rcnn = __ldg(p2 + T.rco);
+        const bool ztop = k + 1 >= D.nz;
+        float px[TV_R], py[TV_R], pz[TV_R], nrm[TV_R];
+#pragma unroll
+        for (int r = 0; r < TV_R; ++r) {
+            const float xn = right_neighbour(c[r], rc, r + 1, T.lane);
+            const float zn = ztop ? T.bz * c[r] : cn[r];
+            const float gx = fmaf(xn, T.xm, -c[r]) * D.ihx, gy = fmaf(c[r + 1], T.ym[r], -c[r]) * D.ihy,
+                        gz = (zn - c[r]) * D.ihz;
+            float inv;
+            nrm[r] = grad_norm(gx, gy, gz, delta2, inv);
+            px[r] = gx * inv; py[r] = gy * inv; pz[r] = gz * inv;
+        }
+        float hpy = 0.0f, hpx = 0.0f;
+        if (T.hy) {                                      // warp-uniform: row j0-1, p_y only
+            const float xn = right_neighbour(hc, rc, 0, T.lane);
+            const float zn = ztop ? T.bz * hc : hcn;
+            const float gx = fmaf(xn, T.xm, -hc) * D.ihx, gy = (c[0] - hc) * D.ihy, gz = (zn - hc) * D.ihz;
+            float inv;
+            grad_norm(gx, gy, gz, delta2, inv);
+            hpy = gy * inv;
+        }
+        if (T.hx) {                                      // warp-uniform: column i0-1, p_x only, rows in lanes 0..TV_R-1
+            // its x-neighbour is lane 0's voxel of the same row, its y-neighbour the next lane's voxel
+            float xn = 0.0f;
+#pragma unroll
+            for (int r = 0; r < TV_R; ++r) {
+                const float v = __shfl_sync(0xffffffffu, c[r], 0);
+                if (T.lane == r) xn = v;
+            }
+            const float yn = __shfl_down_sync(0xffffffffu, lc, 1);
+            const float zn = ztop ? T.bz * lc : lcn;
+            const float gx = (xn - lc) * D.ihx, gy = fmaf(yn, T.lym, -lc) * D.ihy, gz = (zn - lc) * D.ihz;
+            float inv;
+            grad_norm(gx, gy, gz, delta2, inv);
+            hpx = gx * inv;
+        }
+        const bool emit = k >= T.k0;                     // the slice before the chunk only supplies p_z
+        float s_tv = 0.0f, s_q = 0.0f, s_d = 0.0f;
+#pragma unroll
+        for (int r = 0; r < TV_R; ++r) {
+            float left = __shfl_up_sync(0xffffffffu, px[r], 1);
+            const float edge = __shfl_sync(0xffffffffu, hpx, r);
+            if (T.lane == 0) left = edge;
+            const float up = r > 0 ? py[r > 0 ? r - 1 : 0] : hpy;
+            const float div = (px[r] - left) * D.ihx + (py[r] - up) * D.ihy + (pz[r] - pzp[r]) * D.ihz;
+            const float res = FIRST ? 0.0f : c[r] - gc[r];
+            const float dd = FIRST ? -div : fmaf(beta, res, -div);
+            if (emit && T.rv[r]) {
+                pd[T.ro[r]] = dd;
+                s_tv += nrm[r];
+                if (!FIRST) s_q = fmaf(res, res, s_q);
+                s_d = fmaf(dd, dd, s_d);
+            }
+            pzp[r] = pz[r];
+        }
+        e_tv += (double)s_tv; e_d += (double)s_d;
+        if (!FIRST) e_q += (double)s_q;
+        pk += T.plane; pd += T.plane;
+    };
+
+    for (int k = T.ks; k < T.k1; k += 3) {
+        step(k, A, B, C, GA, GC, hA, hB, hC, lA, lB, lC, rA, rC);
+        if (k + 1 >= T.k1) break;
+        step(k + 1, B, C, A, GB, GA, hB, hC, hA, lB, lC, lA, rB, rA);
+        if (k + 2 >= T.k1) break;
+        step(k + 2, C, A, B, GC, GB, hC, hA, hB, lC, lA, lB, rC, rB);
     }
-    const int blk = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
-    double s0 = block_sum(e_tv, slot);
-    if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) partials[blk] = s0;
-    double s1 = block_sum(e_q, slot);
-    if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) partials[stride + blk] = s1;
-    if (GRAD) {
-        double s2 = block_sum(e_d, slot);
-        if (threadIdx.x == 0 && threadIdx.y == 0 && threadIdx.z == 0) partials[2 * stride + blk] = s2;
-    }
+    double s[3];
+    s[0] = block_sum(e_tv, slot);
+    s[1] = block_sum(e_q, slot);
+    s[2] = block_sum(e_d, slot);
+    publish_and_finalize<3>(s, 3, partials, stride, counter, out, slot);
 }
 
-// f_out = f - lam * d  (optionally clipped at 0: Algorithm A1 step 3, L149)
-__global__ void tv_update_kernel(size_t n, const float *__restrict__ f, const float *__restrict__ d,
-                                 const double *__restrict__ lam_ptr, int clip, float *__restrict__ out)
+// Energy pass at u = f - lam*dir (TRIAL) or u = f:  out[0] = sum |grad u|_delta and, when rows == 2,
+// out[1] = sum (u-g)^2.  Same warp tiles and march; nothing but u(i+1) is exchanged between voxels.
+template <bool TRIAL>
+__global__ void __launch_bounds__(32 * TV_WPB)
+tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
+                 const float *__restrict__ g, float lam, float delta2, int zc, int rows,
+                 double *__restrict__ partials, int stride, unsigned int *__restrict__ counter,
+                 double *__restrict__ out)
 {
-    const float lam = (float)lam_ptr[0];
+    __shared__ double slot[32];
+    const TvTile T = tv_tile(D, zc);
+    const bool hasg = g != nullptr;
+    const size_t ok = T.k0 * T.plane;
+    size_t o2 = min(T.k0 + 1, D.nz - 1) * T.plane;                // slice k+2 (after the first advance)
+    float A[TV_R + 1], B[TV_R + 1], C[TV_R + 1], GA[TV_R], GB[TV_R], GC[TV_R];
+    float rA, rB, rC = 0.0f;
+#pragma unroll
+    for (int r = 0; r <= TV_R; ++r) {
+        A[r] = field<TRIAL>(f, dir, lam, ok + T.ro[r]);
+        B[r] = field<TRIAL>(f, dir, lam, o2 + T.ro[r]);
+        C[r] = 0.0f;
+    }
+#pragma unroll
+    for (int r = 0; r < TV_R; ++r) {
+        GA[r] = hasg ? __ldg(g + ok + T.ro[r]) : 0.0f;
+        GB[r] = hasg ? __ldg(g + o2 + T.ro[r]) : 0.0f;
+        GC[r] = 0.0f;
+    }
+    rA = field<TRIAL>(f, dir, lam, ok + T.rco); rB = field<TRIAL>(f, dir, lam, o2 + T.rco);
+    double e_tv = 0.0, e_q = 0.0;
+
+    auto step = [&](int k, float (&c)[TV_R + 1], float (&cn)[TV_R + 1], float (&cnn)[TV_R + 1], float (&gc)[TV_R],
+                    float (&gnn)[TV_R], float rc, float &rcnn) {
+        if (k + 2 < D.nz) o2 += T.plane;
+#pragma unroll
+        for (int r = 0; r <= TV_R; ++r) cnn[r] = field<TRIAL>(f, dir, lam, o2 + T.ro[r]);
+        if (hasg) {
+#pragma unroll
+            for (int r = 0; r < TV_R; ++r) gnn[r] = __ldg(g + o2 + T.ro[r]);
+        }
+        rcnn = field<TRIAL>(f, dir, lam, o2 + T.rco);
+        const bool ztop = k + 1 >= D.nz;
+        float s_tv = 0.0f, s_q = 0.0f;
+#pragma unroll
+        for (int r = 0; r < TV_R; ++r) {
+            const float xn = right_neighbour(c[r], rc, r + 1, T.lane);
+            const float zn = ztop ? T.bz * c[r] : cn[r];
+            const float gx = fmaf(xn, T.xm, -c[r]) * D.ihx, gy = fmaf(c[r + 1], T.ym[r], -c[r]) * D.ihy,
+                        gz = (zn - c[r]) * D.ihz;
+            float inv;
+            const float nrm = grad_norm(gx, gy, gz, delta2, inv);
+            const float res = c[r] - gc[r];
+            if (T.rv[r]) { s_tv += nrm; s_q = fmaf(res, res, s_q); }
+        }
+        e_tv += (double)s_tv; e_q += (double)s_q;
+    };
+
+    for (int k = T.k0; k < T.k1; k += 3) {
+        step(k, A, B, C, GA, GC, rA, rC);
+        if (k + 1 >= T.k1) break;
+        step(k + 1, B, C, A, GB, GA, rB, rA);
+        if (k + 2 >= T.k1) break;
+        step(k + 2, C, A, B, GC, GB, rC, rB);
+    }
+    double s[2];
+    s[0] = block_sum(e_tv, slot);
+    s[1] = hasg ? block_sum(e_q, slot) : 0.0;
+    publish_and_finalize<2>(s, rows, partials, stride, counter, out, slot);
+}
+
+// out = f - lam * d  (optionally clipped at 0: Algorithm A1 step 3, L149); d == NULL: out = f.
+// Plain loads and no __restrict__: out may be f itself (each thread reads an element, then writes it).
+template <typename V>
+__global__ void tv_update_kernel(size_t n, const V *f, const V *d, float lam, int clip, V *out);
+
+template <>
+__global__ void tv_update_kernel<float>(size_t n, const float *f, const float *d, float lam, int clip, float *out)
+{
     for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
-        float v = fmaf(-lam, d[o], f[o]);
+        float v = d ? fmaf(-lam, d[o], f[o]) : f[o];
         out[o] = (clip && v < 0.0f) ? 0.0f : v;
     }
 }
 
-__global__ void clip_copy_kernel(size_t n, const float *__restrict__ in, int clip, float *__restrict__ out)
+template <>
+__global__ void tv_update_kernel<float4>(size_t n, const float4 *f, const float4 *d, float lam, int clip, float4 *out)
 {
     for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
-        float v = in[o];
-        out[o] = (clip && v < 0.0f) ? 0.0f : v;
+        float4 v = f[o];
+        if (d) {
+            const float4 w = d[o];
+            v.x = fmaf(-lam, w.x, v.x); v.y = fmaf(-lam, w.y, v.y); v.z = fmaf(-lam, w.z, v.z); v.w = fmaf(-lam, w.w, v.w);
+        }
+        if (clip) {     // (v < 0) ? 0 : v, so that -0 and NaN pass through like the scalar path
+            v.x = v.x < 0.0f ? 0.0f : v.x; v.y = v.y < 0.0f ? 0.0f : v.y;
+            v.z = v.z < 0.0f ? 0.0f : v.z; v.w = v.w < 0.0f ? 0.0f : v.w;
+        }
+        out[o] = v;
     }
 }
 
-static dim3 tv_grid(const TvDims &D)
+// z-slices per block: long marches amortise the halo slice and the block reduction; short ones
+// keep at least ~8 blocks per SM in flight on small volumes.
+static int tv_zchunk(const cbct_geometry *g, const TvDims &D)
 {
-    return dim3((D.nx + TV_BX - 1) / TV_BX, (D.ny + TV_BY - 1) / TV_BY, (D.nz + TV_BZ - 1) / TV_BZ);
+    const int bxy = ((D.nx + 31) / 32) * ((D.ny + TV_R * TV_WPB - 1) / (TV_R * TV_WPB));
+    int zc = 32;
+    while (zc > 4 && (long)bxy * ((D.nz + zc - 1) / zc) < 8L * g->sm_count) zc >>= 1;
+    return zc;
+}
+
+static dim3 tv_grid(const TvDims &D, int zc)
+{
+    return dim3((D.nx + 31) / 32, (D.ny + TV_R * TV_WPB - 1) / (TV_R * TV_WPB), (D.nz + zc - 1) / zc);
+}
+
+static cbct_status launch_update(const cbct_geometry *g, size_t n, const float *f, const float *d, float lam, int clip,
+                                 float *out, cudaStream_t st)
+{
+    const bool vec = n % 4 == 0 && ((uintptr_t)f % 16 == 0) && ((uintptr_t)out % 16 == 0) && (!d || (uintptr_t)d % 16 == 0);
+    const int blocks = g->sm_count * 8;
+    if (vec)
+        tv_update_kernel<float4><<<blocks, 256, 0, st>>>(n / 4, reinterpret_cast<const float4 *>(f),
+                                                         reinterpret_cast<const float4 *>(d), lam, clip,
+                                                         reinterpret_cast<float4 *>(out));
+    else
+        tv_update_kernel<float><<<blocks, 256, 0, st>>>(n, f, d, lam, clip, out);
+    CBCT_LAUNCH_CHECK(g);
+    return CBCT_OK;
 }
 
 cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float *d_f, double delta,
                              double *d_out, cudaStream_t st)
 {
     TvDims D = tv_dims(L);
-    dim3 gr = tv_grid(D), b(TV_BX, TV_BY, TV_BZ);
-    const int nblk = gr.x * gr.y * gr.z;
-    if (nblk > g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
+    const int zc = tv_zchunk(g, D);
+    dim3 gr = tv_grid(D, zc), b(32, TV_WPB);
+    if ((size_t)gr.x * gr.y * gr.z > (size_t)g->partials_stride)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     StageTimer t(g, st, ST_REDUCE);
-    tv_pass_kernel<false, false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, nullptr, 0.f, (float)(delta * delta),
-                                                  nullptr, g->d_partials, g->partials_stride);
-    CBCT_LAUNCH_CHECK(g);
-    finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 1, g->partials_stride, d_out);
+    tv_energy_kernel<false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, 0.0f, (float)(delta * delta), zc, 1,
+                                              g->d_partials, g->partials_stride, g->d_counter, d_out);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
 
-// Host-driven control loop: every trial reads two fp64 sums back (one stream sync per
-// pass).  Scalars: d_scalars[0..2] = sums, d_scalars[4] = trial step.
+// Host-sequenced control loop (the Armijo test needs two global sums per trial).  The gradient pass
+// and the first trial (its step 1/beta is known beforehand) are queued back to back and read with
+// ONE stream synchronisation; the accepted update carries the non-negativity truncation when the
+// stopping rule already says it is the last.  Scalars: d_scalars[0..2] gradient-pass sums,
+// d_scalars[4..5] trial sums.
 cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,
                         cudaStream_t st)
@@ -151,18 +398,18 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     (void)sync_report;
     cbct_tv_report r = {0, 0, 0.0, 0.0};
     const size_t n = L.nvox;
-    const int cp_blocks = g->sm_count * 8;
-    if (w <= 0.0) {
+    cbct_status s;
+    if (w <= 0.0 || tp.max_inner == 0) {
         StageTimer t(g, st, ST_TV_UPDATE);
-        clip_copy_kernel<<<cp_blocks, 256, 0, st>>>(n, d_g, nonneg, d_f);
-        CBCT_LAUNCH_CHECK(g);
+        if ((s = launch_update(g, n, d_g, nullptr, 0.0f, nonneg, d_f, st)) != CBCT_OK) return s;
         if (rep) *rep = r;
         return CBCT_OK;
     }
     TvDims D = tv_dims(L);
-    dim3 gr = tv_grid(D), b(TV_BX, TV_BY, TV_BZ);
-    const int nblk = gr.x * gr.y * gr.z, S = g->partials_stride;
-    if (nblk > S) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
+    const int zc = tv_zchunk(g, D);
+    dim3 gr = tv_grid(D, zc), b(32, TV_WPB);
+    const int S = g->partials_stride;
+    if ((size_t)gr.x * gr.y * gr.z > (size_t)S) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     const double beta = 1.0 / w, N = (double)n;
     const float delta2 = (float)(tp.eps_delta * tp.eps_delta);
     double *ds = g->d_scalars, *hs = g->h_scalars;
@@ -171,66 +418,54 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     float *bufs[2] = {d_f, L.d_f2};
     int which = 0;
     double E0 = 0.0;
-    bool have_E0 = false;
+    bool have_E0 = false, clipped = false;
     for (int it = 0; it < tp.max_inner; ++it) {
         {
             StageTimer t(g, st, ST_TV_GRAD);
-            tv_pass_kernel<true, false><<<gr, b, 0, st>>>(D, cur, nullptr, d_g, nullptr, (float)beta, delta2, L.d_d,
-                                                         g->d_partials, S);
+            if (cur == d_g) tv_grad_kernel<true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            else tv_grad_kernel<false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
             CBCT_LAUNCH_CHECK(g);
         }
-        {
-            StageTimer t(g, st, ST_REDUCE);
-            finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 3, S, ds);
-            CBCT_LAUNCH_CHECK(g);
-        }
-        CBCT_CUDA(cudaMemcpyAsync(hs, ds, 3 * sizeof(double), cudaMemcpyDeviceToHost, st));
-        CBCT_CUDA(cudaStreamSynchronize(st));
-        if (!have_E0) { E0 = hs[0] / N + 0.5 * beta * hs[1] / N; r.e_first = r.e_last = E0; have_E0 = true; }
-        const double Dm = hs[2] / N;
-        double lam = 1.0 / beta, Enew = E0;
+        double lam = 1.0 / beta, Enew = E0, Dm = 0.0;
         bool accepted = false;
         for (int bt = 0; bt <= tp.max_backtracks; ++bt) {
-            hs[4] = lam;
-            CBCT_CUDA(cudaMemcpyAsync(ds + 4, hs + 4, sizeof(double), cudaMemcpyHostToDevice, st));
             {
                 StageTimer t(g, st, ST_TV_TRIAL);
-                tv_pass_kernel<false, true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, ds + 4, (float)beta, delta2, nullptr,
-                                                             g->d_partials, S);
+                tv_energy_kernel<true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, (float)lam, delta2, zc, 2, g->d_partials, S,
+                                                         g->d_counter, ds + 4);
                 CBCT_LAUNCH_CHECK(g);
             }
-            {
-                StageTimer t(g, st, ST_REDUCE);
-                finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, nblk, 2, S, ds);
-                CBCT_LAUNCH_CHECK(g);
-            }
-            CBCT_CUDA(cudaMemcpyAsync(hs, ds, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CBCT_CUDA(cudaMemcpyAsync(hs, ds, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
             CBCT_CUDA(cudaStreamSynchronize(st));
-            Enew = hs[0] / N + 0.5 * beta * hs[1] / N;
+            if (bt == 0) {
+                if (!have_E0) { E0 = hs[0] / N + 0.5 * beta * hs[1] / N; r.e_first = r.e_last = E0; have_E0 = true; }
+                Dm = hs[2] / N;
+            }
+            Enew = hs[4] / N + 0.5 * beta * hs[5] / N;
             ++r.trials;
             if (Enew <= E0 - tp.armijo_c * lam * Dm) { accepted = true; break; }
             lam *= tp.shrink_alpha;
         }
         if (!accepted) break;
-        float *nxt = bufs[which];
+        const double rel = fabs(Enew - E0) / E0;
+        const bool last = rel < tp.rel_tol || it + 1 == tp.max_inner;
+        float *nxt = last ? d_f : bufs[which];      // d_f, d_f2, d_f, ...: never cur unless last (in place is fine)
         which ^= 1;
         {
             StageTimer t(g, st, ST_TV_UPDATE);
-            tv_update_kernel<<<cp_blocks, 256, 0, st>>>(n, cur, L.d_d, ds + 4, 0, nxt);
-            CBCT_LAUNCH_CHECK(g);
+            if ((s = launch_update(g, n, cur, L.d_d, (float)lam, last ? nonneg : 0, nxt, st)) != CBCT_OK) return s;
         }
         cur = nxt;
+        clipped = last;
         ++r.inner_iters;
-        const double rel = fabs(Enew - E0) / E0;
         E0 = Enew;
         r.e_last = Enew;
-        if (rel < tp.rel_tol) break;
+        if (last) break;
     }
-    // result to d_f, with the non-negativity truncation
-    if (cur != d_f || nonneg) {
+    // result to d_f, with the non-negativity truncation, if the last update did not already do both
+    if (cur != d_f || (nonneg && !clipped)) {
         StageTimer t(g, st, ST_TV_UPDATE);
-        clip_copy_kernel<<<cp_blocks, 256, 0, st>>>(n, cur, nonneg, d_f);
-        CBCT_LAUNCH_CHECK(g);
+        if ((s = launch_update(g, n, cur, nullptr, 0.0f, nonneg, d_f, st)) != CBCT_OK) return s;
     }
     if (rep) *rep = r;
     return CBCT_OK;
