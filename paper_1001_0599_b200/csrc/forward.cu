@@ -55,17 +55,57 @@ __global__ void stage_volume_kernel(const float *__restrict__ in, float *__restr
     }
 }
 
+// Mirror-packed staging (nmir == 2): stage2[i+PM][j+PM][kk] = ( f(i,j,k), f(i,j,nz-1-k) ), k = kk - PZ, for
+// kk in [0, nz/2 + 2 PZ); a component whose k falls outside the grid is 0.  A ray of the lower detector half and
+// its mirror image then read their two cells with ONE 8-byte load at the same offset.  (The entries with
+// k >= nz/2 repeat pairs with the roles swapped: the one-cell slack of the incremental cell tracking may touch
+// k = nz/2 with weight 0.)  Every element of the copy, margins included, is written here.
+__global__ void stage_volume_packed_kernel(const float *__restrict__ in, float2 *__restrict__ stage, int nx, int ny,
+                                           int nz, int istride, int jstride)
+{
+    __shared__ float lo[32][33], hi[32][33];
+    const int j = blockIdx.z;
+    const int i = blockIdx.x * 32 + threadIdx.x, kk0 = blockIdx.y * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int k = kk0 + r - PAD_Z, km = nz - 1 - k;
+        float a = 0.0f, b = 0.0f;
+        if (i < nx) {
+            if (k >= 0 && k < nz) a = __ldg(in + ((size_t)k * ny + j) * nx + i);
+            if (km >= 0 && km < nz) b = __ldg(in + ((size_t)km * ny + j) * nx + i);
+        }
+        lo[r][threadIdx.x] = a; hi[r][threadIdx.x] = b;
+    }
+    __syncthreads();
+    const int kk = kk0 + threadIdx.x, i0 = blockIdx.x * 32;
+    for (int r = threadIdx.y; r < 32; r += blockDim.y) {
+        const int ii = i0 + r;
+        if (ii < nx && kk < jstride)
+            stage[(size_t)(ii + PAD_M) * istride + (size_t)(j + PAD_M) * jstride + kk] =
+                make_float2(lo[threadIdx.x][r], hi[threadIdx.x][r]);
+    }
+}
+
 constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x 8 detector columns
 
+// One staged cell: a voxel value (M == 1) or the mirror pair (f(k), f(nz-1-k)) (M == 2).
+template <int M> struct StageCell { typedef float type; };
+template <> struct StageCell<2> { typedef float2 type; };
+__device__ __forceinline__ float cell_lo(float c) { return c; }
+__device__ __forceinline__ float cell_lo(float2 c) { return c.x; }
+__device__ __forceinline__ float cell_hi(float c) { return c; }
+__device__ __forceinline__ float cell_hi(float2 c) { return c.y; }
+
 // R = quarter-turn views per thread (1 or 4), M = 2 when the thread also walks the mirror image
-// z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again.  MODE as in
-// launch_forward.
+// z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again, and -- the staged
+// copy being mirror-packed -- the same loads.  MODE as in launch_forward.
 template <int R, int M, int MODE>
 __global__ void __launch_bounds__(FWD_BV *FWD_BU, 2)
-forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU *__restrict__ rayu,
+forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
                unsigned int *__restrict__ counter, double *__restrict__ sum_out)
 {
+    typedef typename StageCell<M>::type cell;
+    const cell *__restrict__ stage = reinterpret_cast<const cell *>(stage_v);
     __shared__ double slot[32];
     const int iv = blockIdx.y * FWD_BV + threadIdx.x;
     const int iu = blockIdx.x * FWD_BU + threadIdx.y;
@@ -105,13 +145,10 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
             int ci = r.drive ? jm : s_lo, cj = r.drive ? s_lo : jm;
             int si = r.drive ? 0 : 1, sj = r.drive ? 1 : 0;
             int mi = r.drive ? dj : 0, mj = r.drive ? 0 : dj;
-            const float *p[R * M];
-            int drow[R], dcol[R];
+            int off[R], drow[R], dcol[R];       // element offsets into the staged copy (< 2^31, checked at create)
 #pragma unroll
             for (int q = 0; q < R; ++q) {
-                const int o = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride;
-                p[q] = stage + o + kk;
-                if (M == 2) p[R + q] = stage + o + (P.nzP - 1 - kk);
+                off[q] = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride + kk;
                 drow[q] = si * P.istride + sj * P.jstride;
                 dcol[q] = mi * P.istride + mj * P.jstride;
                 int t = ci; ci = P.nx - 1 - cj; cj = t;
@@ -128,32 +165,29 @@ forward_kernel(const LevelParams P, const float *__restrict__ stage, const RayU 
                 const float wl = 1.0f - hi;
                 const int zc = cz ? dk : 0;
                 // issue every load of the step before the first use: the loop is bound by load latency otherwise
-                const float *pc[R * M];
-                float va[R * M], vc[R * M];
+                int offc[R];
+                cell va[R], vc[R];
+#pragma unroll
+                for (int q = 0; q < R; ++q) offc[q] = off[q] + (cy ? dcol[q] : 0) + zc;
+#pragma unroll
+                for (int q = 0; q < R; ++q) { va[q] = __ldg(stage + off[q]); vc[q] = __ldg(stage + offc[q]); }
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
-                    const int dc = cy ? dcol[q] : 0;
-                    pc[q] = p[q] + (dc + zc);
-                    if (M == 2) pc[R + q] = p[R + q] + (dc - zc);
+                    acc[q] = fmaf(wl, cell_lo(vc[q]), fmaf(lo, cell_lo(va[q]), acc[q]));
+                    if (M == 2) acc[R + q] = fmaf(wl, cell_hi(vc[q]), fmaf(lo, cell_hi(va[q]), acc[R + q]));
                 }
-#pragma unroll
-                for (int q = 0; q < R * M; ++q) { va[q] = __ldg(p[q]); vc[q] = __ldg(pc[q]); }
-#pragma unroll
-                for (int q = 0; q < R * M; ++q) acc[q] = fmaf(wl, vc[q], fmaf(lo, va[q], acc[q]));
                 if (hi > lo) {      // both planes crossed inside this slab, at different parameters (rare): a third cell
                     const float wm = hi - lo;
                     const bool yfirst = sy < sz;
 #pragma unroll
                     for (int q = 0; q < R; ++q) {
-                        acc[q] = fmaf(wm, __ldg(p[q] + (yfirst ? dcol[q] : dk)), acc[q]);
-                        if (M == 2) acc[R + q] = fmaf(wm, __ldg(p[R + q] + (yfirst ? dcol[q] : -dk)), acc[R + q]);
+                        const cell vm = __ldg(stage + off[q] + (yfirst ? dcol[q] : dk));
+                        acc[q] = fmaf(wm, cell_lo(vm), acc[q]);
+                        if (M == 2) acc[R + q] = fmaf(wm, cell_hi(vm), acc[R + q]);
                     }
                 }
 #pragma unroll
-                for (int q = 0; q < R; ++q) {
-                    p[q] = pc[q] + drow[q];
-                    if (M == 2) p[R + q] = pc[R + q] + drow[q];
-                }
+                for (int q = 0; q < R; ++q) off[q] = offc[q] + drow[q];
                 if (cy) nexty += sgny;
                 if (cz) nextz += sgnz;
                 d += 1.0f;
@@ -240,7 +274,7 @@ count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double 
 
 template <int R, int M>
 static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode,
-                                const float *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq)
+                                const void *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq)
 {
     if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
     else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
@@ -265,8 +299,15 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     }
     {
         StageTimer t(g, st, ST_TRANSPOSE);
-        dim3 tb(32, 8), tg((P.nx + 31) / 32, (P.nz + 31) / 32, P.ny);
-        stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nz, P.istride, P.jstride);
+        dim3 tb(32, 8);
+        if (P.nmir == 2) {
+            dim3 tg((P.nx + 31) / 32, (P.nzP + 31) / 32, P.ny);
+            stage_volume_packed_kernel<<<tg, tb, 0, st>>>(d_vol, reinterpret_cast<float2 *>(L.d_stage), P.nx, P.ny, P.nz,
+                                                         P.istride, P.jstride);
+        } else {
+            dim3 tg((P.nx + 31) / 32, (P.nz + 31) / 32, P.ny);
+            stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nz, P.istride, P.jstride);
+        }
         CBCT_LAUNCH_CHECK(g);
     }
     b = dim3(FWD_BV, FWD_BU);

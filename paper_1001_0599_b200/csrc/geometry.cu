@@ -176,11 +176,6 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.bc_xy = desc->bc_xy; p.bc_z = desc->bc_z;
         L.nvox = (size_t)p.nx * p.ny * p.nz;
         L.nray = (size_t)p.nu * p.nv * p.np;
-        // staged copy [nx+2PM][ny+2PM][nz+2PZ], z fastest
-        p.nyP = p.ny + 2 * PAD_M; p.nzP = p.nz + 2 * PAD_Z;
-        p.jstride = p.nzP; p.istride = p.nyP * p.nzP;
-        L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP;
-        if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }
         // quarter-turn symmetry: square centred in-plane grid, views a and a + np/4 a quarter turn apart
         p.nsym = 1;
         if (g->allow_symmetry && p.nx == p.ny && p.nx % 2 == 0 && L.hx == L.hy && desc->vol_off[0] == 0.0 &&
@@ -194,6 +189,14 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.nbase = p.np / p.nsym;
         // mirror symmetry z -> -z: volume centred in z, detector centred in v, even sizes
         p.nmir = (g->allow_symmetry && desc->vol_off[2] == 0.0 && desc->det_off_v == 0.0 && p.nz % 2 == 0 && p.nv % 2 == 0) ? 2 : 1;
+
+        // staged copy [nx+2PM][ny+2PM][nzP], z fastest: floats with nzP = nz + 2PZ, or (mirror symmetry) float2
+        // pairs (f(k), f(nz-1-k)) with nzP = nz/2 + 2PZ; strides in cells
+        p.nyP = p.ny + 2 * PAD_M;
+        p.nzP = (p.nmir == 2 ? p.nz / 2 : p.nz) + 2 * PAD_Z;
+        p.jstride = p.nzP; p.istride = p.nyP * p.nzP;
+        L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP * p.nmir;
+        if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }
 
         std::vector<RayU> rays;
         std::vector<ViewC> views;
