@@ -37,6 +37,10 @@ from paper_1001_0599_b200 import inputs as I  # noqa: E402
 METRIC = "fbs_iterations_per_second"
 UNIT = "iter/s"
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
+# capture of this command (profiles/r01b_ncu_full_summary.txt); None = not captured for that kernel.
+NCU_DRAM_BYTES_PER_LAUNCH = {"back": None, "forward": None}
+
 
 def _peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -303,27 +307,28 @@ def run_ours(args):
     sec_step = ms_total / 1e3 / K
     per = {name: {"ms_per_step": ms / K, "launches_per_step": c / K, "ms_per_launch": (ms / c if c else None)}
            for name, (ms, c) in stages.items()}
-    # kernel rooflines: P and P^T are ALU/gather bound -- reported as GUPS and as the
-    # fraction of the fp32 issue peak their algorithmic flops reach; the TV passes are HBM bound.
-    fp32_peak = 148 * 128 * 2 * sm_max_mhz * 1e6 / 1e12            # TFLOP/s, FMA = 2
-    FLOP_FWD, FLOP_BACK = 36.0, 52.0                              # algorithmic flops per ray-voxel sample
+    # kernel rooflines.
+    # P and P^T: every ray-voxel sample must pull 4 bytes (a volume cell / a residual value) through an SM's L1
+    # data path: the gather roofline is 128 B/clk/SM x 148 SMs x f_clk = 32 samples/clk/SM.  The TV passes stream
+    # the volume arrays once: HBM roofline (measured copy bandwidth).
+    l1_peak_gbs = 148 * 128 * sm_max_mhz * 1e6 / 1e9
+    first = abs(inner / K - 1.0) < 1e-9          # one descent step per prox call: f is g itself in both passes
+    tv_bytes = {"tv_grad": 8.0 if first else 12.0, "tv_trial": 8.0 if first else 12.0, "tv_update": 12.0}
     kern = {}
-    if per["forward"]["ms_per_launch"]:
-        t = per["forward"]["ms_per_launch"] / 1e3
-        kern["forward"] = {"bound": "alu", "gups": S / t / 1e9, "achieved": S * FLOP_FWD / t / 1e12, "peak": fp32_peak,
-                           "unit": "TFLOP/s", "frac": S * FLOP_FWD / t / 1e12 / fp32_peak}
-    if per["back"]["ms_per_launch"]:
-        t = per["back"]["ms_per_launch"] / 1e3
-        kern["back"] = {"bound": "alu", "gups": S / t / 1e9, "achieved": S * FLOP_BACK / t / 1e12, "peak": fp32_peak,
-                        "unit": "TFLOP/s", "frac": S * FLOP_BACK / t / 1e12 / fp32_peak}
-    for name, bpv in (("tv_grad", 12.0), ("tv_trial", 12.0), ("tv_update", 12.0)):
+    for name in ("forward", "back"):
+        if per[name]["ms_per_launch"]:
+            t = per[name]["ms_per_launch"] / 1e3
+            kern[name] = {"bound": "l1-gather", "gups": S / t / 1e9, "achieved": 4.0 * S / t / 1e9, "peak": l1_peak_gbs,
+                          "unit": "GB/s", "frac": 4.0 * S / t / 1e9 / l1_peak_gbs,
+                          "peak_source": "148 SMs x 128 B/clk x %.0f MHz (DESIGN.md section 7)" % sm_max_mhz}
+    for name, bpv in tv_bytes.items():
         if per[name]["ms_per_launch"]:
             t = per[name]["ms_per_launch"] / 1e3
             kern[name] = {"bound": "hbm", "achieved": bpv * nvox / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                          "frac": bpv * nvox / t / 1e9 / hbm_peak}
+                          "frac": bpv * nvox / t / 1e9 / hbm_peak, "bytes_per_voxel": bpv, "peak_source": peak_src}
     dominant = max((n for n in kern), key=lambda n: per[n]["ms_per_step"])
     roof = dict(kern[dominant])
-    roof.update({"kernel": dominant, "traffic": None, "peak_source": peak_src,
+    roof.update({"kernel": dominant, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dominant),
                  "share_of_step": per[dominant]["ms_per_step"] / sum(v["ms_per_step"] for v in per.values())})
 
     base = cpu_baseline(cfg, y_host)
