@@ -39,7 +39,8 @@ UNIT = "iter/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
 # capture of this command (profiles/r01b_ncu_full_summary.txt); None = not captured for that kernel.
-NCU_DRAM_BYTES_PER_LAUNCH = {"back": None, "forward": None}
+NCU_DRAM_BYTES_PER_LAUNCH = {"back": 143.98e6, "forward": 302.43e6, "tv_grad": 98.07e6, "tv_trial": 137.87e6,
+                             "tv_update": 166.45e6}
 
 
 def _peaks():
