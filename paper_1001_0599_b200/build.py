@@ -40,7 +40,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not (force or stale()):
         return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS
+    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("CBCT_NVCC_EXTRA", "").split()
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]

@@ -4,10 +4,10 @@
 // forward.cu ("sum_theta P^T (P f - Y)").  The paper (L187-L191) rejects the
 // ray-driven scatter because threads would collide on voxels and evaluates the continuum
 // adjoint Eq. 6 instead; here each thread owns voxels and enumerates, per view, every
-// detector ray whose slab segment can cross them: the pixel range comes from the voxel ->
-// detector map of Eq. A6 (L401-L406) applied to the voxel's extent (to first order, with
-// inflated half extents, so one reciprocal serves both detector axes), and each candidate's
-// length is the overlap of three intervals in the slab parameter t in [0,1] -- the same
+// detector ray whose slab segment crosses them: the column range comes from the voxel ->
+// detector map of Eq. A6 (L401-L406) applied to the voxel's in-plane extent (to first order,
+// with inflated half extents), the row range per column is exact (see back_kernel), and each
+// ray's length is the overlap of three intervals in the slab parameter t in [0,1] -- the same
 // fp32 crossing parameters, from the same table entries, as the forward projector's
 // (ray.cuh).  No atomics, fixed order (views ascending, columns, rows) => deterministic.
 //
@@ -47,23 +47,39 @@ __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ 
     else out[ot] = res[0];
 }
 
-constexpr int BK_BZ = 32, BK_BX = 8;       // block: 32 consecutive k (lanes) x 8 consecutive i
+constexpr int BK_BX = 8;       // block: one warp (lanes along z) per i, 8 consecutive i
 
-template <int R, int M>
-__global__ void __launch_bounds__(BK_BZ *BK_BX)
+// Lanes run along z, so a warp shares (i,j) and with it the whole in-plane part of every candidate
+// (uniform branches, broadcast table loads); each thread owns KT voxels k = k0 + lane + 32 t of the column,
+// which spreads that in-plane part over KT times as many voxels (KT = 2 with 80 registers measured best at 256^3:
+// the kernel is bound by load latency, so occupancy is worth more than a longer amortisation).
+//
+// Per (base view, voxel image, detector column iu) the in-plane part gives the slab interval
+// [s_lo, s_hi] of t in which the ray is above the voxel's (i,j) square.  There the ray climbs
+// from z = sz + v cA to sz + v cB, c = q (D - sd) > 0, so the rows v that can reach a voxel
+// [zl, zh] + sz are  v in ( zl / c_far , zh / c_near )  (with the roles of c_near / c_far set by the
+// signs of zl, zh): an exact row range from two reciprocals per column, and every row in it is a hit.
+// The row's weight is the overlap of [s_lo, s_hi] with the t-interval between its crossings of the
+// voxel's two z-planes, t = z_plane / (v q) - (d0 - sd): the same crossing parameters as
+// forward.cu's, written relative to the source so that one reciprocal serves both planes.
+template <int R, int M, int KT>
+__global__ void __launch_bounds__(32 * BK_BX, 3)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
             const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
 {
-    // lanes run along z: a warp shares (i,j), hence the whole in-plane part of every candidate test
-    // (uniform branches, broadcast table loads), and its lanes read consecutive detector rows
-    const int k = blockIdx.z * BK_BZ + threadIdx.x;
+    const int lane = threadIdx.x;
     const int i = blockIdx.x * BK_BX + threadIdx.y;
     const int j = blockIdx.y;
     const int ni = R == 4 ? P.nx / 2 : P.nx;
-    if (i >= ni || k >= P.nz / M) return;           // M == 2: the upper half are the mirror images nz-1-k
-    const float zc = fmaf((float)k, P.hz, P.z0);
-    const float zlo_mm = zc - 0.5f * P.hz, zhi_mm = zc + 0.5f * P.hz;
-    const float bz = (float)(k - P.cz), bz1 = bz + 1.0f;
+    const int nzh = P.nz / M;                        // M == 2: the upper half are the mirror images nz-1-k
+    if (i >= ni) return;                             // warp-uniform
+    int kv[KT];
+    float zl[KT];                                    // lower z-plane of the voxel relative to the source plane (index units)
+#pragma unroll
+    for (int t = 0; t < KT; ++t) {
+        kv[t] = blockIdx.z * (32 * KT) + lane + 32 * t;
+        zl[t] = (float)(min(kv[t], nzh - 1) - P.cz) - P.sz;      // a ragged tail recomputes the last voxel, not stored
+    }
     // the R quarter-turn images of the voxel: (i,j), (n-1-j, i), (n-1-i, n-1-j), (j, n-1-i)
     int vi[R], vj[R];
     vi[0] = i; vj[0] = j;
@@ -73,9 +89,12 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
         vi[2 % R] = n1 - i; vj[2 % R] = n1 - j;
         vi[3 % R] = j;      vj[3 % R] = n1 - i;
     }
-    float acc[R * M];
+    float acc[KT][R * M];
 #pragma unroll
-    for (int q = 0; q < R * M; ++q) acc[q] = 0.0f;
+    for (int t = 0; t < KT; ++t)
+#pragma unroll
+        for (int q = 0; q < R * M; ++q) acc[t][q] = 0.0f;
+    const float c0v = -P.v0 * P.inv_dv;
     const size_t plane = (size_t)P.nv * P.nu;
     for (int a = 0; a < P.nbase; ++a) {
         const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);   // c, s, dn, du
@@ -86,19 +105,14 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
             const float bx = (float)(vi[sg] - P.cx), by = (float)(vj[sg] - P.cy);
             const float rn = fmaf(xc, vw.x, fmaf(yc, vw.y, P.sad));   // (X - S).e_n  > 0
             const float ru = fmaf(xc, vw.y, -yc * vw.x);               // (X - S).e_u
-            // shadow of the voxel on the detector (Eq. A6): u* = sdd ru/rn, v* = sdd z/rn, to first
-            // order in the voxel's half extents dn, du (inflated in the table), plus 0.02 pixel
+            // shadow of the (i,j) square on the detector's u axis (Eq. A6): u* = sdd ru/rn to first order in the
+            // voxel's half extents dn, du (inflated in the table), plus 0.02 pixel
             float rinv;
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(rn));
-            const float mag = P.sdd * rinv, tn = ru * rinv, e = vw.z * rinv;
+            const float mag = P.sdd * rinv, tn = ru * rinv;
             const float uc = mag * ru, W = mag * fmaf(fabsf(tn), vw.z, vw.w);
-            const float v_lo = zlo_mm * mag * (zlo_mm < 0.0f ? 1.0f + e : 1.0f - e);
-            const float v_hi = zhi_mm * mag * (zhi_mm > 0.0f ? 1.0f + e : 1.0f - e);
             const int iu_lo = max(0, __float2int_ru((uc - W - P.u0) * P.inv_du - 0.02f));
             const int iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
-            const int iv_lo = max(0, __float2int_ru((v_lo - P.v0) * P.inv_dv - 0.02f));
-            const int iv_hi = min(P.nv - 1, __float2int_rd((v_hi - P.v0) * P.inv_dv + 0.02f));
-            if (iv_lo > iv_hi) continue;
             for (int iu = iu_lo; iu <= iu_hi; ++iu) {
                 const RayU r = load_rayu(rayu, a * P.nu + iu);
                 const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;   // slab coordinate, minor plane
@@ -107,48 +121,106 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
                 const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
                 const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
                 if (!(s_hi > s_lo)) continue;
-                float col[R * M];
+                const float e = d0 - r.sd;                               // slab start relative to the source
+                float icA, icB;
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icA) : "f"(r.q * (e + s_lo)));
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icB) : "f"(r.q * (e + s_hi)));
+                const float ic_near = fmaxf(icA, icB), ic_far = fminf(icA, icB);     // 1/c at the end nearer to / farther from the source
+                const float tiny = copysignf(1.0e-37f, r.q);            // a row with v == 0 counts as v = 0+
+                const int oA = iu * P.nv, oB = oA + P.nv - 1;              // 32-bit entry offsets of rows 0 and nv-1
 #pragma unroll
-                for (int q = 0; q < R * M; ++q) col[q] = 0.0f;
-                for (int iv = iv_lo; iv <= iv_hi; ++iv) {
-                    const float v = fmaf((float)iv, P.dv, P.v0);
-                    const RayZ rz = ray_z(r, v, P.sz);
-                    const float z0 = fmaf(d0, rz.mz, rz.za);
-                    const float q1 = (bz - z0) * rz.inv_mz, q2 = (bz1 - z0) * rz.inv_mz;
-                    const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
-                    const float w = hi - lo;
-                    if (w > 0.0f) {
-#pragma unroll
-                        for (int mm = 0; mm < M; ++mm) {        // the mirror voxel sees the mirror row with the same weight
-                            const size_t ot = (size_t)iu * P.nv + (mm ? P.nv - 1 - iv : iv);
+                for (int t = 0; t < KT; ++t) {
+                    const float zlo = zl[t], zhi = zlo + 1.0f;
+                    const float v_lo = zlo * (zlo >= 0.0f ? ic_far : ic_near);
+                    const float v_hi = zhi * (zhi >= 0.0f ? ic_near : ic_far);
+                    int iv = max(0, __float2int_ru(fmaf(v_lo, P.inv_dv, c0v) - 2.0e-3f));
+                    const int iv_hi = min(P.nv - 1, __float2int_rd(fmaf(v_hi, P.inv_dv, c0v) + 2.0e-3f));
+                    if (iv > iv_hi) continue;
+                    // overlap of [s_lo, s_hi] with the t-interval between the row's crossings of the voxel's z-planes,
+                    // times the slab length per unit of L (inv_dd); rows of the exact range always overlap
+                    auto weight = [&](int row) {
+                        const float v = fmaf((float)row, P.dv, P.v0);
+                        float inv;
+                        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(fmaf(v, r.q, tiny)));
+                        const float q1 = fmaf(zlo, inv, -e), q2 = fmaf(zhi, inv, -e);
+                        const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
+                        return fmaxf(hi - lo, 0.0f) * r.inv_dd;
+                    };
+                    // weights of image sg under base view a serve the pairs (view a + r nbase, image sg + r);
+                    // the mirror voxel sees the mirror row with the same weight
+                    auto gather = [&](float w, const float4 &tA, const float4 &tB) {
+                        acc[t][(sg + 0) % R] = fmaf(w, tA.x, acc[t][(sg + 0) % R]);
+                        if (R == 4) {
+                            acc[t][(sg + 1) % R] = fmaf(w, tA.y, acc[t][(sg + 1) % R]);
+                            acc[t][(sg + 2) % R] = fmaf(w, tA.z, acc[t][(sg + 2) % R]);
+                            acc[t][(sg + 3) % R] = fmaf(w, tA.w, acc[t][(sg + 3) % R]);
+                        }
+                        if (M == 2) {
+                            acc[t][R + (sg + 0) % R] = fmaf(w, tB.x, acc[t][R + (sg + 0) % R]);
                             if (R == 4) {
-                                const float4 t = __ldg(reinterpret_cast<const float4 *>(Ta) + ot);
-                                col[mm * R] = fmaf(w, t.x, col[mm * R]);
-                                col[mm * R + 1 % R] = fmaf(w, t.y, col[mm * R + 1 % R]);
-                                col[mm * R + 2 % R] = fmaf(w, t.z, col[mm * R + 2 % R]);
-                                col[mm * R + 3 % R] = fmaf(w, t.w, col[mm * R + 3 % R]);
-                            } else {
-                                col[mm * R] = fmaf(w, __ldg(Ta + ot), col[mm * R]);
+                                acc[t][R + (sg + 1) % R] = fmaf(w, tB.y, acc[t][R + (sg + 1) % R]);
+                                acc[t][R + (sg + 2) % R] = fmaf(w, tB.z, acc[t][R + (sg + 2) % R]);
+                                acc[t][R + (sg + 3) % R] = fmaf(w, tB.w, acc[t][R + (sg + 3) % R]);
                             }
                         }
+                    };
+                    auto fetch = [&](int o) {
+                        if (R == 4) return __ldg(reinterpret_cast<const float4 *>(Ta) + o);
+                        return make_float4(__ldg(Ta + o), 0.0f, 0.0f, 0.0f);
+                    };
+                    // the first two rows together (about two rows cross a voxel): both weights, then all four
+                    // loads, then the FMAs; a voxel with one row reads it twice with the second weight 0
+                    {
+                        const bool two = iv < iv_hi;
+                        const int ivb = two ? iv + 1 : iv;
+                        const float w0 = weight(iv), w1 = two ? weight(ivb) : 0.0f;
+                        const float4 a0 = fetch(oA + iv), a1 = fetch(oA + ivb);
+                        float4 b0 = a0, b1 = a1;
+                        if (M == 2) { b0 = fetch(oB - iv); b1 = fetch(oB - ivb); }
+                        gather(w0, a0, b0);
+                        gather(w1, a1, b1);
+                    }
+                    for (iv += 2; iv <= iv_hi; ++iv) {
+                        const float w = weight(iv);
+                        const float4 a0 = fetch(oA + iv);
+                        float4 b0 = a0;
+                        if (M == 2) b0 = fetch(oB - iv);
+                        gather(w, a0, b0);
                     }
                 }
-                // weights of image sg under base view a serve the pairs (view a + r nbase, image sg + r)
-#pragma unroll
-                for (int mm = 0; mm < M; ++mm)
-#pragma unroll
-                    for (int q = 0; q < R; ++q)
-                        acc[mm * R + (sg + q) % R] = fmaf(col[mm * R + q], r.inv_dd, acc[mm * R + (sg + q) % R]);
             }
         }
     }
 #pragma unroll
-    for (int mm = 0; mm < M; ++mm)
+    for (int t = 0; t < KT; ++t)
 #pragma unroll
-        for (int q = 0; q < R; ++q) {
-            const size_t o = ((size_t)(mm ? P.nz - 1 - k : k) * P.ny + vj[q]) * P.nx + vi[q];
-            out[o] = f ? fmaf(-coef, acc[mm * R + q], __ldg(f + o)) : acc[mm * R + q];
-        }
+        for (int mm = 0; mm < M; ++mm)
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                const float v = acc[t][mm * R + q];
+                if (kv[t] < nzh) {
+                    const size_t o = ((size_t)(mm ? P.nz - 1 - kv[t] : kv[t]) * P.ny + vj[q]) * P.nx + vi[q];
+                    out[o] = f ? fmaf(-coef, v, __ldg(f + o)) : v;
+                }
+            }
+}
+
+template <int R, int M, int KT>
+static void launch_back_kernel(const LevelParams &P, const Level &L, const float *src, const float *d_f, float coef,
+                               float *d_out, cudaStream_t st)
+{
+    const int nzh = P.nz / M, ni = R == 4 ? P.nx / 2 : P.nx, nj = R == 4 ? P.ny / 2 : P.ny;
+    const int kchunk = 32 * KT;
+    dim3 b(32, BK_BX), gr((ni + BK_BX - 1) / BK_BX, nj, (nzh + kchunk - 1) / kchunk);
+    back_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+}
+
+template <int R, int M>
+static void launch_back_rm(const LevelParams &P, const Level &L, const float *src, const float *d_f, float coef,
+                           float *d_out, cudaStream_t st)
+{
+    if (P.nz / M >= 64) launch_back_kernel<R, M, 2>(P, L, src, d_f, coef, d_out, st);
+    else launch_back_kernel<R, M, 1>(P, L, src, d_f, coef, d_out, st);
 }
 
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
@@ -165,17 +237,10 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
         src = L.d_T;
     }
     StageTimer t(g, st, ST_BACK);
-    dim3 b(BK_BZ, BK_BX);
-    const int nzh = P.nz / P.nmir;
-    if (P.nsym == 4) {
-        dim3 gr((P.nx / 2 + BK_BX - 1) / BK_BX, P.ny / 2, (nzh + BK_BZ - 1) / BK_BZ);
-        if (P.nmir == 2) back_kernel<4, 2><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
-        else back_kernel<4, 1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
-    } else {
-        dim3 gr((P.nx + BK_BX - 1) / BK_BX, P.ny, (nzh + BK_BZ - 1) / BK_BZ);
-        if (P.nmir == 2) back_kernel<1, 2><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
-        else back_kernel<1, 1><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
-    }
+    if (P.nsym == 4 && P.nmir == 2) launch_back_rm<4, 2>(P, L, src, d_f, coef, d_out, st);
+    else if (P.nsym == 4) launch_back_rm<4, 1>(P, L, src, d_f, coef, d_out, st);
+    else if (P.nmir == 2) launch_back_rm<1, 2>(P, L, src, d_f, coef, d_out, st);
+    else launch_back_rm<1, 1>(P, L, src, d_f, coef, d_out, st);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
