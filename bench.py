@@ -104,6 +104,33 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def rank_env():
+    """(rank, world_size, local_rank) from the torchrun environment; (0, 1, 0) when launched plainly."""
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")),
+            int(os.environ.get("LOCAL_RANK", "0")))
+
+
+def rank_seed(seed: int, rank: int) -> int:
+    """Every rank reconstructs its own problem: same phantom and geometry, own noise realisation."""
+    return seed + 1000 * rank
+
+
+def max_over_ranks(ms: float, world: int, device="cuda") -> float:
+    """Device time of the slowest rank (the job's time); a no-op for one process."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(steps: int, world: int, ms_total: float) -> float:
+    """Whole-job throughput: every rank did `steps` units in `ms_total` (max over ranks)."""
+    return world * steps / (ms_total / 1e3)
+
+
 def workload(name: str):
     k = {"config1": 1, "config2": 2, "config3": 3, "config4": 4}[name]
     cfg = I.config(k)
@@ -158,7 +185,7 @@ def cpu_baseline(cfg, y, budget: str = "default"):
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
+    rank, _, _ = rank_env()
     if rank != 0:
         return
     k, cfg = workload(args.workload)
@@ -192,9 +219,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_1001_0599_b200 import cbct
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = rank_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -204,7 +229,7 @@ def run_ours(args):
 
     k, cfg = workload(args.workload)
     g = cfg.geom
-    cfg.seed += 1000 * rank                       # every rank: same phantom, own noise realisation
+    cfg.seed = rank_seed(cfg.seed, rank)
     y_host = I.make_projections(cfg)
     n_levels = len(cfg.fbs.iters_per_level)
     fbs = cfg.fbs
@@ -216,13 +241,6 @@ def run_ours(args):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-
-    def max_over_ranks(ms: float) -> float:
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
 
     with torch.cuda.stream(stream), cbct.geometry_create(g, max_levels=n_levels) as h:
         y = torch.from_numpy(y_host).cuda()
@@ -257,7 +275,7 @@ def run_ours(args):
             ev1.record(stream)
             barrier()
             torch.cuda.profiler.stop()
-        ms_total = max_over_ranks(ev0.elapsed_time(ev1))
+        ms_total = max_over_ranks(ev0.elapsed_time(ev1), world)
         launches = h.launch_count - l0
         clocks = clk.summary()
 
@@ -272,7 +290,7 @@ def run_ours(args):
             h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
         ev1.record(stream)
         barrier()
-        ms_e2e = max_over_ranks(ev0.elapsed_time(ev1))
+        ms_e2e = max_over_ranks(ev0.elapsed_time(ev1), world)
 
         # ---- per-kernel attribution (CUDA events on the library's stream, synchronising) ----
         f.copy_(f_start)
@@ -334,7 +352,7 @@ def run_ours(args):
 
     base = cpu_baseline(cfg, y_host)
     line = {
-        "metric": METRIC, "value": world * K / (ms_total / 1e3), "unit": UNIT, "n_gpus": world, "steps": K,
+        "metric": METRIC, "value": aggregate_value(K, world, ms_total), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{k} ({cfg.name}): {g.nx}x{g.ny}x{g.nz} fp32 voxels at {g.hx} mm, {g.n_proj} views "
@@ -346,7 +364,7 @@ def run_ours(args):
                          % ((5 * nvox + 2 * nray) * 4 / 2 ** 20),
                    "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
         "clocks": clocks,
-        "e2e": {"value": world * K / (ms_e2e / 1e3), "unit": UNIT, "h2d_bytes_per_step": 4 * (nray + nvox),
+        "e2e": {"value": aggregate_value(K, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 4 * (nray + nvox),
                 "d2h_bytes_per_step": 4 * nvox, "ms_per_step": ms_e2e / K},
         "gpu_launches": int(launches),
         "roofline": roof,
