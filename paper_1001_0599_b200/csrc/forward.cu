@@ -107,9 +107,11 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
     typedef typename StageCell<M>::type cell;
     const cell *__restrict__ stage = reinterpret_cast<const cell *>(stage_v);
     __shared__ double slot[32];
-    const int iv = blockIdx.y * FWD_BV + threadIdx.x;
+    // detector-row tiles are the slowest grid dimension: the blocks in flight together then walk one z-slab of the
+    // staged copy for every view, which stays in L2 (with the view slowest, every view re-reads the whole copy)
+    const int iv = blockIdx.z * FWD_BV + threadIdx.x;
     const int iu = blockIdx.x * FWD_BU + threadIdx.y;
-    const int a = blockIdx.z;                  // base view
+    const int a = blockIdx.y;                  // base view
     const int nvh = M == 2 ? P.nv / 2 : P.nv;  // rows this grid walks; the others are their mirrors
     double sq = 0.0;
     if (iu < P.nu && iv < nvh) {
@@ -311,7 +313,7 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         CBCT_LAUNCH_CHECK(g);
     }
     b = dim3(FWD_BV, FWD_BU);
-    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV, P.nbase);
+    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, P.nbase, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
     if (mode == 1 && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
