@@ -382,6 +382,85 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ---------------------------------------------------------------------------------------------
+# config 5: projector / TV microbenchmark sweep (each operator alone)
+# ---------------------------------------------------------------------------------------------
+
+def run_sweep(args):
+    """BASELINE.json config 5: P, P^T and TV-prox each alone on n^3 volumes (n in --sweep-sizes, uniform random in
+    [0, 0.03)/mm, fixed 256 mm field of view) with --sweep-views projections of 512x384; prints ONE JSON line whose
+    "sweep" list holds, per case, milliseconds per call, projector GUPS and fraction of the L1-gather roofline, and the
+    TV passes' achieved HBM GB/s.  Inputs smaller than the 126 MB L2 are followed by an L2 flush between calls."""
+    import torch
+    from paper_1001_0599_b200 import cbct
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    hbm_peak, sm_max_mhz, peak_src = _peaks()
+    l1_peak_gups = 148 * 128 * sm_max_mhz * 1e6 / 4 / 1e9
+    flush = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device="cuda")
+    sizes = [int(x) for x in args.sweep_sizes.split(",")]
+    views = [int(x) for x in args.sweep_views.split(",")]
+    out = []
+
+    def timed(fn, reps):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        for _ in range(3):
+            fn()
+        for e0, e1 in ev:
+            flush.zero_()                       # evict the previous call's lines from L2
+            e0.record()
+            fn()
+            e1.record()
+        torch.cuda.synchronize()
+        t = sorted(e0.elapsed_time(e1) for e0, e1 in ev)
+        return t[len(t) // 2]
+
+    for n in sizes:
+        for nv in views:
+            g = I.sweep_geometry(n, nv)
+            with cbct.geometry_create(g) as h:
+                gen = torch.Generator(device="cuda").manual_seed(I.SEED_BASE + 5)
+                f = torch.rand(g.vol_shape, device="cuda", generator=gen) * 0.03
+                q = torch.rand(g.proj_shape, device="cuda", generator=gen)
+                p, b = torch.empty_like(q), torch.empty_like(f)
+                S = h.count_samples()
+                reps = max(3, min(args.steps, 10))
+                case = {"n": n, "n_proj": nv, "symmetry": h.symmetry, "samples": int(S)}
+                h.set_stage_timing(True)
+                for name, fn, stage in (("forward", lambda: h.forward_project(f, p), "forward"),
+                                        ("back", lambda: h.back_project(q, b), "back")):
+                    ms = timed(fn, reps)
+                    h.set_stage_timing(True)    # reset the accumulators, then attribute the kernel itself
+                    fn()
+                    kms = h.stage_ms()[stage][0]
+                    case[name] = {"ms_per_call": ms, "kernel_ms": kms, "gups": S / kms / 1e6,
+                                  "frac_of_l1_gather_roofline": S / kms / 1e6 / l1_peak_gups}
+                if nv == views[0]:              # TV does not depend on the view count: once per size
+                    setup = I.FbsSetup(max_inner=10, rel_tol=0.0, eps_delta=1e-4)
+                    ms = timed(lambda: h.tv_prox(f, b, 1e-3, setup), reps)
+                    h.set_stage_timing(True)
+                    rep = h.tv_prox(f, b, 1e-3, setup)
+                    st = h.stage_ms()
+                    nvox = f.numel()
+                    tv = {"ms_per_call": ms, "inner_iters": rep.inner_iters, "trials": rep.trials}
+                    for k, bpv in (("tv_grad", 12.0), ("tv_trial", 12.0), ("tv_update", 12.0)):
+                        if st[k][1]:
+                            t = st[k][0] / st[k][1]
+                            tv[k] = {"ms_per_launch": t, "hbm_gbs": bpv * nvox / t / 1e6,
+                                     "frac_of_hbm_peak": bpv * nvox / t / 1e6 / hbm_peak}
+                    case["tv_prox"] = tv
+                h.set_stage_timing(False)
+                out.append(case)
+            del f, q, p, b
+            torch.cuda.empty_cache()
+    print(json.dumps({"metric": "projector_gups_sweep", "unit": "GUPS", "n_gpus": 1, "data": "synthetic", "dtype": "f32",
+                      "config": {"workload": "config5: P, P^T, TV-prox each alone; n^3 volume at 256/n mm, 512x384 detector",
+                                 "l2": "256 MiB flush buffer written between timed calls"},
+                      "peaks": {"l1_gather_gups": l1_peak_gups, "hbm_gbs": hbm_peak, "source": peak_src},
+                      "sweep": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -390,7 +469,12 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--no-recon", action="store_true", help="skip the whole-reconstruction timing")
+    ap.add_argument("--sweep", action="store_true", help="config 5: operator microbenchmarks instead of the FBS step")
+    ap.add_argument("--sweep-sizes", default="64,128,256,512")
+    ap.add_argument("--sweep-views", default="1,40,360")
     args = ap.parse_args()
+    if args.sweep:
+        return run_sweep(args)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":
