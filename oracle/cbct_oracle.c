@@ -19,6 +19,7 @@
  *   tv_energy, tv_gradient, tv_prox                                 pinned (P7-P10)
  *   fbs                                                             pinned (P11, P12, P14)
  *   restrict / prolong / bin                                        pinned (P13)
+ *   back_eq6 (NEXT-1, Eq. 6)                                        pinned (P4, P15, P16)
  *   PARITY UNPINNED: the *choice* of binned detectors on coarse levels (S12) and
  *   the defaults eps_delta, lambda_0 = 1/beta, max_inner (design choices the
  *   paper does not fix; the oracle is their definition).
@@ -303,6 +304,44 @@ void oracle_back(const ogeom *g, const double *p, double *b)
 /* (PAPER.md:L100 E1, L151 E3, L155-L161).                                   */
 /* Forward differences in physical units.  Neighbour outside the grid:       */
 /* value 0 under BC_ZERO, own value under BC_REFLECT (L161).                  */
+/* NEXT-1: the paper's own gradient of E2, Eq. (6) -- the continuum adjoint, NOT the
+ * transpose of the ray-tracing matrix:
+ *     b6(X) = (dV / (du dv)) * sum_theta  L^3(u*,v*) / (L0 l^2(X)) * T^theta(u*, v*)
+ * with (u*, v*) and l from Eq. (A6) (oracle_voxel_to_detector), L = sqrt(L0^2 + u*^2 + v*^2) (A2), and
+ * T^theta(u*, v*) by BILINEAR interpolation between pixel centres (L199).  The factor dV/(du dv) (voxel volume
+ * over pixel area) puts b6 on the scale of P^T T (sum_r a(r,v) = dV L^3/(l^2 du dv L0), survey S1), so that it can
+ * replace P^T T in step 1 of Algorithm A1 with the same step size.  Reading S19: a tap outside the detector is 0. */
+void oracle_back_eq6(const ogeom *g, const double *T, double *b)
+{
+    const double scale = g->hx * g->hy * g->hz / (g->du * g->dv);
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g->nz; ++k)
+        for (int j = 0; j < g->ny; ++j)
+            for (int i = 0; i < g->nx; ++i) {
+                double X[3] = { (i - 0.5 * (g->nx - 1)) * g->hx + g->off[0],
+                                (j - 0.5 * (g->ny - 1)) * g->hy + g->off[1],
+                                (k - 0.5 * (g->nz - 1)) * g->hz + g->off[2] };
+                double acc = 0.0;
+                for (int a = 0; a < g->n_proj; ++a) {
+                    double us, vs, l;
+                    oracle_voxel_to_detector(g, a, X, &us, &vs, &l);
+                    double L = sqrt(g->sdd * g->sdd + us * us + vs * vs);
+                    double fu = (us - g->offu) / g->du + 0.5 * (g->nu - 1);      /* fractional pixel index */
+                    double fv = (vs - g->offv) / g->dv + 0.5 * (g->nv - 1);
+                    double iu0 = floor(fu), iv0 = floor(fv), tu = fu - iu0, tv = fv - iv0;
+                    double val = 0.0;
+                    for (int dv = 0; dv < 2; ++dv)
+                        for (int du = 0; du < 2; ++du) {
+                            long iu = (long)iu0 + du, iv = (long)iv0 + dv;
+                            if (iu < 0 || iu >= g->nu || iv < 0 || iv >= g->nv) continue;
+                            val += (du ? tu : 1.0 - tu) * (dv ? tv : 1.0 - tv) * T[((long)a * g->nv + iv) * g->nu + iu];
+                        }
+                    acc += L * L * L / (g->sdd * l * l) * val;
+                }
+                b[((long)k * g->ny + j) * g->nx + i] = scale * acc;
+            }
+}
+
 /* ---------------------------------------------------------------------- */
 static inline double fwd_diff(double here, double next_or_nan, int at_edge, int bc, double h)
 {

@@ -175,6 +175,15 @@ def back(g, p):
     return b
 
 
+def back_eq6(g, T):
+    """The paper's closed-form gradient Eq. 6 (L195-L199): voxel-driven, bilinear T, on the scale of P^T T."""
+    s, keep = _geom(g)
+    T = _arr(T, g.proj_shape)
+    b = np.zeros(g.vol_shape)
+    lib().oracle_back_eq6(C.byref(s), _p(T), _p(b))
+    return b
+
+
 # -- TV / ROF ---------------------------------------------------------------
 
 def tv_energy(g, f, delta) -> float:

@@ -212,3 +212,59 @@ def test_truncated_detector_and_rays_missing_the_volume(orc):
     assert np.all(p[:, 0, :] == 0.0) and np.all(p[:, -1, :] == 0.0) and p.max() > 0
     b = orc.back(g, np.ones(g.proj_shape))
     assert b.min() == 0.0 and b.max() > 0
+
+
+# ---------------------------------------------------------------------------
+# NEXT-1: the paper's Eq. 6 back-projector, oracle_back_eq6
+# ---------------------------------------------------------------------------
+
+def test_P15_eq6_isocentre_voxel_and_theta0_by_hand(orc):
+    """Values the paper's formulas fix by hand.  (i) A voxel at the isocentre sees u* = v* = 0, l = SAD, L = L0 in
+    every view (A6, L401-L406), so with T = 1 Eq. 6 gives  dV/(du dv) * N_theta * L0^2 / SAD^2.  (ii) At theta = 0
+    the appendix formulas hold literally (A6: u* = -(y-ys) L0/(x-xs), v* = (z-zs) L0/(x-xs); A2: L^2 = L0^2+u^2+v^2);
+    a T that is linear in (u, v) is reproduced exactly by bilinear interpolation, so the expected value needs no
+    interpolation code."""
+    g = I.Geometry(nx=5, ny=5, nz=5, hx=2.0, hy=2.0, hz=3.0, nu=64, nv=64, du=1.5, dv=2.5, sad=400.0, sdd=700.0,
+                   n_proj=7, angles=np.deg2rad([0.0, 31.0, 77.0, 140.0, 201.0, 260.0, 333.0]))
+    b = orc.back_eq6(g, np.ones(g.proj_shape))
+    assert b[2, 2, 2] == pytest.approx(2.0 * 2.0 * 3.0 / (1.5 * 2.5) * 7 * 700.0 ** 2 / 400.0 ** 2, rel=1e-12)
+    g0 = g.replace(n_proj=1, angles=np.array([0.0]))
+    u = (np.arange(g0.nu) - (g0.nu - 1) / 2) * g0.du
+    v = (np.arange(g0.nv) - (g0.nv - 1) / 2) * g0.dv
+    U, V = np.meshgrid(u, v)
+    a0, a1, a2 = 0.7, 0.013, -0.021
+    b = orc.back_eq6(g0, (a0 + a1 * U + a2 * V)[None])
+    for (i, j, k) in [(0, 0, 0), (4, 1, 3), (2, 4, 0), (3, 3, 4)]:
+        x, y, z = (i - 2) * 2.0, (j - 2) * 2.0, (k - 2) * 3.0
+        xs = -400.0
+        us, vs = -(y - 0.0) * 700.0 / (x - xs), (z - 0.0) * 700.0 / (x - xs)
+        L = np.sqrt(700.0 ** 2 + us ** 2 + vs ** 2)
+        l2 = (x - xs) ** 2 + y ** 2 + z ** 2
+        want = 12.0 / 3.75 * L ** 3 / (700.0 * l2) * (a0 + a1 * us + a2 * vs)
+        assert b[k, j, i] == pytest.approx(want, rel=1e-12), (i, j, k)
+
+
+def test_P16_eq6_agrees_with_the_exact_transpose_in_the_continuum_limit_and_not_at_config_sampling(orc):
+    """Survey S1: with a detector much finer than the voxel footprint and a smooth T, Eq. 6 and the exact transpose
+    agree to ~1 %; at the configs' sampling (footprint ~ 1.9 pixels) they differ by tens of per cent voxel by voxel
+    (aliasing of the footprint against the pixel grid) -- the two are not interchangeable."""
+    Tfun = lambda uu, vv: 1.0 + 0.004 * uu - 0.003 * vv + 1e-5 * uu * vv
+    def both(nu, du):
+        g = I.Geometry(nx=8, ny=8, nz=8, hx=2.0, hy=2.0, hz=2.0, nu=nu, nv=nu, du=du, dv=du, sad=400.0, sdd=600.0,
+                       n_proj=3, angles=np.deg2rad([10.0, 130.0, 250.0]))
+        u = (np.arange(nu) - (nu - 1) / 2) * du
+        U, V = np.meshgrid(u, u)
+        T = np.repeat(Tfun(U, V)[None], 3, axis=0)
+        return orc.back(g, T), orc.back_eq6(g, T)
+    exact, eq6 = both(400, 0.1)
+    assert np.abs(eq6 / exact - 1).max() < 0.02
+    exact, eq6 = both(14, 2.9)        # footprint 2 * 1.5 / 2.9 ~ 1 pixel
+    assert np.abs(eq6 / exact - 1).max() > 0.05
+
+
+def test_eq6_taps_outside_the_detector_are_zero(orc):
+    """Reading S19: a voxel whose (u*, v*) falls off the detector by more than a pixel gets nothing from that view."""
+    g = I.Geometry(nx=9, ny=9, nz=9, hx=4.0, hy=4.0, hz=4.0, nu=6, nv=6, du=1.0, dv=1.0, sad=300.0, sdd=450.0,
+                   n_proj=1)
+    b = orc.back_eq6(g, np.ones(g.proj_shape))
+    assert b[4, 4, 4] > 0 and b[0, 4, 4] == 0.0 and b[4, 0, 4] == 0.0 and b[8, 8, 4] == 0.0
