@@ -96,6 +96,15 @@ cbct_status cbct_forward_project(const cbct_geometry *g, int level, const float 
 cbct_status cbct_back_project(const cbct_geometry *g, int level, const float *d_proj,
                               float *d_vol, void *cuda_stream);
 
+/* NEXT-1: d_vol = b6(d_proj), the paper's own closed-form gradient of the data term, Eq. 6 (L195-L199):
+ *   b6(X) = (dV / (du dv)) sum_theta L^3(u*,v*) / (L0 l^2(X)) T^theta(u*,v*),
+ * (u*,v*) and l from Eq. A6 (L401-L406), T^theta(u*,v*) by bilinear interpolation between pixel centres
+ * (L199; a tap outside the detector is 0).  It is the continuum adjoint, NOT the transpose of
+ * cbct_forward_project: the two agree only when the pixels are much finer than a voxel's shadow.  The factor
+ * dV/(du dv) puts it on the scale of cbct_back_project.  Voxel-driven, no atomics.  Overwrites d_vol. */
+cbct_status cbct_back_project_eq6(const cbct_geometry *g, int level, const float *d_proj,
+                                  float *d_vol, void *cuda_stream);
+
 /* S = number of (ray, voxel) pairs with a(ray, voxel) > 0 at `level`: the "ray-voxel samples" one
  * forward (or back) projection processes -- the unit of the GUPS metric.  Synchronises the stream. */
 cbct_status cbct_count_samples(const cbct_geometry *g, int level, unsigned long long *count,
@@ -157,12 +166,17 @@ cbct_status cbct_prolong_volume(const cbct_geometry *g, int level, const float *
  * Coarse data are 2x2-binned; the volume moves up by cbct_prolong_volume.
  * d_vol_inout: finest-level volume; the initial guess if use_initial (restricted down to
  * the coarsest level first), else ignored on entry; the result on return. */
+#define CBCT_BACKPROJECTOR_EXACT 0
+#define CBCT_BACKPROJECTOR_EQ6 1
 typedef struct {
     double tv_weight; /* lambda = 1/mu of Eq. 2 (L97) */
     double step;      /* relative gradient step in (0, 2); 1 = 1/Lhat */
     int n_levels;     /* <= max_levels of the handle */
     const int *iters_per_level;
     int nonneg, use_initial;
+    int backprojector; /* CBCT_BACKPROJECTOR_EXACT (0): g = f - tau c_norm P^T T, the matched pair;
+                          CBCT_BACKPROJECTOR_EQ6 (1): g = f - tau c_norm b6(T), the paper's Eq. 6 (unmatched pair;
+                          Lhat is still the matched pair's bound) */
     cbct_tv_params tv;
 } cbct_fbs_params;
 

@@ -565,7 +565,7 @@ double oracle_step_bound(const ogeom *g)
 /* n_iter iterations at one level.  objective[it] = tv_weight * E1^delta(f) +
  * E2(f) for the f that ENTERS iteration it (may be NULL).  Returns tau. */
 double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_weight, double step,
-                        int n_iter, int nonneg, const otv_params *tp, double *objective,
+                        int n_iter, int nonneg, int use_eq6, const otv_params *tp, double *objective,
                         int *inner_total, int *trials_total)
 {
     long nvox = (long)g->nx * g->ny * g->nz, nray = (long)g->n_proj * g->nv * g->nu;
@@ -580,7 +580,8 @@ double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_we
         for (long r = 0; r < nray; ++r) { T[r] -= y[r]; E2 += T[r] * T[r]; }
         E2 /= (double)nray;
         if (objective) objective[it] = tv_weight * oracle_tv_energy(g, f, tp->eps_delta) + E2;
-        oracle_back(g, T, b);
+        if (use_eq6) oracle_back_eq6(g, T, b);      /* the paper's step 1: Eq. 6 in place of P^T T (L195) */
+        else oracle_back(g, T, b);
         for (long v = 0; v < nvox; ++v) gg[v] = f[v] - tau * c_norm * b[v];
         otv_report rep;
         oracle_tv_prox(g, gg, f, w, tp, &rep);
@@ -601,7 +602,7 @@ double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_we
  * sum(iters) entries (may be NULL); step_abs[n_levels] receives tau per level
  * in the same coarsest -> finest order (may be NULL). */
 void oracle_fbs(const ogeom *g0, const double *y0, double *f, double tv_weight, double step,
-                int n_levels, const int *iters, int nonneg, int use_initial,
+                int n_levels, const int *iters, int nonneg, int use_initial, int use_eq6,
                 const otv_params *tp, double *objective, double *step_abs, int *inner_total,
                 int *trials_total)
 {
@@ -631,7 +632,7 @@ void oracle_fbs(const ogeom *g0, const double *y0, double *f, double tv_weight, 
     int done = 0;
     for (int l = n_levels - 1; l >= 0; --l) {
         int n_it = iters[n_levels - 1 - l];
-        double tau = oracle_fbs_level(&gl[l], yl[l], cur, tv_weight, step, n_it, nonneg, tp,
+        double tau = oracle_fbs_level(&gl[l], yl[l], cur, tv_weight, step, n_it, nonneg, use_eq6, tp,
                                       objective ? objective + done : NULL, inner_total, trials_total);
         if (step_abs) step_abs[n_levels - 1 - l] = tau;
         done += n_it;

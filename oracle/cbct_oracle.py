@@ -282,6 +282,7 @@ def fbs(g, y, fbs_setup, f0=None):
     inner = C.c_int(0); trials = C.c_int(0)
     lib().oracle_fbs(C.byref(s), _p(y), _p(f), C.c_double(fbs_setup.tv_weight),
                      C.c_double(fbs_setup.step), n_levels, iters.ctypes.data_as(C.POINTER(C.c_int)),
-                     int(bool(fbs_setup.nonneg)), int(f0 is not None), C.byref(tp), _p(obj),
+                     int(bool(fbs_setup.nonneg)), int(f0 is not None),
+                     int(getattr(fbs_setup, "backprojector", 0)), C.byref(tp), _p(obj),
                      _p(step_abs), C.byref(inner), C.byref(trials))
     return FbsResult(f, obj, step_abs, inner.value, trials.value)

@@ -28,7 +28,7 @@ STATUS_NAMES = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_GEOMETRY",
 # every symbol include/cbct.h declares
 EXPORTS = [
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_symmetry", "cbct_geometry_device_bytes",
-    "cbct_forward_project", "cbct_back_project", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
+    "cbct_forward_project", "cbct_back_project", "cbct_back_project_eq6", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
     "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_last_error", "cbct_version",
@@ -64,7 +64,7 @@ class _TvReport(C.Structure):
 class _FbsParams(C.Structure):
     _fields_ = [("tv_weight", C.c_double), ("step", C.c_double), ("n_levels", C.c_int),
                 ("iters_per_level", C.POINTER(C.c_int)), ("nonneg", C.c_int), ("use_initial", C.c_int),
-                ("tv", _TvParams)]
+                ("backprojector", C.c_int), ("tv", _TvParams)]
 
 
 class _FbsReport(C.Structure):
@@ -115,6 +115,7 @@ def load_library():
     lib.cbct_geometry_device_bytes.restype = C.c_ulonglong
     lib.cbct_forward_project.argtypes = [vp, ip, vp, vp, vp]
     lib.cbct_back_project.argtypes = [vp, ip, vp, vp, vp]
+    lib.cbct_back_project_eq6.argtypes = [vp, ip, vp, vp, vp]
     lib.cbct_count_samples.argtypes = [vp, ip, C.POINTER(C.c_ulonglong), vp]
     lib.cbct_step_bound.argtypes = [vp, ip, C.POINTER(dp), vp]
     lib.cbct_tv_prox.argtypes = [vp, ip, vp, vp, dp, ip, C.POINTER(_TvParams), C.POINTER(_TvReport), vp]
@@ -240,6 +241,11 @@ class Geometry:
                                                 _dev(vol, self._nvox(level), "vol"), _stream_ptr(stream)))
         return vol
 
+    def back_project_eq6(self, proj, vol, level: int = 0, stream=None):
+        _check(load_library().cbct_back_project_eq6(self._h, level, _dev(proj, self._nray(level), "proj"),
+                                                    _dev(vol, self._nvox(level), "vol"), _stream_ptr(stream)))
+        return vol
+
     def count_samples(self, level: int = 0, stream=None) -> int:
         out = C.c_ulonglong()
         _check(load_library().cbct_count_samples(self._h, level, C.byref(out), _stream_ptr(stream)))
@@ -287,6 +293,7 @@ class Geometry:
         p.tv_weight, p.step, p.n_levels = fbs.tv_weight, fbs.step, len(iters)
         p.iters_per_level = iters.ctypes.data_as(C.POINTER(C.c_int))
         p.nonneg, p.use_initial = int(bool(fbs.nonneg)), int(bool(use_initial))
+        p.backprojector = int(getattr(fbs, "backprojector", 0))
         p.tv = _tv_params(fbs)
         obj = np.zeros(int(iters.sum()) if want_objective else 0)
         step_abs = np.zeros(len(iters))

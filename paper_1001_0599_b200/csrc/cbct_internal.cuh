@@ -60,6 +60,7 @@ struct Level {
     size_t nvox, nray;
     RayU *d_rayu = nullptr;     // [np][nu]
     ViewC *d_view = nullptr;    // [np]
+    double2 *d_cs = nullptr;    // [np] cos, sin of the view angles in fp64 (back_eq6.cu)
     // scratch (all fp32 unless noted)
     float *d_stage = nullptr;   // zero-padded, z-fastest copy of the volume: [i+PM][j+PM][k+PZ]
     size_t stage_elems = 0;
@@ -150,12 +151,16 @@ static inline const Level *get_level(const cbct_geometry *g, int level)
 //              mode 1: out = L * (P vol - y) in the d_T layout, *d_sum_sq = sum (P vol - y)^2.
 //              mode 2: out = L * (P vol) in the d_T layout.
 //              mode 3: *d_sum_sq = number of (ray, voxel) pairs, no volume read
+//              mode 4: out = P vol - y (plain layout), *d_sum_sq = sum (P vol - y)^2
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
                            float *d_out, int mode, double *d_sum_sq, cudaStream_t st);
 // back.cu : scaled != 0: d_in already holds L*T in the d_T layout; else plain layout, unscaled.
 //           out = f - coef * P^T in (f may be NULL: out = P^T in)
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
                         const float *d_f, float coef, float *d_out, cudaStream_t st);
+// back_eq6.cu : out = f - coef * b6(T) with T in the plain [view][row][column] layout (f may be NULL: out = b6(T))
+cbct_status launch_back_eq6(const cbct_geometry *g, const Level &L, const float *d_T, const float *d_f, float coef,
+                            float *d_out, cudaStream_t st);
 // tv.cu
 cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,

@@ -77,6 +77,7 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         }
     }
 
+    const bool eq6 = p->backprojector == CBCT_BACKPROJECTOR_EQ6;
     int done = 0, inner_total = 0, trials_total = 0;
     for (int l = nl - 1; l >= 0; --l) {
         const Level &L = g->levels[l];
@@ -93,13 +94,15 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         if (rep && rep->step_abs) rep->step_abs[nl - 1 - l] = tau;
         for (int it = 0; it < n_it; ++it, ++done) {
             {
-                if ((s = launch_forward(g, L, f, y, L.d_T, 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
+                if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
             }
             if (want_obj) {
                 if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, g->d_objective + 2 * done, st)) != CBCT_OK) return s;
             }
             {
-                if ((s = launch_back(g, L, L.d_T, 1, f, (float)(tau * c_norm), L.d_g, st)) != CBCT_OK) return s;
+                if (eq6) s = launch_back_eq6(g, L, L.d_T, f, (float)(tau * c_norm), L.d_g, st);
+                else s = launch_back(g, L, L.d_T, 1, f, (float)(tau * c_norm), L.d_g, st);
+                if (s != CBCT_OK) return s;
             }
             {
                 cbct_tv_report tr;

@@ -211,6 +211,10 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                 const size_t o1 = (size_t)(a + q * P.nbase) * plane + pix;
                 if (MODE == 0) {
                     out[o1] = pr;
+                } else if (MODE == 4) {                // plain residual for the Eq. 6 back-projector
+                    const float T = pr - __ldg(y + o1);
+                    out[o1] = T;
+                    sq += (double)T * (double)T;
                 } else if (MODE == 2) {
                     res[q] = pr * Lr;                  // L * (P f): input of the transpose without a residual
                 } else {
@@ -219,14 +223,14 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                     sq += (double)T * (double)T;
                 }
             }
-            if (MODE != 0) {                           // d_T layout: [base view][iu][iv] (x4 interleaved)
+            if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
                 const size_t ot = ((size_t)a * P.nu + iu) * P.nv + ivm;
                 if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
                 else out[ot] = res[0];
             }
         }
     }
-    if (MODE == 1) {        // E2 numerator: sum of squared residuals, second stage fused (reduce.cuh)
+    if (MODE == 1 || MODE == 4) {        // E2 numerator: sum of squared residuals, second stage fused (reduce.cuh)
         double s[1];
         s[0] = block_sum(sq, slot);
         publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
@@ -280,6 +284,8 @@ static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, di
 {
     if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
     else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
+    else if (mode == 4) forward_kernel<R, M, 4><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                                 g->d_counter, d_sum_sq);
     else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
                                                    g->d_counter, d_sum_sq);
 }
@@ -315,7 +321,7 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     b = dim3(FWD_BV, FWD_BU);
     dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, P.nbase, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;
-    if (mode == 1 && nblk > (size_t)g->partials_stride)
+    if ((mode == 1 || mode == 4) && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
     {
         StageTimer t(g, st, ST_FORWARD);

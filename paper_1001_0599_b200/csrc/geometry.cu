@@ -113,7 +113,7 @@ static void free_all(cbct_geometry *g)
 {
     if (!g) return;
     for (Level &L : g->levels) {
-        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_stage); cudaFree(L.d_T);
+        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_cs); cudaFree(L.d_stage); cudaFree(L.d_T);
         cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_y);
     }
     cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter);
@@ -205,6 +205,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
 #define TRY(x) do { st = (x); if (st != CBCT_OK) { free_all(g); return st; } } while (0)
         TRY(dev_alloc(g, &L.d_rayu, rays.size()));
         TRY(dev_alloc(g, &L.d_view, views.size()));
+        TRY(dev_alloc(g, &L.d_cs, views.size()));
         TRY(dev_alloc(g, &L.d_stage, L.stage_elems));
         if (cudaMemset(L.d_stage, 0, L.stage_elems * sizeof(float)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the staged volume failed"); }
         TRY(dev_alloc(g, &L.d_T, L.nray));
@@ -216,6 +217,11 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         cudaError_t e = cudaMemcpy(L.d_rayu, rays.data(), rays.size() * sizeof(RayU), cudaMemcpyHostToDevice);
         if (e == cudaSuccess)
             e = cudaMemcpy(L.d_view, views.data(), views.size() * sizeof(ViewC), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) {
+            std::vector<double2> cs(p.np);
+            for (int a = 0; a < p.np; ++a) cs[a] = make_double2(cos(g->angles[a]), sin(g->angles[a]));
+            e = cudaMemcpy(L.d_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice);
+        }
         if (e != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "table upload: %s", cudaGetErrorString(e)); }
     }
     {

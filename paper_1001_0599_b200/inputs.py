@@ -97,6 +97,7 @@ class FbsSetup:
     armijo_c: float = 0.01
     shrink_alpha: float = 0.6
     rel_tol: float = 1e-3
+    backprojector: int = 0    # 0: exact transpose P^T (matched pair); 1: the paper's Eq. 6
 
 
 @dataclass

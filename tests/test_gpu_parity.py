@@ -326,3 +326,44 @@ def test_error_paths(torch, cbct):
     with pytest.raises(cbct.CbctError) as e:
         cbct.geometry_create(flat)
     assert e.value.status == 2
+
+
+# ---------------------------------------------------------------------------
+# NEXT-1: the paper's Eq. 6 back-projector
+# ---------------------------------------------------------------------------
+
+@pytest.mark.parametrize("name", list(GEOMS))
+def test_eq6_back_projector_matches_oracle(torch, cbct, orc, name):
+    g = GEOMS[name]
+    q = I.uniform_projections(g, 13)
+    want = orc.back_eq6(g, q)
+    outs = []
+    with cbct.geometry_create(g) as h:
+        for _ in range(2):
+            b = torch.empty(g.vol_shape, device="cuda", dtype=torch.float32)
+            h.back_project_eq6(dev(torch, q), b)
+            outs.append(b.cpu().numpy())
+    assert rel_l2(outs[0], want) <= TOL_PROJ, (name, rel_l2(outs[0], want))
+    assert np.abs(outs[0] - want).max() <= 1e-4 * np.abs(want).max()
+    assert np.array_equal(outs[0] == 0.0, want == 0.0)             # voxels no view sees are exactly 0 on both sides
+    assert outs[0].tobytes() == outs[1].tobytes()
+
+
+def test_fbs_with_the_papers_eq6_gradient_matches_oracle(torch, cbct, orc):
+    """Algorithm A1 as the paper ran it: step 1 with Eq. 6 in place of P^T (an unmatched pair), two levels."""
+    g = I.Geometry(nx=48, ny=48, nz=32, hx=2.0, hy=2.0, hz=2.5, nu=64, nv=48, du=2.4, dv=2.4, sad=1000.0,
+                   sdd=1500.0, n_proj=10)
+    ell = [I.Ellipsoid((0.0, 0.0, 0.0), (40.0, 34.0, 36.0), 0.0, 0.02)] + \
+        I.random_ellipsoids(np.random.default_rng(71), 6, (48.0, 48.0, 40.0), axes_range=(4.0, 14.0))
+    y = I.poisson_log(I.analytic_projections(ell, g), 1e5, 72).astype(np.float32)
+    setup = I.FbsSetup(iters_per_level=(5, 4), backprojector=1, step=0.8)
+    want = orc.fbs(g, y, setup)
+    with cbct.geometry_create(g, max_levels=2) as h:
+        f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+        rep = h.fbs_reconstruct(dev(torch, y), f, setup)
+        got = f.cpu().numpy()
+    assert rel_l2(got, want.f) <= TOL_VOL, rel_l2(got, want.f)
+    np.testing.assert_allclose(rep.objective, want.objective, rtol=1e-4)
+    # and it is a different iteration from the matched pair's
+    exact = orc.fbs(g, y, I.FbsSetup(iters_per_level=(5, 4), step=0.8))
+    assert rel_l2(want.f, exact.f) > 1e-3
