@@ -147,6 +147,13 @@ cbct_status cbct_tv_prox(const cbct_geometry *g, int level, const float *d_g, fl
 cbct_status cbct_tv_energy(const cbct_geometry *g, int level, const float *d_f, double eps_delta,
                            double *e1, void *cuda_stream);
 
+/* NEXT-3: the paper's image-quality metrics of a reconstruction d_f against a ground truth d_f0 (L263):
+ *   *rel_error = ||f - f0||_2 / ||f0||_2,   *correlation = corr(f, f0) (Pearson, over all voxels);
+ * one fused pass, fp64 sums in a fixed order.  0 is returned for a metric whose denominator vanishes.
+ * Synchronises the stream. */
+cbct_status cbct_quality_metrics(const cbct_geometry *g, int level, const float *d_f, const float *d_f0,
+                                 double *rel_error, double *correlation, void *cuda_stream);
+
 /* A8 grid transfers (L215-L223; readings S12, S13).  `level` is the FINE level of the pair.
  *   restrict: fine volume -> 2x2x2 mean on level+1.   bin: fine projections -> 2x2 mean.
  *   prolong : coarse volume (level+1) -> fine, cell-centred trilinear (3/4, 1/4); a missing

@@ -252,6 +252,19 @@ def prolong(coarse, bc_xy, bc_z):
     return out
 
 
+# -- quality metrics (NEXT-3) -------------------------------------------------
+
+def quality_metrics(f, f0):
+    """The paper's metrics (L263) written out: e = ||f - f0||_2 / ||f0||_2 and the Pearson correlation
+    c = sum (f - mean f)(f0 - mean f0) / sqrt(sum (f - mean f)^2 sum (f0 - mean f0)^2), in fp64."""
+    f = np.asarray(f, dtype=np.float64).ravel()
+    f0 = np.asarray(f0, dtype=np.float64).ravel()
+    e = float(np.sqrt(np.sum((f - f0) ** 2) / np.sum(f0 ** 2)))
+    a, b = f - f.mean(), f0 - f0.mean()
+    c = float(np.sum(a * b) / np.sqrt(np.sum(a * a) * np.sum(b * b)))
+    return e, c
+
+
 # -- FBS --------------------------------------------------------------------
 
 def step_bound(g) -> float:

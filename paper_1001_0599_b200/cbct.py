@@ -29,6 +29,7 @@ STATUS_NAMES = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_GEOMETRY",
 EXPORTS = [
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_symmetry", "cbct_geometry_device_bytes",
     "cbct_forward_project", "cbct_back_project", "cbct_back_project_eq6", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
+    "cbct_quality_metrics",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
     "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_last_error", "cbct_version",
@@ -118,6 +119,7 @@ def load_library():
     lib.cbct_back_project_eq6.argtypes = [vp, ip, vp, vp, vp]
     lib.cbct_count_samples.argtypes = [vp, ip, C.POINTER(C.c_ulonglong), vp]
     lib.cbct_step_bound.argtypes = [vp, ip, C.POINTER(dp), vp]
+    lib.cbct_quality_metrics.argtypes = [vp, ip, vp, vp, C.POINTER(dp), C.POINTER(dp), vp]
     lib.cbct_tv_prox.argtypes = [vp, ip, vp, vp, dp, ip, C.POINTER(_TvParams), C.POINTER(_TvReport), vp]
     lib.cbct_tv_energy.argtypes = [vp, ip, vp, dp, C.POINTER(dp), vp]
     lib.cbct_restrict_volume.argtypes = [vp, ip, vp, vp, vp]
@@ -270,6 +272,14 @@ class Geometry:
         _check(load_library().cbct_tv_energy(self._h, level, _dev(f, self._nvox(level), "f"),
                                              C.c_double(eps_delta), C.byref(out), _stream_ptr(stream)))
         return out.value
+
+    def quality_metrics(self, f, f0, level: int = 0, stream=None):
+        """(relative error e, correlation coefficient c) of f against the ground truth f0."""
+        e, c = C.c_double(), C.c_double()
+        _check(load_library().cbct_quality_metrics(self._h, level, _dev(f, self._nvox(level), "f"),
+                                                   _dev(f0, self._nvox(level), "f0"), C.byref(e), C.byref(c),
+                                                   _stream_ptr(stream)))
+        return e.value, c.value
 
     def restrict_volume(self, fine, coarse, level: int = 0, stream=None):
         _check(load_library().cbct_restrict_volume(self._h, level, _dev(fine, self._nvox(level), "fine"),
