@@ -38,9 +38,9 @@ METRIC = "fbs_iterations_per_second"
 UNIT = "iter/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
-# capture of this command (profiles/r01b_ncu_full_summary.txt); None = not captured for that kernel.
-NCU_DRAM_BYTES_PER_LAUNCH = {"back": 143.98e6, "forward": 302.43e6, "tv_grad": 98.07e6, "tv_trial": 137.87e6,
-                             "tv_update": 166.45e6}
+# capture of this command (profiles/r01c_ncu_full_summary.txt); None = not captured for that kernel.
+NCU_DRAM_BYTES_PER_LAUNCH = {"back": 149.14e6, "forward": 120.92e6, "tv_grad": 98.34e6, "tv_trial": 138.37e6,
+                             "tv_update": 166.68e6}
 
 
 def _peaks():
@@ -467,7 +467,7 @@ def run_sweep(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
