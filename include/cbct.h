@@ -184,6 +184,9 @@ typedef struct {
     int backprojector; /* CBCT_BACKPROJECTOR_EXACT (0): g = f - tau c_norm P^T T, the matched pair;
                           CBCT_BACKPROJECTOR_EQ6 (1): g = f - tau c_norm b6(T), the paper's Eq. 6 (unmatched pair;
                           Lhat is still the matched pair's bound) */
+    double conv_tol;   /* NEXT-2, "until convergence" (L145, L223; reading S20): 0 = run iters_per_level[] iterations;
+                          > 0: a level also stops after the first iteration with
+                          ||f_new - f_old||_2 <= conv_tol ||f_old||_2 (iters_per_level[] is then the cap) */
     cbct_tv_params tv;
 } cbct_fbs_params;
 
@@ -192,6 +195,9 @@ typedef struct {
     double *objective;   /* caller-owned HOST array of sum(iters) doubles or NULL:
                             objective[it] = tv_weight*E1(f) + E2(f) of the f entering iteration it */
     double *step_abs;    /* caller-owned HOST array of n_levels doubles or NULL: tau per level */
+    int *iters_done;     /* caller-owned HOST array of n_levels ints or NULL: iterations run per level, coarsest ->
+                            finest (= iters_per_level[] unless conv_tol stopped a level early); objective[] holds
+                            sum(iters_done) entries in that order */
     int inner_total, trials_total; /* summed over all TV-prox calls */
     float ms_total;      /* device time of the whole call (CUDA events on the stream) */
 } cbct_fbs_report;

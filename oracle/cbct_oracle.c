@@ -565,8 +565,8 @@ double oracle_step_bound(const ogeom *g)
 /* n_iter iterations at one level.  objective[it] = tv_weight * E1^delta(f) +
  * E2(f) for the f that ENTERS iteration it (may be NULL).  Returns tau. */
 double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_weight, double step,
-                        int n_iter, int nonneg, int use_eq6, const otv_params *tp, double *objective,
-                        int *inner_total, int *trials_total)
+                        int n_iter, int nonneg, int use_eq6, double conv_tol, const otv_params *tp,
+                        double *objective, int *inner_total, int *trials_total, int *iters_done)
 {
     long nvox = (long)g->nx * g->ny * g->nz, nray = (long)g->n_proj * g->nv * g->nu;
     double c_norm = 2.0 * (double)nvox / (double)nray;
@@ -574,7 +574,10 @@ double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_we
     double tau = step / Lhat, w = tau * tv_weight;
     double *T = malloc(sizeof(double) * nray), *b = malloc(sizeof(double) * nvox);
     double *gg = malloc(sizeof(double) * nvox);
+    double *prev = malloc(sizeof(double) * nvox);
+    int done = 0;
     for (int it = 0; it < n_iter; ++it) {
+        memcpy(prev, f, sizeof(double) * nvox);
         oracle_forward(g, f, T);
         double E2 = 0.0;
         for (long r = 0; r < nray; ++r) { T[r] -= y[r]; E2 += T[r] * T[r]; }
@@ -589,8 +592,15 @@ double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_we
         if (trials_total) *trials_total += rep.trials;
         if (nonneg)
             for (long v = 0; v < nvox; ++v) if (f[v] < 0.0) f[v] = 0.0;
+        ++done;
+        if (conv_tol > 0.0) {   /* "until convergence" (L145, L223; reading S20): relative change of the volume */
+            double d2 = 0.0, p2 = 0.0;
+            for (long v = 0; v < nvox; ++v) { double d = f[v] - prev[v]; d2 += d * d; p2 += prev[v] * prev[v]; }
+            if (p2 > 0.0 && d2 <= conv_tol * conv_tol * p2) break;
+        }
     }
-    free(T); free(b); free(gg);
+    if (iters_done) *iters_done = done;
+    free(T); free(b); free(gg); free(prev);
     return tau;
 }
 
@@ -602,9 +612,9 @@ double oracle_fbs_level(const ogeom *g, const double *y, double *f, double tv_we
  * sum(iters) entries (may be NULL); step_abs[n_levels] receives tau per level
  * in the same coarsest -> finest order (may be NULL). */
 void oracle_fbs(const ogeom *g0, const double *y0, double *f, double tv_weight, double step,
-                int n_levels, const int *iters, int nonneg, int use_initial, int use_eq6,
+                int n_levels, const int *iters, int nonneg, int use_initial, int use_eq6, double conv_tol,
                 const otv_params *tp, double *objective, double *step_abs, int *inner_total,
-                int *trials_total)
+                int *trials_total, int *iters_done)
 {
     ogeom *gl = malloc(sizeof(ogeom) * n_levels);
     double **yl = malloc(sizeof(double *) * n_levels);
@@ -632,10 +642,12 @@ void oracle_fbs(const ogeom *g0, const double *y0, double *f, double tv_weight, 
     int done = 0;
     for (int l = n_levels - 1; l >= 0; --l) {
         int n_it = iters[n_levels - 1 - l];
-        double tau = oracle_fbs_level(&gl[l], yl[l], cur, tv_weight, step, n_it, nonneg, use_eq6, tp,
-                                      objective ? objective + done : NULL, inner_total, trials_total);
+        int ran = 0;
+        double tau = oracle_fbs_level(&gl[l], yl[l], cur, tv_weight, step, n_it, nonneg, use_eq6, conv_tol, tp,
+                                      objective ? objective + done : NULL, inner_total, trials_total, &ran);
         if (step_abs) step_abs[n_levels - 1 - l] = tau;
-        done += n_it;
+        if (iters_done) iters_done[n_levels - 1 - l] = ran;
+        done += ran;
         if (l > 0) {
             double *fine = malloc(sizeof(double) * (long)gl[l - 1].nx * gl[l - 1].ny * gl[l - 1].nz);
             oracle_prolong(gl[l].nx, gl[l].ny, gl[l].nz, g0->bc_xy, g0->bc_z, cur, fine);

@@ -280,6 +280,7 @@ class FbsResult:
     step_abs: np.ndarray
     inner_total: int
     trials_total: int
+    iters_done: tuple = ()
 
 
 def fbs(g, y, fbs_setup, f0=None):
@@ -293,9 +294,11 @@ def fbs(g, y, fbs_setup, f0=None):
     step_abs = np.zeros(n_levels)
     tp = _tvp(fbs_setup)
     inner = C.c_int(0); trials = C.c_int(0)
+    done = np.zeros(n_levels, dtype=np.int32)
     lib().oracle_fbs(C.byref(s), _p(y), _p(f), C.c_double(fbs_setup.tv_weight),
                      C.c_double(fbs_setup.step), n_levels, iters.ctypes.data_as(C.POINTER(C.c_int)),
                      int(bool(fbs_setup.nonneg)), int(f0 is not None),
-                     int(getattr(fbs_setup, "backprojector", 0)), C.byref(tp), _p(obj),
-                     _p(step_abs), C.byref(inner), C.byref(trials))
-    return FbsResult(f, obj, step_abs, inner.value, trials.value)
+                     int(getattr(fbs_setup, "backprojector", 0)),
+                     C.c_double(float(getattr(fbs_setup, "conv_tol", 0.0))), C.byref(tp), _p(obj),
+                     _p(step_abs), C.byref(inner), C.byref(trials), done.ctypes.data_as(C.POINTER(C.c_int)))
+    return FbsResult(f, obj[:int(done.sum())], step_abs, inner.value, trials.value, tuple(int(x) for x in done))

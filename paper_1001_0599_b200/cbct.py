@@ -65,12 +65,12 @@ class _TvReport(C.Structure):
 class _FbsParams(C.Structure):
     _fields_ = [("tv_weight", C.c_double), ("step", C.c_double), ("n_levels", C.c_int),
                 ("iters_per_level", C.POINTER(C.c_int)), ("nonneg", C.c_int), ("use_initial", C.c_int),
-                ("backprojector", C.c_int), ("tv", _TvParams)]
+                ("backprojector", C.c_int), ("conv_tol", C.c_double), ("tv", _TvParams)]
 
 
 class _FbsReport(C.Structure):
     _fields_ = [("n_iters_total", C.c_int), ("objective", C.POINTER(C.c_double)),
-                ("step_abs", C.POINTER(C.c_double)), ("inner_total", C.c_int), ("trials_total", C.c_int),
+                ("step_abs", C.POINTER(C.c_double)), ("iters_done", C.POINTER(C.c_int)), ("inner_total", C.c_int), ("trials_total", C.c_int),
                 ("ms_total", C.c_float)]
 
 
@@ -90,6 +90,7 @@ class FbsReport:
     inner_total: int
     trials_total: int
     ms_total: float
+    iters_done: tuple = ()
 
 
 _lib = None
@@ -304,18 +305,22 @@ class Geometry:
         p.iters_per_level = iters.ctypes.data_as(C.POINTER(C.c_int))
         p.nonneg, p.use_initial = int(bool(fbs.nonneg)), int(bool(use_initial))
         p.backprojector = int(getattr(fbs, "backprojector", 0))
+        p.conv_tol = float(getattr(fbs, "conv_tol", 0.0))
         p.tv = _tv_params(fbs)
         obj = np.zeros(int(iters.sum()) if want_objective else 0)
         step_abs = np.zeros(len(iters))
+        done = np.zeros(len(iters), dtype=np.int32)
         r = _FbsReport()
+        r.iters_done = done.ctypes.data_as(C.POINTER(C.c_int))
         r.objective = obj.ctypes.data_as(C.POINTER(C.c_double)) if want_objective else None
         r.step_abs = step_abs.ctypes.data_as(C.POINTER(C.c_double))
-        return p, r, (iters, obj, step_abs)
+        return p, r, (iters, obj, step_abs, done)
 
     @staticmethod
     def _fbs_report(r, keep):
-        _, obj, step_abs = keep
-        return FbsReport(r.n_iters_total, obj, step_abs, r.inner_total, r.trials_total, float(r.ms_total))
+        _, obj, step_abs, done = keep
+        return FbsReport(r.n_iters_total, obj[:int(done.sum())] if len(obj) else obj, step_abs, r.inner_total,
+                         r.trials_total, float(r.ms_total), tuple(int(x) for x in done))
 
     def fbs_reconstruct(self, proj_y, vol_inout, fbs, use_initial: bool = False, objective: bool = True,
                         stream=None) -> FbsReport:

@@ -71,6 +71,7 @@ struct Level {
     float *d_d = nullptr;       // descent direction of the ROF sub-solver
     float *d_f2 = nullptr;      // second volume (ping-pong / level volume)
     float *d_f = nullptr;       // level volume for levels > 0 and for the host entry point
+    float *d_prev = nullptr;    // the volume that entered the current iteration (convergence test, NEXT-2)
     float *d_y = nullptr;       // binned data for levels > 0; staging for level 0 host entry
     mutable double lhat = -1.0; // A5 step bound: a property of the geometry alone, computed on first use
 };
@@ -161,6 +162,9 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
 // back_eq6.cu : out = f - coef * b6(T) with T in the plain [view][row][column] layout (f may be NULL: out = b6(T))
 cbct_status launch_back_eq6(const cbct_geometry *g, const Level &L, const float *d_T, const float *d_f, float coef,
                             float *d_out, cudaStream_t st);
+// metrics.cu : *sum_d2 = sum (a - b)^2, *sum_b2 = sum b^2 over n elements (fp64, fixed order); synchronises the stream
+cbct_status volume_change(const cbct_geometry *g, size_t n, const float *d_a, const float *d_b, double *sum_d2,
+                          double *sum_b2, cudaStream_t st);
 // tv.cu
 cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,

@@ -45,6 +45,9 @@ cbct_status check_params(const cbct_geometry *g, const cbct_fbs_params *p)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: more than %d iterations in one call", g->objective_cap);
     if (!(p->tv_weight >= 0.0) || !(p->step > 0.0 && p->step < 2.0))
         return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: need tv_weight >= 0 and 0 < step < 2");
+    if (!(p->conv_tol >= 0.0)) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: conv_tol must be >= 0");
+    if (p->backprojector != CBCT_BACKPROJECTOR_EXACT && p->backprojector != CBCT_BACKPROJECTOR_EQ6)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: unknown backprojector %d", p->backprojector);
     if (p->tv.max_inner < 0 || p->tv.max_backtracks < 0 || !(p->tv.shrink_alpha > 0.0 && p->tv.shrink_alpha < 1.0))
         return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: bad TV parameters");
     return CBCT_OK;
@@ -79,6 +82,7 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
 
     const bool eq6 = p->backprojector == CBCT_BACKPROJECTOR_EQ6;
     int done = 0, inner_total = 0, trials_total = 0;
+    int iters_done[8] = {0, 0, 0, 0, 0, 0, 0, 0};      // per level, coarsest -> finest (max_levels <= 8)
     for (int l = nl - 1; l >= 0; --l) {
         const Level &L = g->levels[l];
         float *f = (l == 0) ? d_vol : L.d_f;
@@ -92,7 +96,10 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         const double c_norm = 2.0 * (double)L.nvox / (double)L.nray;
         const double tau = p->step / lhat, w = tau * p->tv_weight;
         if (rep && rep->step_abs) rep->step_abs[nl - 1 - l] = tau;
+        int it_done = 0;
         for (int it = 0; it < n_it; ++it, ++done) {
+            if (p->conv_tol > 0.0)      // keep the volume that enters the iteration for the convergence test
+                CBCT_CUDA(cudaMemcpyAsync(L.d_prev, f, L.nvox * sizeof(float), cudaMemcpyDeviceToDevice, st));
             {
                 if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
             }
@@ -110,7 +117,15 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
                 inner_total += tr.inner_iters;
                 trials_total += tr.trials;
             }
+            ++it_done;
+            if (p->conv_tol > 0.0) {    // "until convergence" (L145; reading S20): relative change of the volume
+                double d2 = 0.0, p2 = 0.0;
+                if ((s = volume_change(g, L.nvox, f, L.d_prev, &d2, &p2, st)) != CBCT_OK) return s;
+                if (p2 > 0.0 && d2 <= p->conv_tol * p->conv_tol * p2) { ++done; break; }
+            }
         }
+        iters_done[nl - 1 - l] = it_done;
+        if (rep && rep->iters_done) rep->iters_done[nl - 1 - l] = it_done;
         if (l > 0) {
             float *fine = (l == 1) ? d_vol : g->levels[l - 1].d_f;
             if ((s = launch_prolong(g, g->levels[l - 1], L.d_f, fine, st)) != CBCT_OK) return s;
@@ -130,7 +145,7 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
             int idx = 0;
             for (int l = nl - 1; l >= 0; --l) {
                 const Level &L = g->levels[l];
-                for (int it = 0; it < p->iters_per_level[nl - 1 - l]; ++it, ++idx)
+                for (int it = 0; it < iters_done[nl - 1 - l]; ++it, ++idx)
                     rep->objective[idx] = p->tv_weight * h[2 * idx] / (double)L.nvox + h[2 * idx + 1] / (double)L.nray;
             }
         }

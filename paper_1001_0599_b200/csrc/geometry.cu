@@ -114,7 +114,7 @@ static void free_all(cbct_geometry *g)
     if (!g) return;
     for (Level &L : g->levels) {
         cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_cs); cudaFree(L.d_stage); cudaFree(L.d_T);
-        cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_y);
+        cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_prev); cudaFree(L.d_y);
     }
     cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter);
     if (g->h_scalars) cudaFreeHost(g->h_scalars);
@@ -213,6 +213,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         TRY(dev_alloc(g, &L.d_d, L.nvox));
         TRY(dev_alloc(g, &L.d_f2, L.nvox));
         TRY(dev_alloc(g, &L.d_f, L.nvox));
+        TRY(dev_alloc(g, &L.d_prev, L.nvox));
         TRY(dev_alloc(g, &L.d_y, L.nray));
         cudaError_t e = cudaMemcpy(L.d_rayu, rays.data(), rays.size() * sizeof(RayU), cudaMemcpyHostToDevice);
         if (e == cudaSuccess)

@@ -25,23 +25,39 @@ quality_metrics_kernel(size_t n, const float *__restrict__ f, const float *__res
     publish_and_finalize<6>(v, 6, partials, (int)gridDim.x, counter, out, slot);
 }
 
-// out[0..5] = the six sums; the caller forms e and c on the host from the fp64 sums (a handful of flops)
+static cbct_status six_sums(const cbct_geometry *g, size_t n, const float *d_a, const float *d_b, cudaStream_t st)
+{
+    int blocks = g->sm_count * MET_BLOCKS_PER_SM;
+    if ((size_t)blocks * 6 > (size_t)4 * g->partials_stride) blocks = 4 * g->partials_stride / 6;
+    {
+        StageTimer t(g, st, ST_REDUCE);
+        quality_metrics_kernel<<<blocks, MET_THREADS, 0, st>>>(n, d_a, d_b, g->d_partials, g->d_counter, g->d_scalars);
+        CBCT_LAUNCH_CHECK(g);
+    }
+    CBCT_CUDA(cudaMemcpyAsync(g->h_scalars, g->d_scalars, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
+cbct_status volume_change(const cbct_geometry *g, size_t n, const float *d_a, const float *d_b, double *sum_d2,
+                          double *sum_b2, cudaStream_t st)
+{
+    cbct_status s = six_sums(g, n, d_a, d_b, st);
+    if (s != CBCT_OK) return s;
+    *sum_d2 = g->h_scalars[5];
+    *sum_b2 = g->h_scalars[3];
+    return CBCT_OK;
+}
+
+// the six sums come back to the host, which forms e and c from them (a handful of fp64 flops)
 extern "C" cbct_status cbct_quality_metrics(const cbct_geometry *g, int level, const float *d_f, const float *d_f0,
                                             double *rel_error, double *correlation, void *cuda_stream)
 {
     const Level *L = get_level(g, level);
     if (!L || !d_f || !d_f0 || !rel_error || !correlation)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_quality_metrics: bad handle, level or NULL");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    int blocks = g->sm_count * MET_BLOCKS_PER_SM;
-    if ((size_t)blocks * 6 > (size_t)4 * g->partials_stride) blocks = 4 * g->partials_stride / 6;
-    {
-        StageTimer t(g, st, ST_REDUCE);
-        quality_metrics_kernel<<<blocks, MET_THREADS, 0, st>>>(L->nvox, d_f, d_f0, g->d_partials, g->d_counter, g->d_scalars);
-        CBCT_LAUNCH_CHECK(g);
-    }
-    CBCT_CUDA(cudaMemcpyAsync(g->h_scalars, g->d_scalars, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    CBCT_CUDA(cudaStreamSynchronize(st));
+    cbct_status s = six_sums(g, L->nvox, d_f, d_f0, (cudaStream_t)cuda_stream);
+    if (s != CBCT_OK) return s;
     const double *h = g->h_scalars, n = (double)L->nvox;
     *rel_error = h[3] > 0.0 ? sqrt(h[5] / h[3]) : 0.0;
     const double cov = h[4] - h[0] * h[1] / n, va = h[2] - h[0] * h[0] / n, vb = h[3] - h[1] * h[1] / n;

@@ -98,6 +98,7 @@ class FbsSetup:
     shrink_alpha: float = 0.6
     rel_tol: float = 1e-3
     backprojector: int = 0    # 0: exact transpose P^T (matched pair); 1: the paper's Eq. 6
+    conv_tol: float = 0.0     # > 0: a level stops once ||f_new - f_old|| <= conv_tol ||f_old||
 
 
 @dataclass

@@ -367,3 +367,22 @@ def test_fbs_with_the_papers_eq6_gradient_matches_oracle(torch, cbct, orc):
     # and it is a different iteration from the matched pair's
     exact = orc.fbs(g, y, I.FbsSetup(iters_per_level=(5, 4), step=0.8))
     assert rel_l2(want.f, exact.f) > 1e-3
+
+
+def test_fbs_convergence_stopping_matches_oracle(torch, cbct, orc):
+    """NEXT-2: 'until convergence' with the relative-change test, two levels; same iteration counts, same volume."""
+    g = I.Geometry(nx=48, ny=48, nz=32, hx=2.0, hy=2.0, hz=2.5, nu=64, nv=48, du=2.4, dv=2.4, sad=1000.0,
+                   sdd=1500.0, n_proj=10)
+    ell = [I.Ellipsoid((0.0, 0.0, 0.0), (40.0, 34.0, 36.0), 0.0, 0.02)] + \
+        I.random_ellipsoids(np.random.default_rng(91), 6, (48.0, 48.0, 40.0), axes_range=(4.0, 14.0))
+    y = I.poisson_log(I.analytic_projections(ell, g), 1e5, 92).astype(np.float32)
+    setup = I.FbsSetup(iters_per_level=(30, 30), conv_tol=0.03)
+    want = orc.fbs(g, y, setup)
+    with cbct.geometry_create(g, max_levels=2) as h:
+        f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+        rep = h.fbs_reconstruct(dev(torch, y), f, setup)
+        got = f.cpu().numpy()
+    assert rep.iters_done == want.iters_done and all(0 < n < 30 for n in rep.iters_done)
+    assert rep.n_iters_total == sum(want.iters_done) and len(rep.objective) == len(want.objective)
+    assert rel_l2(got, want.f) <= TOL_VOL
+    np.testing.assert_allclose(rep.objective, want.objective, rtol=1e-4)

@@ -92,3 +92,20 @@ def test_multigrid_driver_structure(orc):
     cb = orc.fbs(gc, orc.bin2(y), I.FbsSetup(iters_per_level=(2,)), f0=orc.restrict(f0))
     b = orc.fbs(g, y, I.FbsSetup(iters_per_level=(1,)), f0=orc.prolong(cb.f, g.bc_xy, g.bc_z))
     np.testing.assert_allclose(a.f, b.f, rtol=0, atol=1e-15)
+
+
+def test_convergence_stopping_is_the_fixed_count_run_cut_at_the_first_small_change(orc):
+    """NEXT-2, 'until convergence' (reading S20): with conv_tol the level stops after the first
+    iteration whose relative change ||f_new - f_old|| / ||f_old|| is <= conv_tol.  Pinned against runs with FIXED
+    counts (which do not execute the test): the stopped run equals the n-iteration run, its last change is below the
+    tolerance and every earlier change above it."""
+    cfg = I.config(1)
+    y = I.make_projections(cfg)
+    tol = 0.05
+    r = orc.fbs(cfg.geom, y, I.FbsSetup(iters_per_level=(40,), conv_tol=tol))
+    n = r.iters_done[0]
+    assert 2 < n < 40 and len(r.objective) == n
+    runs = [orc.fbs(cfg.geom, y, I.FbsSetup(iters_per_level=(m,))).f for m in range(1, n + 1)]
+    assert np.array_equal(r.f, runs[-1])
+    change = [np.linalg.norm(runs[m] - runs[m - 1]) / np.linalg.norm(runs[m - 1]) for m in range(1, n)]
+    assert change[-1] <= tol and all(c > tol for c in change[:-1])
