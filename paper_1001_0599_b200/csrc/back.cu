@@ -62,6 +62,78 @@ constexpr int BK_BX = 8;       // block: one warp (lanes along z) per i, 8 conse
 // The row's weight is the overlap of [s_lo, s_hi] with the t-interval between its crossings of the
 // voxel's two z-planes, t = z_plane / (v q) - (d0 - sd): the same crossing parameters as
 // forward.cu's, written relative to the source so that one reciprocal serves both planes.
+// One detector column's contribution to the KT voxels of a thread.  In: the slab interval [s_lo, s_hi] of the column's ray
+// above the voxel's (i,j) square, e = slab start relative to the source, q, inv_dd of the ray, 1/c at the two ends of
+// the interval, and the 32-bit entry offset oA of the column's row 0 in the residual stack T (float4 entries for
+// R == 4, floats for R == 1).  SG = the voxel image the interval belongs to: its weights serve the pairs
+// (view a + r nbase, image SG + r); the mirror voxel sees the mirror row nv-1-iv with the same weight.
+template <int R, int M, int KT, int SG>
+__device__ __forceinline__ void gather_column(float (&acc)[KT][R * M], const float (&zl)[KT], const LevelParams &P,
+                                              const float *__restrict__ T, float c0v, float s_lo, float s_hi, float e,
+                                              float q, float inv_dd, float ic_near, float ic_far, int oA)
+{
+    const float tiny = copysignf(1.0e-37f, q);            // a row with v == 0 counts as v = 0+
+    const int oB = oA + P.nv - 1;                         // row nv-1
+#pragma unroll
+    for (int t = 0; t < KT; ++t) {
+        const float zlo = zl[t], zhi = zlo + 1.0f;
+        const float v_lo = zlo * (zlo >= 0.0f ? ic_far : ic_near);
+        const float v_hi = zhi * (zhi >= 0.0f ? ic_near : ic_far);
+        int iv = max(0, __float2int_ru(fmaf(v_lo, P.inv_dv, c0v) - 2.0e-3f));
+        const int iv_hi = min(P.nv - 1, __float2int_rd(fmaf(v_hi, P.inv_dv, c0v) + 2.0e-3f));
+        if (iv > iv_hi) continue;
+        // overlap of [s_lo, s_hi] with the t-interval between the row's crossings of the voxel's z-planes,
+        // times the slab length per unit of L (inv_dd); rows of the exact range always overlap
+        auto weight = [&](int row) {
+            const float v = fmaf((float)row, P.dv, P.v0);
+            float inv;
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(fmaf(v, q, tiny)));
+            const float q1 = fmaf(zlo, inv, -e), q2 = fmaf(zhi, inv, -e);
+            const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
+            return fmaxf(hi - lo, 0.0f) * inv_dd;
+        };
+        auto gather = [&](float w, const float4 &tA, const float4 &tB) {
+            acc[t][(SG + 0) % R] = fmaf(w, tA.x, acc[t][(SG + 0) % R]);
+            if (R == 4) {
+                acc[t][(SG + 1) % R] = fmaf(w, tA.y, acc[t][(SG + 1) % R]);
+                acc[t][(SG + 2) % R] = fmaf(w, tA.z, acc[t][(SG + 2) % R]);
+                acc[t][(SG + 3) % R] = fmaf(w, tA.w, acc[t][(SG + 3) % R]);
+            }
+            if (M == 2) {
+                acc[t][R + (SG + 0) % R] = fmaf(w, tB.x, acc[t][R + (SG + 0) % R]);
+                if (R == 4) {
+                    acc[t][R + (SG + 1) % R] = fmaf(w, tB.y, acc[t][R + (SG + 1) % R]);
+                    acc[t][R + (SG + 2) % R] = fmaf(w, tB.z, acc[t][R + (SG + 2) % R]);
+                    acc[t][R + (SG + 3) % R] = fmaf(w, tB.w, acc[t][R + (SG + 3) % R]);
+                }
+            }
+        };
+        auto fetch = [&](int o) {
+            if (R == 4) return __ldg(reinterpret_cast<const float4 *>(T) + o);
+            return make_float4(__ldg(T + o), 0.0f, 0.0f, 0.0f);
+        };
+        // the first two rows together (about two rows cross a voxel): both weights, then all four
+        // loads, then the FMAs; a voxel with one row reads it twice with the second weight 0
+        {
+            const bool two = iv < iv_hi;
+            const int ivb = two ? iv + 1 : iv;
+            const float w0 = weight(iv), w1 = two ? weight(ivb) : 0.0f;
+            const float4 a0 = fetch(oA + iv), a1 = fetch(oA + ivb);
+            float4 b0 = a0, b1 = a1;
+            if (M == 2) { b0 = fetch(oB - iv); b1 = fetch(oB - ivb); }
+            gather(w0, a0, b0);
+            gather(w1, a1, b1);
+        }
+        for (iv += 2; iv <= iv_hi; ++iv) {
+            const float w = weight(iv);
+            const float4 a0 = fetch(oA + iv);
+            float4 b0 = a0;
+            if (M == 2) b0 = fetch(oB - iv);
+            gather(w, a0, b0);
+        }
+    }
+}
+
 template <int R, int M, int KT>
 __global__ void __launch_bounds__(32 * BK_BX, 3)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
@@ -95,10 +167,8 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
 #pragma unroll
         for (int q = 0; q < R * M; ++q) acc[t][q] = 0.0f;
     const float c0v = -P.v0 * P.inv_dv;
-    const size_t plane = (size_t)P.nv * P.nu;
     for (int a = 0; a < P.nbase; ++a) {
         const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);   // c, s, dn, du
-        const float *__restrict__ Ta = TL + (size_t)a * plane * R;
 #pragma unroll
         for (int sg = 0; sg < R; ++sg) {
             const float xc = fmaf((float)vi[sg], P.hx, P.x0), yc = fmaf((float)vj[sg], P.hy, P.y0);
@@ -126,70 +196,145 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
                 asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icA) : "f"(r.q * (e + s_lo)));
                 asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icB) : "f"(r.q * (e + s_hi)));
                 const float ic_near = fmaxf(icA, icB), ic_far = fminf(icA, icB);     // 1/c at the end nearer to / farther from the source
-                const float tiny = copysignf(1.0e-37f, r.q);            // a row with v == 0 counts as v = 0+
-                const int oA = iu * P.nv, oB = oA + P.nv - 1;              // 32-bit entry offsets of rows 0 and nv-1
-#pragma unroll
-                for (int t = 0; t < KT; ++t) {
-                    const float zlo = zl[t], zhi = zlo + 1.0f;
-                    const float v_lo = zlo * (zlo >= 0.0f ? ic_far : ic_near);
-                    const float v_hi = zhi * (zhi >= 0.0f ? ic_near : ic_far);
-                    int iv = max(0, __float2int_ru(fmaf(v_lo, P.inv_dv, c0v) - 2.0e-3f));
-                    const int iv_hi = min(P.nv - 1, __float2int_rd(fmaf(v_hi, P.inv_dv, c0v) + 2.0e-3f));
-                    if (iv > iv_hi) continue;
-                    // overlap of [s_lo, s_hi] with the t-interval between the row's crossings of the voxel's z-planes,
-                    // times the slab length per unit of L (inv_dd); rows of the exact range always overlap
-                    auto weight = [&](int row) {
-                        const float v = fmaf((float)row, P.dv, P.v0);
-                        float inv;
-                        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(fmaf(v, r.q, tiny)));
-                        const float q1 = fmaf(zlo, inv, -e), q2 = fmaf(zhi, inv, -e);
-                        const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
-                        return fmaxf(hi - lo, 0.0f) * r.inv_dd;
-                    };
-                    // weights of image sg under base view a serve the pairs (view a + r nbase, image sg + r);
-                    // the mirror voxel sees the mirror row with the same weight
-                    auto gather = [&](float w, const float4 &tA, const float4 &tB) {
-                        acc[t][(sg + 0) % R] = fmaf(w, tA.x, acc[t][(sg + 0) % R]);
-                        if (R == 4) {
-                            acc[t][(sg + 1) % R] = fmaf(w, tA.y, acc[t][(sg + 1) % R]);
-                            acc[t][(sg + 2) % R] = fmaf(w, tA.z, acc[t][(sg + 2) % R]);
-                            acc[t][(sg + 3) % R] = fmaf(w, tA.w, acc[t][(sg + 3) % R]);
-                        }
-                        if (M == 2) {
-                            acc[t][R + (sg + 0) % R] = fmaf(w, tB.x, acc[t][R + (sg + 0) % R]);
-                            if (R == 4) {
-                                acc[t][R + (sg + 1) % R] = fmaf(w, tB.y, acc[t][R + (sg + 1) % R]);
-                                acc[t][R + (sg + 2) % R] = fmaf(w, tB.z, acc[t][R + (sg + 2) % R]);
-                                acc[t][R + (sg + 3) % R] = fmaf(w, tB.w, acc[t][R + (sg + 3) % R]);
-                            }
-                        }
-                    };
-                    auto fetch = [&](int o) {
-                        if (R == 4) return __ldg(reinterpret_cast<const float4 *>(Ta) + o);
-                        return make_float4(__ldg(Ta + o), 0.0f, 0.0f, 0.0f);
-                    };
-                    // the first two rows together (about two rows cross a voxel): both weights, then all four
-                    // loads, then the FMAs; a voxel with one row reads it twice with the second weight 0
-                    {
-                        const bool two = iv < iv_hi;
-                        const int ivb = two ? iv + 1 : iv;
-                        const float w0 = weight(iv), w1 = two ? weight(ivb) : 0.0f;
-                        const float4 a0 = fetch(oA + iv), a1 = fetch(oA + ivb);
-                        float4 b0 = a0, b1 = a1;
-                        if (M == 2) { b0 = fetch(oB - iv); b1 = fetch(oB - ivb); }
-                        gather(w0, a0, b0);
-                        gather(w1, a1, b1);
-                    }
-                    for (iv += 2; iv <= iv_hi; ++iv) {
-                        const float w = weight(iv);
-                        const float4 a0 = fetch(oA + iv);
-                        float4 b0 = a0;
-                        if (M == 2) b0 = fetch(oB - iv);
-                        gather(w, a0, b0);
-                    }
-                }
+                const int oA = (a * P.nu + iu) * P.nv;                  // 32-bit entry offset of the column's row 0
+                if (sg == 0) gather_column<R, M, KT, 0>(acc, zl, P, TL, c0v, s_lo, s_hi, e, r.q, r.inv_dd, ic_near, ic_far, oA);
+                else if (sg == 1) gather_column<R, M, KT, 1 % R>(acc, zl, P, TL, c0v, s_lo, s_hi, e, r.q, r.inv_dd, ic_near, ic_far, oA);
+                else if (sg == 2) gather_column<R, M, KT, 2 % R>(acc, zl, P, TL, c0v, s_lo, s_hi, e, r.q, r.inv_dd, ic_near, ic_far, oA);
+                else gather_column<R, M, KT, 3 % R>(acc, zl, P, TL, c0v, s_lo, s_hi, e, r.q, r.inv_dd, ic_near, ic_far, oA);
             }
         }
+    }
+#pragma unroll
+    for (int t = 0; t < KT; ++t)
+#pragma unroll
+        for (int mm = 0; mm < M; ++mm)
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                const float v = acc[t][mm * R + q];
+                if (kv[t] < nzh) {
+                    const size_t o = ((size_t)(mm ? P.nz - 1 - kv[t] : kv[t]) * P.ny + vj[q]) * P.nx + vi[q];
+                    out[o] = f ? fmaf(-coef, v, __ldg(f + o)) : v;
+                }
+            }
+}
+
+// The same back-projector with the in-plane part taken out of the warp-uniform instruction stream.  In back_kernel
+// every lane of a warp repeats the in-plane arithmetic of its (i,j) (about a fifth of all instructions at 256^3); here
+// the lanes of the warp first work through DIFFERENT (base view, voxel image) pairs -- 32 / R base views per round --
+// and append the columns that hit to a per-warp list in shared memory (s_lo, s_hi, e, q | 1/c near, 1/c far, inv_dd,
+// entry offset), in a fixed order (candidate index, then lane): ballot + popc, no atomics.  Then all lanes walk the
+// list (broadcast reads) and gather their KT voxels as before.  A round holds at most BK_MAXC candidate columns per
+// pair (checked at launch against the geometry; larger shadows take back_kernel).
+constexpr int BK_MAXC = 5, BK_LIST = 32 * BK_MAXC;      // list entries per warp and round (all images together)
+
+#ifndef BACK_MINB
+#define BACK_MINB 3
+#endif
+template <int R, int M, int KT>
+__global__ void __launch_bounds__(32 * BK_BX, BACK_MINB)
+back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
+                 const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
+{
+    __shared__ float4 s_list[BK_BX][2][BK_LIST];
+    constexpr int LCAP = BK_LIST / R;                 // per image: (32 / R) base views x BK_MAXC
+    const int lane = threadIdx.x;
+    const int i = blockIdx.x * BK_BX + threadIdx.y;
+    const int j = blockIdx.y;
+    const int ni = R == 4 ? P.nx / 2 : P.nx;
+    const int nzh = P.nz / M;
+    if (i >= ni) return;                             // warp-uniform
+    float4 *__restrict__ l0 = s_list[threadIdx.y][0], *__restrict__ l1 = s_list[threadIdx.y][1];
+    int kv[KT];
+    float zl[KT];
+#pragma unroll
+    for (int t = 0; t < KT; ++t) {
+        kv[t] = blockIdx.z * (32 * KT) + lane + 32 * t;
+        zl[t] = (float)(min(kv[t], nzh - 1) - P.cz) - P.sz;
+    }
+    int vi[R], vj[R];
+    vi[0] = i; vj[0] = j;
+    if (R == 4) {
+        const int n1 = P.nx - 1;
+        vi[1 % R] = n1 - j; vj[1 % R] = i;
+        vi[2 % R] = n1 - i; vj[2 % R] = n1 - j;
+        vi[3 % R] = j;      vj[3 % R] = n1 - i;
+    }
+    float acc[KT][R * M];
+#pragma unroll
+    for (int t = 0; t < KT; ++t)
+#pragma unroll
+        for (int q = 0; q < R * M; ++q) acc[t][q] = 0.0f;
+    const float c0v = -P.v0 * P.inv_dv;
+    // this lane's pair in a round: image my_sg of base view a0 + lane / R
+    const int my_sg = lane % R;
+    int mi = vi[0], mj = vj[0];
+#pragma unroll
+    for (int q = 1; q < R; ++q) if (my_sg == q) { mi = vi[q]; mj = vj[q]; }
+    const float xc = fmaf((float)mi, P.hx, P.x0), yc = fmaf((float)mj, P.hy, P.y0);
+    const float bx = (float)(mi - P.cx), by = (float)(mj - P.cy);
+    const unsigned lt_mask = (1u << lane) - 1u;
+    const unsigned all_sg = R == 4 ? 0x11111111u : 0xffffffffu;      // lanes that hold image 0
+    const unsigned my_mask = all_sg << my_sg;
+    for (int a0 = 0; a0 < P.nbase; a0 += 32 / R) {
+        int cnt[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) cnt[q] = 0;
+        const int a = a0 + lane / R;
+        int iu_lo = 0, ncand = 0;
+        if (a < P.nbase) {
+            const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);   // c, s, dn, du
+            const float rn = fmaf(xc, vw.x, fmaf(yc, vw.y, P.sad));   // (X - S).e_n  > 0
+            const float ru = fmaf(xc, vw.y, -yc * vw.x);               // (X - S).e_u
+            float rinv;
+            asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rinv) : "f"(rn));
+            const float mag = P.sdd * rinv, tn = ru * rinv;
+            const float uc = mag * ru, W = mag * fmaf(fabsf(tn), vw.z, vw.w);
+            iu_lo = max(0, __float2int_ru((uc - W - P.u0) * P.inv_du - 0.02f));
+            const int iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
+            ncand = min(iu_hi - iu_lo + 1, BK_MAXC);
+        }
+        for (int c = 0; __any_sync(0xffffffffu, c < ncand); ++c) {
+            bool ok = c < ncand;
+            float4 e0 = make_float4(0.f, 0.f, 0.f, 0.f), e1 = e0;
+            if (ok) {
+                const int iu = iu_lo + c;
+                const RayU r = load_rayu(rayu, a * P.nu + iu);
+                const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;   // slab coordinate, minor plane
+                const float y0 = fmaf(d0, r.m, r.a0);
+                const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
+                const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
+                ok = s_hi > s_lo;
+                const float e = d0 - r.sd;
+                float icA, icB;
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icA) : "f"(r.q * (e + s_lo)));
+                asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(icB) : "f"(r.q * (e + s_hi)));
+                e0 = make_float4(s_lo, s_hi, e, r.q);
+                e1 = make_float4(fmaxf(icA, icB), fminf(icA, icB), r.inv_dd, __int_as_float((a * P.nu + iu) * P.nv));
+            }
+            const unsigned hit = __ballot_sync(0xffffffffu, ok);
+            if (ok) {
+                int my_cnt = cnt[0];
+#pragma unroll
+                for (int q = 1; q < R; ++q) if (my_sg == q) my_cnt = cnt[q];
+                const int pos = my_sg * LCAP + my_cnt + __popc(hit & my_mask & lt_mask);
+                l0[pos] = e0; l1[pos] = e1;
+            }
+#pragma unroll
+            for (int q = 0; q < R; ++q) cnt[q] += __popc(hit & (all_sg << q));
+        }
+        __syncwarp();
+#pragma unroll
+        for (int sg = 0; sg < R; ++sg) {
+            for (int n = 0; n < cnt[sg]; ++n) {
+                const float4 e0 = l0[sg * LCAP + n], e1 = l1[sg * LCAP + n];
+                const int oA = __float_as_int(e1.w);
+                if (sg == 0) gather_column<R, M, KT, 0>(acc, zl, P, TL, c0v, e0.x, e0.y, e0.z, e0.w, e1.z, e1.x, e1.y, oA);
+                else if (sg == 1) gather_column<R, M, KT, 1 % R>(acc, zl, P, TL, c0v, e0.x, e0.y, e0.z, e0.w, e1.z, e1.x, e1.y, oA);
+                else if (sg == 2) gather_column<R, M, KT, 2 % R>(acc, zl, P, TL, c0v, e0.x, e0.y, e0.z, e0.w, e1.z, e1.x, e1.y, oA);
+                else gather_column<R, M, KT, 3 % R>(acc, zl, P, TL, c0v, e0.x, e0.y, e0.z, e0.w, e1.z, e1.x, e1.y, oA);
+            }
+        }
+        __syncwarp();
     }
 #pragma unroll
     for (int t = 0; t < KT; ++t)
@@ -212,13 +357,17 @@ static void launch_back_kernel(const LevelParams &P, const Level &L, const float
     const int nzh = P.nz / M, ni = R == 4 ? P.nx / 2 : P.nx, nj = R == 4 ? P.ny / 2 : P.ny;
     const int kchunk = 32 * KT;
     dim3 b(32, BK_BX), gr((ni + BK_BX - 1) / BK_BX, nj, (nzh + kchunk - 1) / kchunk);
-    back_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    if (L.back_maxc <= BK_MAXC) back_list_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    else back_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
 }
 
 template <int R, int M>
 static void launch_back_rm(const LevelParams &P, const Level &L, const float *src, const float *d_f, float coef,
                            float *d_out, cudaStream_t st)
 {
+#ifdef BACK_KT
+    launch_back_kernel<R, M, BACK_KT>(P, L, src, d_f, coef, d_out, st); return;
+#endif
     if (P.nz / M >= 64) launch_back_kernel<R, M, 2>(P, L, src, d_f, coef, d_out, st);
     else launch_back_kernel<R, M, 1>(P, L, src, d_f, coef, d_out, st);
 }

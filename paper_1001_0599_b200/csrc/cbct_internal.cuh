@@ -73,6 +73,7 @@ struct Level {
     float *d_f = nullptr;       // level volume for levels > 0 and for the host entry point
     float *d_prev = nullptr;    // the volume that entered the current iteration (convergence test, NEXT-2)
     float *d_y = nullptr;       // binned data for levels > 0; staging for level 0 host entry
+    int back_maxc = 1 << 30;    // upper bound of the detector columns in the shadow of one voxel's (i,j) square (back.cu)
     mutable double lhat = -1.0; // A5 step bound: a property of the geometry alone, computed on first use
 };
 

@@ -203,6 +203,16 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         st = build_tables(g, L, rays, views);
         if (st != CBCT_OK) { free_all(g); return st; }
 #define TRY(x) do { st = (x); if (st != CBCT_OK) { free_all(g); return st; } } while (0)
+        {   // widest shadow of a voxel square on the detector's u axis, in columns: back.cu's W at the largest
+            // magnification (volume corner nearest to the source) and fan angle, as that kernel inflates it
+            double rx = 0.5 * p.nx * L.hx + fabs(desc->vol_off[0]), ry = 0.5 * p.ny * L.hy + fabs(desc->vol_off[1]);
+            double rmax = sqrt(rx * rx + ry * ry), mag = desc->sdd / (desc->sad - rmax);
+            double umax = 0.5 * p.nu * L.du + fabs(desc->det_off_u), tn = fmax(umax / desc->sdd, rmax / (desc->sad - rmax));
+            double dn = 0, du = 0;
+            for (const ViewC &v : views) { dn = fmax(dn, v.dn); du = fmax(du, v.du); }
+            double W = mag * (tn * dn + du);
+            L.back_maxc = (int)floor(2.0 * W / L.du + 0.04) + 1;       // integers in an interval of that length
+        }
         TRY(dev_alloc(g, &L.d_rayu, rays.size()));
         TRY(dev_alloc(g, &L.d_view, views.size()));
         TRY(dev_alloc(g, &L.d_cs, views.size()));
