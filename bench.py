@@ -38,8 +38,8 @@ METRIC = "fbs_iterations_per_second"
 UNIT = "iter/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
-# capture of this command (profiles/r01c_ncu_full_summary.txt); None = not captured for that kernel.
-NCU_DRAM_BYTES_PER_LAUNCH = {"back": 149.14e6, "forward": 120.92e6, "tv_grad": 98.34e6, "tv_trial": 138.37e6,
+# capture of this command (profiles/r01d_ncu_full_summary.txt); None = not captured for that kernel.
+NCU_DRAM_BYTES_PER_LAUNCH = {"back": 150.62e6, "forward": 120.92e6, "tv_grad": 98.34e6, "tv_trial": 138.37e6,
                              "tv_update": 166.68e6}
 
 
