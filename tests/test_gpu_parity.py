@@ -63,12 +63,19 @@ def geoms():
                               sad=600.0, sdd=900.0, n_proj=16, vol_off=(0.0, 0.0, 1.3), det_off_u=0.9,
                               det_off_v=-2.1,
                               angles=np.deg2rad(11.0) + 2 * np.pi * np.arange(16) / 16)
+    # coarse voxels on a fine detector: a voxel's shadow is ~9 columns wide, which takes the back-projector's
+    # general kernel (back_kernel) instead of the shared-memory list kernel (at most 5 columns per voxel and view)
+    out["wide"] = I.Geometry(nx=24, ny=20, nz=12, hx=4.0, hy=4.0, hz=4.0, nu=160, nv=96, du=1.0, dv=1.0,
+                             sad=500.0, sdd=800.0, n_proj=5, angles=np.deg2rad([3.0, 80.0, 155.0, 222.0, 301.0]))
+    # the same regime with every symmetry on (square centred grid, 8 equally spaced views)
+    out["wide8"] = I.Geometry(nx=24, ny=24, nz=12, hx=4.0, hy=4.0, hz=4.0, nu=160, nv=96, du=1.0, dv=1.0,
+                              sad=500.0, sdd=800.0, n_proj=8)
     return out
 
 
 GEOMS = geoms()
 # every geometry through the generic kernels; the symmetric ones also through the quarter-turn kernels
-CASES = [(n, True) for n in GEOMS] + [(n, False) for n in ("config1", "aniso", "sym48")]
+CASES = [(n, True) for n in GEOMS] + [(n, False) for n in ("config1", "aniso", "sym48", "wide8")]
 
 
 @pytest.mark.parametrize("name,generic", CASES)
@@ -77,7 +84,7 @@ def test_forward_projector_matches_oracle(torch, cbct, orc, name, generic):
     f = I.uniform_volume(g, 11)
     want = orc.forward(g, f)
     with cbct.geometry_create(g, no_symmetry=generic) as h:
-        assert h.symmetry == (1 if generic else {"config1": 8, "aniso": 8, "sym48": 4, "cube64": 2}.get(name, 1))
+        assert h.symmetry == (1 if generic else {"config1": 8, "aniso": 8, "sym48": 4, "cube64": 2, "wide8": 8}.get(name, 1))
         p = torch.empty(g.proj_shape, device="cuda", dtype=torch.float32)
         h.forward_project(dev(torch, f), p)
         got = p.cpu().numpy()
