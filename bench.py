@@ -464,6 +464,45 @@ def run_sweep(args):
                       "sweep": out}))
 
 
+# ---------------------------------------------------------------------------------------------
+# Table-1-style sweep: quality metrics and time against the number of views
+# ---------------------------------------------------------------------------------------------
+
+def run_table1(args):
+    """The shape of the paper's Table 1 on the synthetic torso phantom of config 3: for N_theta in --table1-views, the
+    full multi-grid reconstruction (config 3's levels and iteration counts) from N_theta equally spaced noisy views,
+    the relative error e and the correlation coefficient c against the voxelised phantom (cbct_quality_metrics) and
+    the device time.  Prints ONE JSON line."""
+    import torch
+    from paper_1001_0599_b200 import cbct
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    k, cfg = workload(args.workload)
+    rows = []
+    for n_theta in [int(x) for x in args.table1_views.split(",")]:
+        c = I.Config(cfg.name, cfg.geom.replace(n_proj=n_theta, angles=None), cfg.fbs, cfg.ellipsoids, cfg.photons, cfg.seed)
+        g = c.geom
+        y = torch.from_numpy(I.make_projections(c)).cuda()
+        truth = torch.from_numpy(I.paint(c.ellipsoids, g)).cuda()
+        with cbct.geometry_create(g, max_levels=len(c.fbs.iters_per_level)) as h:
+            f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+            h.fbs_reconstruct(y, f, c.fbs, objective=False)          # warm-up (step bounds are cached in the handle)
+            f.zero_()
+            rep = h.fbs_reconstruct(y, f, c.fbs, objective=False)
+            e, cc = h.quality_metrics(f, truth)
+            rows.append({"n_theta": n_theta, "symmetry": h.symmetry, "rel_error_e": e, "correlation_c": cc,
+                         "recon_seconds": rep.ms_total / 1e3, "iterations": rep.n_iters_total})
+    print(json.dumps({"metric": "table1_quality_vs_views", "n_gpus": 1, "data": "synthetic", "dtype": "f32",
+                      "config": {"workload": f"config{k} geometry and phantom, N_theta equally spaced views, "
+                                             f"{len(cfg.fbs.iters_per_level)} levels x {list(cfg.fbs.iters_per_level)} iterations",
+                                 "tv_weight": cfg.fbs.tv_weight, "step": cfg.fbs.step},
+                      "paper_table1": "e = 28.63 / 15.96 / 11.38 / 7.10 %, c = 0.9386 / 0.9813 / 0.9906 / 0.9963, "
+                                      "t = 38.7 / 51.2 / 77.8 / 130.3 s for N_theta = 5 / 10 / 20 / 40 on the NCAT phantom, "
+                                      "Tesla C1060 (PAPER.md:L255): context, other phantom and hardware",
+                      "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -475,9 +514,13 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="config 5: operator microbenchmarks instead of the FBS step")
     ap.add_argument("--sweep-sizes", default="64,128,256,512")
     ap.add_argument("--sweep-views", default="1,40,360")
+    ap.add_argument("--table1", action="store_true", help="quality metrics and time against the number of views")
+    ap.add_argument("--table1-views", default="5,10,20,40")
     args = ap.parse_args()
     if args.sweep:
         return run_sweep(args)
+    if args.table1:
+        return run_table1(args)
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: fewer than 3 warm-up steps", file=sys.stderr)
     if args.impl == "reference":
