@@ -350,6 +350,12 @@ def run_ours(args):
                           "frac": bpv * nvox / t / 1e9 / hbm_peak, "bytes_per_voxel": bpv, "peak_source": peak_src}
     dominant = max((n for n in kern), key=lambda n: per[n]["ms_per_step"])
     roof = dict(kern[dominant])
+    # the same kernel against the HBM roofline, for reference: algorithmic HBM bytes per launch
+    alg_hbm = {"back": 4.0 * nray + 8.0 * nvox, "forward": 4.0 * nvox * 1.1 + 8.0 * nray}.get(dominant)
+    if alg_hbm is not None:
+        t = per[dominant]["ms_per_launch"] / 1e3
+        roof["hbm"] = {"algorithmic_bytes": alg_hbm, "achieved": alg_hbm / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                       "frac": alg_hbm / t / 1e9 / hbm_peak, "peak_source": peak_src}
     roof.update({"kernel": dominant, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dominant),
                  "share_of_step": per[dominant]["ms_per_step"] / sum(v["ms_per_step"] for v in per.values())})
 
