@@ -109,6 +109,7 @@ __device__ __forceinline__ void gather_column(float (&acc)[KT][R * M], const flo
             }
         };
         auto fetch = [&](int o) {
+            CBCT_DEV_ASSERT(o >= 0 && o < P.t_entries);
             if (R == 4) return __ldg(reinterpret_cast<const float4 *>(T) + o);
             return make_float4(__ldg(T + o), 0.0f, 0.0f, 0.0f);
         };
@@ -288,6 +289,7 @@ back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC
             const float uc = mag * ru, W = mag * fmaf(fabsf(tn), vw.z, vw.w);
             iu_lo = max(0, __float2int_ru((uc - W - P.u0) * P.inv_du - 0.02f));
             const int iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
+            CBCT_DEV_ASSERT(iu_hi - iu_lo + 1 <= BK_MAXC);       // the bound checked at create (Level::back_maxc)
             ncand = min(iu_hi - iu_lo + 1, BK_MAXC);
         }
         for (int c = 0; __any_sync(0xffffffffu, c < ncand); ++c) {
@@ -314,6 +316,7 @@ back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC
 #pragma unroll
                 for (int q = 1; q < R; ++q) if (my_sg == q) my_cnt = cnt[q];
                 const int pos = my_sg * LCAP + my_cnt + __popc(hit & my_mask & lt_mask);
+                CBCT_DEV_ASSERT(pos >= my_sg * LCAP && pos < (my_sg + 1) * LCAP);
                 l0[pos] = e0; l1[pos] = e1;
             }
 #pragma unroll

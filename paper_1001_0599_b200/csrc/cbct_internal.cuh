@@ -42,6 +42,7 @@ struct LevelParams {
     int nx, ny, nz, nu, nv, np;
     int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
     int nmir;                  // 2 when the z-mirror image of every ray / voxel shares its weights, else 1
+    int stage_cells, t_entries; // cells of the staged copy / entries (R floats) of the residual stack: bounds of the gathers
     int nyP, nzP;              // padded extents of the staged volume [i + PM][j + PM][k + PZ] (k fastest)
     int istride, jstride;      // its element strides along i and j (nyP * nzP, nzP)
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
@@ -97,6 +98,14 @@ struct cbct_geometry {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     int sm_count = 148;
 };
+
+// Debug builds (-DCBCT_ASSERT): device-side bounds checks of every gather index (compute-sanitizer stand-in).
+#ifdef CBCT_ASSERT
+#include <assert.h>
+#define CBCT_DEV_ASSERT(x) assert(x)
+#else
+#define CBCT_DEV_ASSERT(x) ((void)0)
+#endif
 
 constexpr int kScalars = 16;
 

@@ -172,7 +172,10 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
 #pragma unroll
                 for (int q = 0; q < R; ++q) offc[q] = off[q] + (cy ? dcol[q] : 0) + zc;
 #pragma unroll
-                for (int q = 0; q < R; ++q) { va[q] = __ldg(stage + off[q]); vc[q] = __ldg(stage + offc[q]); }
+                for (int q = 0; q < R; ++q) {
+                    CBCT_DEV_ASSERT(off[q] >= 0 && off[q] < P.stage_cells && offc[q] >= 0 && offc[q] < P.stage_cells);
+                    va[q] = __ldg(stage + off[q]); vc[q] = __ldg(stage + offc[q]);
+                }
 #pragma unroll
                 for (int q = 0; q < R; ++q) {
                     acc[q] = fmaf(wl, cell_lo(vc[q]), fmaf(lo, cell_lo(va[q]), acc[q]));
@@ -183,6 +186,7 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                     const bool yfirst = sy < sz;
 #pragma unroll
                     for (int q = 0; q < R; ++q) {
+                        CBCT_DEV_ASSERT(off[q] + (yfirst ? dcol[q] : dk) >= 0 && off[q] + (yfirst ? dcol[q] : dk) < P.stage_cells);
                         const cell vm = __ldg(stage + off[q] + (yfirst ? dcol[q] : dk));
                         acc[q] = fmaf(wm, cell_lo(vm), acc[q]);
                         if (M == 2) acc[R + q] = fmaf(wm, cell_hi(vm), acc[R + q]);

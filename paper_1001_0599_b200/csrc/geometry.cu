@@ -196,6 +196,8 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.nzP = (p.nmir == 2 ? p.nz / 2 : p.nz) + 2 * PAD_Z;
         p.jstride = p.nzP; p.istride = p.nyP * p.nzP;
         L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP * p.nmir;
+        p.stage_cells = (int)(L.stage_elems / p.nmir);
+        p.t_entries = (int)(L.nray / p.nsym);
         if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }
 
         std::vector<RayU> rays;
