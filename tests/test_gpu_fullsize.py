@@ -140,3 +140,24 @@ def test_config4_sampled_outputs(torch, cbct, orc):
         blk = got_b[k0:k0 + 16, j0:j0 + 16, i0:i0 + 16]
         assert rel_l2(blk, want) <= TOL_PROJ, ((i0, j0, k0), rel_l2(blk, want))
         assert np.abs(blk - want).max() <= 1e-4 * scale
+
+
+def test_config2_as_stated_full_iteration_counts(torch, cbct, orc):
+    """Config 2 of BASELINE.json exactly as stated: 128^3, 40 noisy views of 256x192, 50 FBS iterations on each of
+    2 multi-grid levels, against the whole oracle reconstruction (about a minute of host time)."""
+    cfg = I.config(2)
+    g = cfg.geom
+    y = I.make_projections(cfg)
+    want = orc.fbs(g, y, cfg.fbs)
+    with cbct.geometry_create(g, max_levels=2) as h:
+        f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+        rep = h.fbs_reconstruct(dev(torch, y), f, cfg.fbs)
+        got = f.cpu().numpy()
+    assert rep.n_iters_total == 100
+    assert rel_l2(got, want.f) <= TOL_VOL, rel_l2(got, want.f)
+    np.testing.assert_allclose(rep.objective, want.objective, rtol=1e-4)
+    assert np.all(rep.objective[1:50] <= rep.objective[:49] * (1 + 1e-6))      # monotone within a level
+    assert np.all(rep.objective[51:] <= rep.objective[50:-1] * (1 + 1e-6))
+    if (rep.inner_total, rep.trials_total) != (want.inner_total, want.trials_total):
+        print(f"note: inner/trials GPU {(rep.inner_total, rep.trials_total)} vs oracle "
+              f"{(want.inner_total, want.trials_total)}")
