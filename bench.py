@@ -182,12 +182,20 @@ def oracle_sample(cfg, y, views: int, z_div: int):
 
 
 def cpu_baseline(cfg, y, budget: str = "default"):
-    views, z_div = (2, 4) if budget == "default" else (1, 16)
+    # the sample is sized for ~10 s of oracle work on the GPU box's host (all 40 views of config 3); "small" (the per-step
+    # sample of the reference arm, repeated warmup + steps times) is 16 views and a sixteenth of the TV slab, ~4 s
+    g = cfg.geom
+    cost = float(g.nu) * g.nv * max(g.nx, g.ny)                     # per-view cost of P / P^T, relative
+    views = min(g.n_proj, max(1, int(round(40 * 5.0e7 / cost))))
+    z_div = 1 if g.nx * g.ny * g.nz <= 2.0e7 else 4
+    if budget != "default":
+        # the oracle's back-projector deals views to threads: fewer views than threads would idle cores
+        views, z_div = min(g.n_proj, max(1, int(round(16 * 5.0e7 / cost)))), 16
     r = oracle_sample(cfg, y, views, z_div)
     return {"value": 1.0 / r["seconds_full_iteration"], "unit": UNIT, "cores": r["threads"], "kind": "oracle",
             "sample": r["sample"], "sample_seconds": round(r["sample_seconds"], 3),
             "full_iteration_seconds_by_part": {k: round(v, 3) for k, v in r["parts_s"].items()},
-            "extrapolated": True}
+            "extrapolated": not (views == g.n_proj and z_div == 1)}
 
 
 def run_reference(args):
