@@ -352,7 +352,8 @@ def run_ours(args):
     # the volume arrays once: HBM roofline (measured copy bandwidth).
     l1_peak_gbs = 148 * 128 * sm_max_mhz * 1e6 / 1e9
     first = abs(inner / K - 1.0) < 1e-9          # one descent step per prox call: f is g itself in both passes
-    tv_bytes = {"tv_grad": 8.0 if first else 12.0, "tv_trial": 8.0 if first else 12.0, "tv_update": 12.0}
+    # the trial pass also writes its volume (the result, when the step is accepted and last): + 4 bytes per voxel
+    tv_bytes = {"tv_grad": 8.0 if first else 12.0, "tv_trial": 12.0 if first else 16.0, "tv_update": 12.0}
     kern = {}
     for name in ("forward", "back"):
         if per[name]["ms_per_launch"]:

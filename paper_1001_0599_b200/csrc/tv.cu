@@ -247,12 +247,13 @@ __global__ void __launch_bounds__(32 * TV_WPB)
 tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
                  const float *__restrict__ g, float lam, float delta2, int zc, int rows,
                  double *__restrict__ partials, int stride, unsigned int *__restrict__ counter,
-                 double *__restrict__ out)
+                 double *__restrict__ out, float *__restrict__ cand, int cand_clip)
 {
     __shared__ double slot[32];
     const TvTile T = tv_tile(D, zc);
     const bool hasg = g != nullptr;
     const size_t ok = T.k0 * T.plane;
+    size_t ocur = ok;                                             // slice k
     size_t o2 = min(T.k0 + 1, D.nz - 1) * T.plane;                // slice k+2 (after the first advance)
     float A[TV_R + 1], B[TV_R + 1], C[TV_R + 1], GA[TV_R], GB[TV_R], GC[TV_R];
     float rA, rB, rC = 0.0f;
@@ -292,9 +293,15 @@ tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__res
             float inv;
             const float nrm = grad_norm(gx, gy, gz, delta2, inv);
             const float res = c[r] - gc[r];
-            if (T.rv[r]) { s_tv += nrm; s_q = fmaf(res, res, s_q); }
+            if (T.rv[r]) {
+                s_tv += nrm; s_q = fmaf(res, res, s_q);
+                // the trial volume itself, truncated as the LAST update would: if the step is accepted and is the last
+                // one, this is the result and the update pass is skipped (same expression as tv_update_kernel)
+                if (TRIAL && cand) cand[ocur + T.ro[r]] = (cand_clip && c[r] < 0.0f) ? 0.0f : c[r];
+            }
         }
         e_tv += (double)s_tv; e_q += (double)s_q;
+        ocur += T.plane;
     };
 
     for (int k = T.k0; k < T.k1; k += 3) {
@@ -381,7 +388,7 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
         return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     StageTimer t(g, st, ST_REDUCE);
     tv_energy_kernel<false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, 0.0f, (float)(delta * delta), zc, 1,
-                                              g->d_partials, g->partials_stride, g->d_counter, d_out);
+                                              g->d_partials, g->partials_stride, g->d_counter, d_out, nullptr, 0);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
@@ -431,8 +438,9 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         for (int bt = 0; bt <= tp.max_backtracks; ++bt) {
             {
                 StageTimer t(g, st, ST_TV_TRIAL);
+                // the trial also leaves its (truncated) volume in d_f unless d_f is what it reads
                 tv_energy_kernel<true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, (float)lam, delta2, zc, 2, g->d_partials, S,
-                                                         g->d_counter, ds + 4);
+                                                         g->d_counter, ds + 4, cur != d_f ? d_f : nullptr, nonneg);
                 CBCT_LAUNCH_CHECK(g);
             }
             CBCT_CUDA(cudaMemcpyAsync(hs, ds, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -451,7 +459,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         const bool last = rel < tp.rel_tol || it + 1 == tp.max_inner;
         float *nxt = last ? d_f : bufs[which];      // d_f, d_f2, d_f, ...: never cur unless last (in place is fine)
         which ^= 1;
-        {
+        if (!(last && cur != d_f)) {                 // else the accepted trial already wrote max(f - lam d, 0) to d_f
             StageTimer t(g, st, ST_TV_UPDATE);
             if ((s = launch_update(g, n, cur, L.d_d, (float)lam, last ? nonneg : 0, nxt, st)) != CBCT_OK) return s;
         }
