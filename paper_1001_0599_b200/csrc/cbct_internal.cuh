@@ -95,7 +95,7 @@ struct cbct_geometry {
     int stage_timing = 0;
     mutable float stage_ms[CBCT_N_STAGES] = {0};
     mutable unsigned long long stage_calls[CBCT_N_STAGES] = {0};
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // 0,1 whole call; 2,3 stage timers; 4 first TV trial
     int sm_count = 148;
 };
 
@@ -176,9 +176,17 @@ cbct_status launch_back_eq6(const cbct_geometry *g, const Level &L, const float 
 cbct_status volume_change(const cbct_geometry *g, size_t n, const float *d_a, const float *d_b, double *sum_d2,
                           double *sum_b2, cudaStream_t st);
 // tv.cu
+// `ahead` (may be NULL): work the caller wants queued behind the first trial pass, which has left the candidate result in
+// d_f; it is called once, before the host waits for that trial's sums.  *ahead_valid tells whether d_f still held that
+// candidate when the call returned (the first step was accepted and was the last), i.e. whether the queued work is good.
+struct TvAhead {
+    cbct_status (*fn)(void *ctx);
+    void *ctx;
+    bool valid;
+};
 cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,
-                        cudaStream_t st);
+                        cudaStream_t st, TvAhead *ahead = nullptr);
 cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float *d_f, double delta,
                              double *d_out, cudaStream_t st);
 // transfer.cu

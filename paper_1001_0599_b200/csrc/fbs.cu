@@ -12,6 +12,23 @@
 
 namespace {
 
+// The forward projection of the NEXT iteration, queued behind the first TV trial pass of this one (run_tv_prox, TvAhead):
+// the trial leaves the candidate result in f, and in the usual case -- first step accepted and last -- that is the result,
+// so the device goes straight on while the host is still reading the trial's sums.  Otherwise the projection is redone.
+struct ForwardAhead {
+    const cbct_geometry *g;
+    const Level *L;
+    const float *f, *y;
+    int mode;
+    double *sum_slot;
+    cudaStream_t st;
+};
+cbct_status forward_ahead(void *ctx)
+{
+    const ForwardAhead *a = static_cast<const ForwardAhead *>(ctx);
+    return launch_forward(a->g, *a->L, a->f, a->y, a->L->d_T, a->mode, a->sum_slot, a->st);
+}
+
 // Lhat of one level (cached in the handle after the first evaluation: it depends on the geometry only).
 cbct_status step_bound_level(const cbct_geometry *g, const Level &L, double *lhat, cudaStream_t st)
 {
@@ -97,12 +114,14 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         const double tau = p->step / lhat, w = tau * p->tv_weight;
         if (rep && rep->step_abs) rep->step_abs[nl - 1 - l] = tau;
         int it_done = 0;
+        bool fwd_queued = false;        // this iteration's forward projection was queued by the previous one
         for (int it = 0; it < n_it; ++it, ++done) {
             if (p->conv_tol > 0.0)      // keep the volume that enters the iteration for the convergence test
                 CBCT_CUDA(cudaMemcpyAsync(L.d_prev, f, L.nvox * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            {
+            if (!fwd_queued) {
                 if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
             }
+            fwd_queued = false;
             if (want_obj) {
                 if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, g->d_objective + 2 * done, st)) != CBCT_OK) return s;
             }
@@ -113,7 +132,11 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
             }
             {
                 cbct_tv_report tr;
-                if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st)) != CBCT_OK) return s;
+                ForwardAhead fa = {g, &L, f, y, eq6 ? 4 : 1, g->d_objective + 2 * (done + 1) + 1, st};
+                TvAhead ah = {forward_ahead, &fa, false};
+                const bool look_ahead = !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
+                if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st, look_ahead ? &ah : nullptr)) != CBCT_OK) return s;
+                fwd_queued = look_ahead && ah.valid;
                 inner_total += tr.inner_iters;
                 trials_total += tr.trials;
             }

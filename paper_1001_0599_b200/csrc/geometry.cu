@@ -118,7 +118,7 @@ static void free_all(cbct_geometry *g)
     }
     cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter);
     if (g->h_scalars) cudaFreeHost(g->h_scalars);
-    for (int i = 0; i < 4; ++i) if (g->ev[i]) cudaEventDestroy(g->ev[i]);
+    for (int i = 0; i < 5; ++i) if (g->ev[i]) cudaEventDestroy(g->ev[i]);
     delete g;
 }
 
@@ -261,7 +261,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         free_all(g);
         return cbct_fail(CBCT_ERR_OOM, "pinned host allocation failed");
     }
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 5; ++i)
         if (cudaEventCreate(&g->ev[i]) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "event create failed"); }
     tls_error[0] = 0;
     *out = g;

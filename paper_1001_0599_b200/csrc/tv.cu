@@ -400,9 +400,10 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
 // d_scalars[4..5] trial sums.
 cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,
-                        cudaStream_t st)
+                        cudaStream_t st, TvAhead *ahead)
 {
     (void)sync_report;
+    if (ahead) ahead->valid = false;
     cbct_tv_report r = {0, 0, 0.0, 0.0};
     const size_t n = L.nvox;
     cbct_status s;
@@ -444,7 +445,15 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
                 CBCT_LAUNCH_CHECK(g);
             }
             CBCT_CUDA(cudaMemcpyAsync(hs, ds, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
-            CBCT_CUDA(cudaStreamSynchronize(st));
+            if (ahead && it == 0 && bt == 0) {
+                // the candidate result is in d_f: let the caller queue what follows a successful prox behind this trial,
+                // then wait for the trial's sums only -- the device keeps working while the host decides
+                CBCT_CUDA(cudaEventRecord(g->ev[4], st));
+                if ((s = ahead->fn(ahead->ctx)) != CBCT_OK) return s;
+                CBCT_CUDA(cudaEventSynchronize(g->ev[4]));
+            } else {
+                CBCT_CUDA(cudaStreamSynchronize(st));
+            }
             if (bt == 0) {
                 if (!have_E0) { E0 = hs[0] / N + 0.5 * beta * hs[1] / N; r.e_first = r.e_last = E0; have_E0 = true; }
                 Dm = hs[2] / N;
@@ -459,6 +468,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         const bool last = rel < tp.rel_tol || it + 1 == tp.max_inner;
         float *nxt = last ? d_f : bufs[which];      // d_f, d_f2, d_f, ...: never cur unless last (in place is fine)
         which ^= 1;
+        if (ahead && it == 0 && last) ahead->valid = true;      // d_f holds the candidate and stays as it is
         if (!(last && cur != d_f)) {                 // else the accepted trial already wrote max(f - lam d, 0) to d_f
             StageTimer t(g, st, ST_TV_UPDATE);
             if ((s = launch_update(g, n, cur, L.d_d, (float)lam, last ? nonneg : 0, nxt, st)) != CBCT_OK) return s;

@@ -393,3 +393,28 @@ def test_fbs_convergence_stopping_matches_oracle(torch, cbct, orc):
     assert rep.n_iters_total == sum(want.iters_done) and len(rep.objective) == len(want.objective)
     assert rel_l2(got, want.f) <= TOL_VOL
     np.testing.assert_allclose(rep.objective, want.objective, rtol=1e-4)
+
+
+@pytest.mark.parametrize("tv_weight", [0.01, 300.0])
+def test_fbs_look_ahead_projection_changes_nothing(torch, cbct, orc, tv_weight):
+    """Without the objective monitor the driver queues the next iteration's forward projection behind the first TV
+    trial pass (whose volume is the result when that step is accepted and last) and redoes it otherwise.  Both ways
+    must give bit for bit the volume of the plain sequence (objective monitor on: no look-ahead).  tv_weight 0.01:
+    every prox call ends after one step (look-ahead used); 300: several descent steps per call (look-ahead redone)."""
+    g = I.Geometry(nx=48, ny=48, nz=32, hx=2.0, hy=2.0, hz=2.5, nu=64, nv=48, du=2.4, dv=2.4, sad=1000.0,
+                   sdd=1500.0, n_proj=12)
+    ell = [I.Ellipsoid((0.0, 0.0, 0.0), (40.0, 34.0, 36.0), 0.0, 0.02)] + \
+        I.random_ellipsoids(np.random.default_rng(101), 6, (48.0, 48.0, 40.0), axes_range=(4.0, 14.0))
+    y = I.poisson_log(I.analytic_projections(ell, g), 1e5, 102).astype(np.float32)
+    setup = I.FbsSetup(iters_per_level=(4, 6), tv_weight=tv_weight)
+    outs, reps = [], []
+    with cbct.geometry_create(g, max_levels=2) as h:
+        for objective in (True, False, False):
+            f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+            reps.append(h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective))
+            outs.append(f.cpu().numpy())
+    assert outs[0].tobytes() == outs[1].tobytes() == outs[2].tobytes()
+    assert reps[0].inner_total == reps[1].inner_total and reps[0].trials_total == reps[1].trials_total
+    assert (reps[0].inner_total > 10) == (tv_weight > 1.0)           # the two regimes the test is about
+    want = orc.fbs(g, y, setup)
+    assert rel_l2(outs[1], want.f) <= TOL_VOL
