@@ -274,25 +274,32 @@ def run_ours(args):
 
         for _ in range(args.warmup):
             step_device()
-        # ---- timed region: K device-resident steps ------------------------------------------
+        # ---- K steps as K separate one-iteration calls: per-step statistics ----------------------
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+        barrier()
+        ev0.record(stream)
+        for i_step in range(args.steps):
+            step_device()
+            marks[i_step].record(stream)
+        barrier()
+        per_step = [a_.elapsed_time(b_) for a_, b_ in zip([ev0] + marks[:-1], marks)]
+        # ---- timed region: EXACTLY K steps = one cbct_fbs_reconstruct call of K finest-level iterations -----------
+        # (the library's own loop: inside one call the next iteration's forward projection is queued while the host
+        # reads the TV trial's sums, which K separate calls cannot do)
+        k_steps = I.FbsSetup(**{**fbs.__dict__, "iters_per_level": (args.steps,)})
+        f.copy_(f_start)
         l0 = h.launch_count
-        inner = trials = 0
         barrier()
         with ClockSampler(local) as clk:
             torch.cuda.profiler.start()        # cudaProfilerStart: `ncu --profile-from-start off` sees only the timed region
-            marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
             ev0.record(stream)
-            for i_step in range(args.steps):
-                r = step_device()
-                marks[i_step].record(stream)
-                inner += r.inner_total
-                trials += r.trials_total
+            r = h.fbs_reconstruct(y, f, k_steps, use_initial=True, objective=False, stream=stream)
             ev1.record(stream)
             barrier()
             torch.cuda.profiler.stop()
+        inner, trials = r.inner_total, r.trials_total
         ms_total = max_over_ranks(ev0.elapsed_time(ev1), world)
-        per_step = [a_.elapsed_time(b_) for a_, b_ in zip([ev0] + marks[:-1], marks)]
         launches = h.launch_count - l0
         clocks = clk.summary()
 
@@ -384,8 +391,10 @@ def run_ours(args):
     base = cpu_baseline(cfg, y_host)
     line = {
         "metric": METRIC, "value": aggregate_value(K, world, ms_total), "unit": UNIT, "n_gpus": world, "steps": K,
-        "warmup": args.warmup, "ms_per_step": ms_total / K, "ms_per_step_median": float(np.median(per_step)),
-        "ms_per_step_best": float(np.min(per_step)), "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_total / K,
+        "separate_calls_ms_per_step": {"mean": float(np.mean(per_step)), "median": float(np.median(per_step)),
+                                       "best": float(np.min(per_step))},
+        "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{k} ({cfg.name}): {g.nx}x{g.ny}x{g.nz} fp32 voxels at {g.hx} mm, {g.n_proj} views "
                                f"of {g.nu}x{g.nv} at {g.du} mm, one finest-level FBS iteration per step after "
