@@ -38,15 +38,15 @@ METRIC = "fbs_iterations_per_second"
 UNIT = "iter/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
-# capture of this command (profiles/r01d_ncu_full_summary.txt); None = not captured for that kernel.
+# capture of this command (profiles/r01e_ncu_full_summary.txt); None = not captured for that kernel.
 # L1 / L2 sector hit rates (%) and DRAM GB/s under ncu of the same capture (cold-cache, serialised launches): evidence for
 # the memory-path design of each kernel, not a timing
 NCU_COUNTERS = {"forward": {"l1_hit_pct": 68.1, "l2_hit_pct": 91.0, "l1tex_throughput_pct": 59.2},
                 "back": {"l1_hit_pct": 54.1, "l2_hit_pct": 95.1, "l1tex_throughput_pct": 83.4},
                 "tv_grad": {"l1_hit_pct": 18.4, "l2_hit_pct": 28.4}, "tv_trial": {"l1_hit_pct": 35.9, "l2_hit_pct": 27.4},
                 "tv_update": {"l1_hit_pct": 0.0, "l2_hit_pct": 0.0}}
-NCU_DRAM_BYTES_PER_LAUNCH = {"back": 150.62e6, "forward": 120.88e6, "tv_grad": 99.37e6, "tv_trial": 137.89e6,
-                             "tv_update": 165.84e6}
+NCU_DRAM_BYTES_PER_LAUNCH = {"back": 149.91e6, "forward": 120.75e6, "tv_grad": 98.30e6, "tv_trial": 178.88e6,
+                             "tv_update": None}
 
 
 def _peaks():
@@ -376,7 +376,7 @@ def run_ours(args):
     for name in kern:
         if args.workload == "config3":          # the committed capture is of this workload
             kern[name]["ncu"] = dict(NCU_COUNTERS.get(name, {}), dram_bytes_per_launch=NCU_DRAM_BYTES_PER_LAUNCH.get(name),
-                                     source="profiles/r01d_ncu_full_summary.txt")
+                                     source="profiles/r01e_ncu_full_summary.txt")
     dominant = max((n for n in kern), key=lambda n: per[n]["ms_per_step"])
     roof = dict(kern[dominant])
     # the same kernel against the HBM roofline, for reference: algorithmic HBM bytes per launch
