@@ -68,7 +68,11 @@ typedef struct {
                                  images of a ray; when the volume is centred in z and the detector in v
                                  (even nz, nv) also for the mirror image z -> -z.
                                  1: always use the generic one-ray-at-a-time kernels. */
+    int kernel_flags;         /* 0 (default): every level takes the fastest kernels its geometry allows.
+                                 CBCT_KERNEL_NO_TMA: never the TMA / shared-memory back-projector (cbct_geometry_back_path);
+                                 for A/B measurements and for keeping the other paths under test. */
 } cbct_geometry_desc;
+#define CBCT_KERNEL_NO_TMA 1
 
 /* Validates the description, uploads per-view tables and allocates all scratch for
  * `max_levels` levels.  *out is NULL on failure. */
@@ -78,6 +82,18 @@ void cbct_geometry_destroy(cbct_geometry *g);
 /* Rays (voxels) per thread the projectors of `level` handle with one weight computation: 4 by
  * quarter-turn symmetry, times 2 by the mirror symmetry z -> -z; 8, 4, 2 or 1 (0: bad level). */
 int cbct_geometry_symmetry(const cbct_geometry *g, int level);
+
+/* Which exact-transpose back-projector `level` runs: the TMA / shared-memory tile kernel (quarter-turn and mirror
+ * symmetric geometries whose voxel shadows are at most 8 detector columns and 4 rows wide), the per-warp list kernel
+ * (shadows of at most 5 columns), or the general gather kernel.  All three compute the same sums.  -1: bad level. */
+#define CBCT_BACK_PATH_GATHER 0
+#define CBCT_BACK_PATH_LIST 1
+#define CBCT_BACK_PATH_TMA 2
+int cbct_geometry_back_path(const cbct_geometry *g, int level);
+
+/* Number of times a kernel found a tile bound computed at create too small (it then stays inside its buffers and the
+ * result is wrong): 0 on every geometry the bounds were derived for; tests assert it.  Synchronises the stream. */
+cbct_status cbct_bound_violations(const cbct_geometry *g, unsigned int *count, void *cuda_stream);
 
 /* Device bytes the handle allocated (scratch + tables). */
 unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g);

@@ -28,6 +28,7 @@ STATUS_NAMES = {0: "CBCT_OK", 1: "CBCT_ERR_INVALID_ARG", 2: "CBCT_ERR_GEOMETRY",
 # every symbol include/cbct.h declares
 EXPORTS = [
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_symmetry", "cbct_geometry_device_bytes",
+    "cbct_geometry_back_path", "cbct_bound_violations",
     "cbct_forward_project", "cbct_back_project", "cbct_back_project_eq6", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
     "cbct_quality_metrics",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
@@ -50,7 +51,8 @@ class _Desc(C.Structure):
                 ("du", C.c_double), ("dv", C.c_double), ("det_off_u", C.c_double), ("det_off_v", C.c_double),
                 ("sad", C.c_double), ("sdd", C.c_double),
                 ("n_proj", C.c_int), ("angles_rad", C.POINTER(C.c_double)),
-                ("bc_xy", C.c_int), ("bc_z", C.c_int), ("max_levels", C.c_int), ("no_symmetry", C.c_int)]
+                ("bc_xy", C.c_int), ("bc_z", C.c_int), ("max_levels", C.c_int), ("no_symmetry", C.c_int),
+                ("kernel_flags", C.c_int)]
 
 
 class _TvParams(C.Structure):
@@ -113,6 +115,8 @@ def load_library():
     lib.cbct_geometry_destroy.argtypes = [vp]
     lib.cbct_geometry_destroy.restype = None
     lib.cbct_geometry_symmetry.argtypes = [vp, ip]
+    lib.cbct_geometry_back_path.argtypes = [vp, ip]
+    lib.cbct_bound_violations.argtypes = [vp, C.POINTER(C.c_uint), vp]
     lib.cbct_geometry_device_bytes.argtypes = [vp]
     lib.cbct_geometry_device_bytes.restype = C.c_ulonglong
     lib.cbct_forward_project.argtypes = [vp, ip, vp, vp, vp]
@@ -170,7 +174,7 @@ class Geometry:
     `desc` is any object with the attributes of `inputs.Geometry`.
     """
 
-    def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False):
+    def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False):
         lib = load_library()
         self._h = C.c_void_p()
         self.desc = desc
@@ -187,6 +191,7 @@ class Geometry:
         d.angles_rad = ang.ctypes.data_as(C.POINTER(C.c_double))
         d.bc_xy, d.bc_z, d.max_levels = desc.bc_xy, desc.bc_z, self.max_levels
         d.no_symmetry = int(bool(no_symmetry))
+        d.kernel_flags = 1 if no_tma else 0          # CBCT_KERNEL_NO_TMA
         _check(lib.cbct_geometry_create(C.byref(d), C.byref(self._h)))
 
     def close(self):
@@ -224,6 +229,15 @@ class Geometry:
     @property
     def symmetry(self) -> int:
         return int(load_library().cbct_geometry_symmetry(self._h, 0))
+
+    def back_path(self, level: int = 0) -> str:
+        """cbct_geometry_back_path: which exact-transpose back-projector the level runs."""
+        return {0: "gather", 1: "list", 2: "tma"}[int(load_library().cbct_geometry_back_path(self._h, level))]
+
+    def bound_violations(self, stream=None) -> int:
+        n = C.c_uint(0)
+        _check(load_library().cbct_bound_violations(self._h, C.byref(n), _stream_ptr(stream)))
+        return int(n.value)
 
     @property
     def device_bytes(self) -> int:
@@ -363,8 +377,8 @@ class Geometry:
         return {k: (float(m), int(c)) for k, m, c in zip(self.STAGES, ms, calls)}
 
 
-def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False) -> Geometry:
-    return Geometry(desc, max_levels, no_symmetry)
+def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False) -> Geometry:
+    return Geometry(desc, max_levels, no_symmetry, no_tma)
 
 
 def version() -> str:

@@ -11,8 +11,8 @@
 // fp32 crossing parameters, from the same table entries, as the forward projector's
 // (ray.cuh).  No atomics, fixed order (views ascending, columns, rows) => deterministic.
 //
-// Input is T scaled by L(u,v) (ray length source -> pixel), so the per-candidate weight is
-// overlap * inv_dd(view, iu).
+// Input is T scaled by L(u,v) inv_dd(view, iu) (the length of one unit slab of the ray), so the per-candidate weight
+// is the bare overlap.
 //
 // Rotation symmetry (R == 4, see forward.cu): a thread owns the four quarter-turn images
 // w_0..w_3 of a voxel of the first quadrant.  For a base view t and the image w_s, the
@@ -27,7 +27,7 @@
 #include "ray.cuh"
 #include "reduce.cuh"
 
-// d_out = d_in * L(u,v) in the d_T layout (plain for R == 1, quarter-turn interleaved for R == 4)
+// d_out = d_in * L(u,v) * inv_dd(view, iu) in the d_T layout (plain for R == 1, quarter-turn interleaved for R == 4)
 template <int R>
 __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ rayu,
                                   const float *__restrict__ in, float *__restrict__ out)
@@ -37,12 +37,12 @@ __global__ void scale_by_L_kernel(const LevelParams P, const RayU *__restrict__ 
     if (iu >= P.nu) return;
     const RayU r = load_rayu(rayu, a * P.nu + iu);
     const float v = fmaf((float)iv, P.dv, P.v0);
-    const float Lr = ray_len_L(r, v);
+    const float Lr = ray_len_L(r, v) * r.inv_dd;
     const size_t plane = (size_t)P.nv * P.nu, pix = (size_t)iv * P.nu + iu;
     float res[R];
 #pragma unroll
     for (int q = 0; q < R; ++q) res[q] = __ldg(in + (size_t)(a + q * P.nbase) * plane + pix) * Lr;
-    const size_t ot = ((size_t)a * P.nu + iu) * P.nv + iv;          // d_T layout: detector rows fastest
+    const size_t ot = ((size_t)a * P.nu + iu) * P.nv + t_row_slot(P, iv);   // d_T layout: detector rows fastest
     if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
     else out[ot] = res[0];
 }
@@ -90,7 +90,7 @@ __device__ __forceinline__ void gather_column(float (&acc)[KT][R * M], const flo
             asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(inv) : "f"(fmaf(v, q, tiny)));
             const float q1 = fmaf(zlo, inv, -e), q2 = fmaf(zhi, inv, -e);
             const float lo = fmaxf(fminf(q1, q2), s_lo), hi = fminf(fmaxf(q1, q2), s_hi);
-            return fmaxf(hi - lo, 0.0f) * inv_dd;
+            return fmaxf(hi - lo, 0.0f);          // the slab length per unit of L (inv_dd) is folded into T
         };
         auto gather = [&](float w, const float4 &tA, const float4 &tB) {
             acc[t][(SG + 0) % R] = fmaf(w, tA.x, acc[t][(SG + 0) % R]);
@@ -375,6 +375,8 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
 {
     const LevelParams &P = L.p;
     const float *src = d_in;
+    if (L.bt.ok && scaled && d_in != L.d_T)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_back: the TMA path reads the level's own residual stack");
     if (!scaled) {
         StageTimer t(g, st, ST_TRANSFER);
         dim3 b(128), gr((P.nu + 127) / 128, P.nv, P.nbase);
@@ -384,6 +386,7 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
         src = L.d_T;
     }
     StageTimer t(g, st, ST_BACK);
+    if (L.bt.ok) return launch_back_tma(g, L, d_f, coef, d_out, st);      // src is L.d_T on this path (below)
     if (P.nsym == 4 && P.nmir == 2) launch_back_rm<4, 2>(P, L, src, d_f, coef, d_out, st);
     else if (P.nsym == 4) launch_back_rm<4, 1>(P, L, src, d_f, coef, d_out, st);
     else if (P.nmir == 2) launch_back_rm<1, 2>(P, L, src, d_f, coef, d_out, st);

@@ -1,0 +1,540 @@
+// back_tma.cu -- A3/A4: the exact-transpose back-projector on TMA + shared memory (sm_100a).
+//
+// Same operator as back.cu -- (P^T T)[voxel] = sum_views sum_rays len(ray ∩ voxel) T[ray] with the coefficients of
+// forward.cu ("sum_theta P^T (P f - Y)"; the paper itself evaluates the continuum adjoint Eq. 6,
+// L195-L199, because a scatter collides on voxels, L187-L191) -- and the same arithmetic per (ray, voxel) pair (ray.cuh),
+// with the residual stack moved off the L1/LSU path:
+//
+//  * A block owns a BRICK of BI x BJ voxel columns of the first quadrant and 32 z-slices of the lower half of the
+//    volume, together with their quarter-turn and mirror images (8 voxels per weight, back.cu).  A warp owns CPW of the
+//    brick's columns; its lanes run along z.
+//  * The work is cut into STAGES (base view a, voxel image sg).  For one stage the brick casts a compact shadow on
+//    the detector of the base view: a few columns x the rows its 32 slices reach (exactly those rows again, mirrored,
+//    for the upper half of the volume).  A producer warp computes that rectangle and has the TMA unit copy it from the
+//    quarter-turn-interleaved residual stack (16-byte entries, detector rows fastest) into a ring of shared-memory tiles:
+//    one `cp.async.bulk.tensor` per power-of-two group of columns, completion counted on an mbarrier, rows outside the
+//    detector zero-filled by the copy unit -- so the gather loop holds no range clamp and no global load.
+//  * The consumer warps wait on the tile's "full" barrier, gather from shared memory and release the tile through its
+//    "empty" barrier; the producer runs one stage ahead, so the L2 round trips the L1-path kernel waited on (35 %
+//    occupancy, profiles/r01d) overlap the arithmetic of the previous stage.
+//  * About two detector rows cross a voxel, so consecutive lanes read 16-byte entries ~2 rows apart: in a plain layout
+//    that is a two-way bank conflict on every load.  The residual stack is therefore stored split by row parity
+//    (LevelParams::tP == 2: even rows, then odd rows of a column) and the odd plane of a tile is shifted by one entry,
+//    which puts rows r and r + 2 in adjacent 16-byte bank groups and rows r, r + 1 apart.
+//  * The in-plane part of every (column of voxels, base view, image, detector column) is worked out once per warp by
+//    lanes in parallel, as in back_list_kernel, into a per-warp list; the rows of a voxel start at an exact first row
+//    and take a fixed number NSLOT of slots (a bound from the geometry, checked at create): rows past the voxel get
+//    weight 0 from the same clipping that computes every weight, and the last slot's loads are predicated on it.
+//  * The 8 x 32 x BI x BJ results of a brick go through shared memory once more and leave in x-fastest order with
+//    16-byte stores (fused with g = f - coef * b, A4).
+//
+// Summation order per voxel: base view, image, detector column, row -- fixed, no atomics: bitwise reproducible.
+#include <cuda.h>
+#include <math.h>
+#include "cbct_internal.cuh"
+#include "ray.cuh"
+
+namespace {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        " .reg .pred p;\n"
+        "BT_WAIT:\n"
+        " mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra BT_DONE;\n"
+        " bra BT_WAIT;\n"
+        "BT_DONE:\n"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// one box of the 4-d view (row pair index within a plane, plane, detector column, base view) of the residual stack
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap *map, int c0, int c1, int c2, int c3, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// image sg of the first-quadrant voxel (i, j) under quarter turns: (i,j), (n1-j, i), (n1-i, n1-j), (j, n1-i)
+__device__ __forceinline__ void bt_image(int sg, int i, int j, int n1, int &mi, int &mj)
+{
+    mi = sg == 0 ? i : sg == 1 ? n1 - j : sg == 2 ? n1 - i : j;
+    mj = sg == 0 ? j : sg == 1 ? i : sg == 2 ? n1 - j : n1 - i;
+}
+
+// Shadow of the (mi, mj) voxel square on the u axis of base view `vw` (Eq. A6, to first order in the inflated
+// half extents; the expressions of back.cu): detector columns [iu_lo, iu_hi], and the voxel centre's depth rn along e_n.
+__device__ __forceinline__ void bt_shadow(const LevelParams &P, const float4 vw, int mi, int mj, int &iu_lo, int &iu_hi, float &rn)
+{
+    const float xc = fmaf((float)mi, P.hx, P.x0), yc = fmaf((float)mj, P.hy, P.y0);
+    rn = fmaf(xc, vw.x, fmaf(yc, vw.y, P.sad));
+    const float ru = fmaf(xc, vw.y, -yc * vw.x);
+    const float rinv = rcp_approx(rn);
+    const float mag = P.sdd * rinv, tn = ru * rinv;
+    const float uc = mag * ru, W = mag * fmaf(fabsf(tn), vw.z, vw.w);
+    iu_lo = max(0, __float2int_ru((uc - W - P.u0) * P.inv_du - 0.02f));
+    iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
+}
+
+// One detector column's contribution to a voxel and its 7 images.  e0 = (s_lo, s_hi, e, q) as in back.cu; icn = 1/c at
+// the strip end nearer to the source, in detector rows per z-index; colA = the column's first entry in the stage's A
+// tile.  The voxel lies below the source plane (zlo + 1 <= 0): its rows have v < 0, so the two z-plane crossings come in
+// a known order -- plane zlo + 1 first when q > 0 -- and rows with v > 0 clip to weight 0 by the same expressions.
+template <int SG, int NSLOT, int TP>
+__device__ __forceinline__ void bt_visit(float (&acc)[8], const char *__restrict__ colA, int KB, int plane_bytes,
+                                         float zlo, const float4 e0, float icn, int r0A, const BtConsts C)
+{
+    const int r = __float2int_ru(fmaf(zlo, icn, C.c0v_m));
+    const int rr = r - r0A;
+    CBCT_DEV_ASSERT(rr >= 0 && rr + NSLOT - 1 <= C.rr_max);
+    const float q = e0.w, e = e0.z;
+    const bool qpos = q > 0.0f;
+    const float zA = qpos ? zlo + 1.0f : zlo, zB = qpos ? zlo : zlo + 1.0f;
+    const float tiny = copysignf(1.0e-37f, q);
+    int o0, d1;
+    if (TP == 2) {
+        const int p = rr & 1;
+        o0 = p * (plane_bytes + 16) + ((rr >> 1) << 4);
+        d1 = p ? -plane_bytes : plane_bytes + 16;
+    } else {
+        o0 = rr << 4;
+        d1 = 16;
+    }
+    const float rf = (float)r;
+#pragma unroll
+    for (int s = 0; s < NSLOT; ++s) {
+        const float v = fmaf(rf + (float)s, C.dv, C.v0);
+        const float inv = rcp_approx(fmaf(v, q, tiny));
+        const float qa = fmaf(zA, inv, -e), qb = fmaf(zB, inv, -e);
+        const float w = fmaxf(fminf(qb, e0.y) - fmaxf(qa, e0.x), 0.0f);
+        const int os = TP == 2 ? o0 + (s & 1) * d1 + (s >> 1) * 16 : o0 + 16 * s;
+        if (s < NSLOT - 1 || w > 0.0f) {
+            const float4 tA = *reinterpret_cast<const float4 *>(colA + os);
+            const float4 tB = *reinterpret_cast<const float4 *>(colA + KB - os);
+            acc[(SG + 0) % 4] = fmaf(w, tA.x, acc[(SG + 0) % 4]);
+            acc[(SG + 1) % 4] = fmaf(w, tA.y, acc[(SG + 1) % 4]);
+            acc[(SG + 2) % 4] = fmaf(w, tA.z, acc[(SG + 2) % 4]);
+            acc[(SG + 3) % 4] = fmaf(w, tA.w, acc[(SG + 3) % 4]);
+            acc[4 + (SG + 0) % 4] = fmaf(w, tB.x, acc[4 + (SG + 0) % 4]);
+            acc[4 + (SG + 1) % 4] = fmaf(w, tB.y, acc[4 + (SG + 1) % 4]);
+            acc[4 + (SG + 2) % 4] = fmaf(w, tB.z, acc[4 + (SG + 2) % 4]);
+            acc[4 + (SG + 3) % 4] = fmaf(w, tB.w, acc[4 + (SG + 3) % 4]);
+        }
+    }
+}
+
+// R == 4, M == 2 only (square centred in-plane grid with quarter-turn views, volume and detector centred in z / v).
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
+__global__ void __launch_bounds__((BI * BJ / CPW + 1) * 32, MINB)
+back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const BtParams Q,
+                const RayU *__restrict__ rayu, const ViewC *__restrict__ views, const float *__restrict__ f, float coef,
+                float *__restrict__ out, unsigned int *__restrict__ errflag)
+{
+    constexpr int NIJ = BI * BJ, NW = NIJ / CPW;      // voxel columns of the brick, consumer warps
+    constexpr int SPR = 4 / CPW;                      // stages per list round: 32 lanes = SPR stages x CPW columns x 8 candidates
+    static_assert(CPW == 1 || CPW == 2 || CPW == 4, "a list round is 32 lanes");
+    extern __shared__ __align__(1024) char smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int i0 = blockIdx.x * BI, j0 = blockIdx.y * BJ, k0 = blockIdx.z * 32;
+    const int ni = P.nx / 2, nj = P.ny / 2, n1 = P.nx - 1;
+    const int n_stages = 4 * P.nbase;
+
+    float4 *s_view = reinterpret_cast<float4 *>(smem + Q.view_off);
+    int4 *s_hdr = reinterpret_cast<int4 *>(smem + Q.hdr_off);
+    const uint32_t bar0 = smem_u32(smem + Q.bar_off);             // full[0], full[1], empty[0], empty[1]
+    for (int a = threadIdx.x; a < P.nbase; a += blockDim.x) s_view[a] = __ldg(reinterpret_cast<const float4 *>(views) + a);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < BT_NST; ++s) { mbar_init(bar0 + 8 * s, 1); mbar_init(bar0 + 8 * (BT_NST + s), NW); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    BtConsts C;
+    C.c0v_m = Q.c0v_m; C.dv = P.dv; C.v0 = P.v0; C.rr_max = TP * Q.XB - (TP == 2 ? 3 : 1);
+
+    float acc[CPW][8];
+#pragma unroll
+    for (int cp = 0; cp < CPW; ++cp)
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[cp][q] = 0.0f;
+
+    if (warp == NW) {
+        // ---------------- producer: the stage's detector rectangle, then the tile copies ----------------
+        for (int s = 0; s < n_stages; ++s) {
+            const int a = s >> 2, sg = s & 3, slot = s % BT_NST, use = s / BT_NST;
+            if (use > 0) mbar_wait(bar0 + 8 * (BT_NST + slot), (use - 1) & 1);
+            const float4 vw = s_view[a];
+            int cmin = 1 << 30, cmax = -1;
+            float rn_lo = 3.0e38f, rn_hi = -3.0e38f;
+            for (int v = lane; v < NIJ; v += 32) {
+                const int i = i0 + v % BI, j = j0 + v / BI;
+                if (i < ni && j < nj) {
+                    int mi, mj, lo, hi;
+                    float rn;
+                    bt_image(sg, i, j, n1, mi, mj);
+                    bt_shadow(P, vw, mi, mj, lo, hi, rn);
+                    if (lo <= hi) { cmin = min(cmin, lo); cmax = max(cmax, min(hi, lo + BT_MAXC - 1)); }
+                    rn_lo = fminf(rn_lo, rn); rn_hi = fmaxf(rn_hi, rn);
+                }
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                cmin = min(cmin, __shfl_xor_sync(0xffffffffu, cmin, o));
+                cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
+                rn_lo = fminf(rn_lo, __shfl_xor_sync(0xffffffffu, rn_lo, o));
+                rn_hi = fmaxf(rn_hi, __shfl_xor_sync(0xffffffffu, rn_hi, o));
+            }
+            // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
+            // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
+            const int klast = min(k0 + 31, Q.nzh - 1);
+            const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
+            const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
+            const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
+            const int rlast = __float2int_ru(fmaf(zl, ic_min, Q.c0v_m)) + NSLOT;
+            int ncols = cmax - cmin + 1;
+            const bool skip = ncols <= 0 || rlast < 0 || rmin > P.nv - 1;
+            const int x0 = TP == 2 ? (rmin >> 1) : rmin, r0A = TP * x0;
+            if (!skip && (ncols > Q.ncols || rlast - r0A > C.rr_max)) {   // the bounds of create do not hold: flag, stay in bounds
+                if (lane == 0) atomicAdd(errflag, 1u);
+                ncols = min(ncols, Q.ncols);
+            }
+            if (lane == 0) {
+                s_hdr[slot] = make_int4(skip ? 1 : 0, cmin, r0A, ncols);
+                const uint32_t full = bar0 + 8 * slot;
+                if (skip) {
+                    mbar_arrive(full);
+                } else {
+                    const uint32_t tile = smem_u32(smem + slot * Q.stage_bytes);
+                    const uint32_t col_bytes = Q.XB * 16;
+                    mbar_arrive_expect_tx(full, (uint32_t)(2 * TP * ncols) * col_bytes);
+                    int c = 0;
+#pragma unroll
+                    for (int b = BT_NMAPS - 1; b >= 0; --b) {
+                        if (ncols & (1 << b)) {
+                            const uint32_t dst = tile + c * col_bytes;
+                            if (TP == 2) {
+                                const int xb1 = P.nv / 2 - x0 - Q.XB;      // origin of the mirror rows' odd plane
+                                tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
+                                tma_load_4d(dst + Q.plane_bytes, &maps.m[b], 2 * (x0 - 1), 1, cmin + c, a, full);
+                                tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (xb1 + 1), 0, cmin + c, a, full);
+                                tma_load_4d(dst + Q.half_bytes + Q.plane_bytes, &maps.m[b], 2 * xb1, 1, cmin + c, a, full);
+                            } else {
+                                tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
+                                tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (P.nv - x0 - Q.XB), 0, cmin + c, a, full);
+                            }
+                            c += 1 << b;
+                        }
+                    }
+                }
+            }
+            __syncwarp();
+        }
+    } else {
+        // ---------------- consumers ----------------
+        float4 *__restrict__ l0 = reinterpret_cast<float4 *>(smem + Q.list_off) + warp * 64, *__restrict__ l1 = l0 + 32;
+        const int kv = k0 + lane;
+        const float zlo = (float)(min(kv, Q.nzh - 1) - P.cz) - P.sz;
+        const int KB = Q.half_bytes + (TP == 2 ? Q.plane_bytes : 0) + (Q.XB - 1) * 16;
+        // this lane's candidate in a list round: unit u = lane / 8 -> (stage of the round, column of the warp), candidate lane % 8
+        const int u = lane >> 3, cnd = lane & 7;
+        const int my_cp = u % CPW, my_t = u / CPW;
+        const int col = warp * CPW + my_cp;
+        const int vi0 = i0 + col % BI, vj0 = j0 + col / BI;
+        const bool col_ok = vi0 < ni && vj0 < nj;
+        const unsigned lt_mask = (1u << lane) - 1u;
+        for (int a = 0; a < P.nbase; ++a) {
+            const float4 vw = s_view[a];
+#pragma unroll
+            for (int rd = 0; rd < CPW; ++rd) {
+                // ---- list round: every lane takes one (stage, column, candidate detector column) ----
+                bool ok = false;
+                float4 e0 = make_float4(0.f, 0.f, 0.f, 0.f), e1 = e0;
+                {
+                    const int sg = rd * SPR + my_t;
+                    int mi, mj, iu_lo, iu_hi;
+                    float rn;
+                    bt_image(sg, vi0, vj0, n1, mi, mj);
+                    bt_shadow(P, vw, mi, mj, iu_lo, iu_hi, rn);
+                    CBCT_DEV_ASSERT(!col_ok || iu_hi - iu_lo + 1 <= BT_MAXC);
+                    if (col_ok && cnd <= iu_hi - iu_lo) {
+                        const int iu = iu_lo + cnd;
+                        const RayU r = load_rayu(rayu, a * P.nu + iu);
+                        const float bx = (float)(mi - P.cx), by = (float)(mj - P.cy);
+                        const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;
+                        const float y0 = fmaf(d0, r.m, r.a0);
+                        const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
+                        const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
+                        ok = s_hi > s_lo;
+                        const float e = d0 - r.sd;
+                        const float icA = rcp_approx(r.q * (e + s_lo)), icB = rcp_approx(r.q * (e + s_hi));
+                        e0 = make_float4(s_lo, s_hi, e, r.q);
+                        e1 = make_float4(fmaxf(icA, icB) * P.inv_dv, __int_as_float(iu), 0.f, 0.f);
+                    }
+                }
+                const unsigned hit = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    const int pos = u * 8 + __popc(hit & (0xffu << (8 * u)) & lt_mask);
+                    l0[pos] = e0; l1[pos] = e1;
+                }
+                __syncwarp();
+                // ---- the round's stages ----
+#pragma unroll
+                for (int t = 0; t < SPR; ++t) {
+                    const int sg = rd * SPR + t;
+                    const int s = 4 * a + sg, slot = s % BT_NST, use = s / BT_NST;
+                    mbar_wait(bar0 + 8 * slot, use & 1);
+                    const int4 hdr = s_hdr[slot];
+                    if (!hdr.x) {
+                        const char *tile = smem + slot * Q.stage_bytes;
+#pragma unroll
+                        for (int cp = 0; cp < CPW; ++cp) {
+                            const int uu = t * CPW + cp;
+                            const int n_u = __popc(hit & (0xffu << (8 * uu)));
+                            for (int n = 0; n < n_u; ++n) {
+                                const float4 E0 = l0[uu * 8 + n], E1 = l1[uu * 8 + n];
+                                const int cidx = __float_as_int(E1.y) - hdr.y;
+                                CBCT_DEV_ASSERT(cidx >= 0 && cidx < hdr.w);
+                                const char *colA = tile + cidx * (Q.XB * 16);
+                                if (sg == 0) bt_visit<0, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
+                                else if (sg == 1) bt_visit<1, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
+                                else if (sg == 2) bt_visit<2, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
+                                else bt_visit<3, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
+                            }
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar0 + 8 * (BT_NST + slot));
+                }
+            }
+        }
+    }
+
+    // ---------------- results: through shared memory into x-fastest order, then g = f - coef b (A4) ----------------
+    __syncthreads();        // every tile has been consumed; the ring is free
+    float *s_out = reinterpret_cast<float *>(smem);      // [image 8][k 32][rows of the image's footprint][its columns]
+    if (warp < NW) {
+#pragma unroll
+        for (int cp = 0; cp < CPW; ++cp) {
+            const int col = warp * CPW + cp, ii = col % BI, jj = col / BI;
+#pragma unroll
+            for (int img = 0; img < 8; ++img) {
+                const int r = img & 3;
+                const int wr = (r & 1) ? BJ : BI;                                  // footprint width of image r
+                const int xl = r == 0 ? ii : r == 1 ? BJ - 1 - jj : r == 2 ? BI - 1 - ii : jj;
+                const int yl = r == 0 ? jj : r == 1 ? ii : r == 2 ? BJ - 1 - jj : BI - 1 - ii;
+                s_out[(img * 32 + lane) * NIJ + yl * wr + xl] = acc[cp][img];
+            }
+        }
+    }
+    __syncthreads();
+    const bool full_brick = i0 + BI <= ni && j0 + BJ <= nj;
+    if (Q.vec4 && full_brick) {
+        constexpr int NV4 = 8 * 32 * NIJ / 4;
+        for (int e4 = threadIdx.x; e4 < NV4; e4 += blockDim.x) {
+            const int e = e4 * 4, img = e / (32 * NIJ), k = (e / NIJ) % 32, w = e % NIJ;
+            const int r = img & 3, wr = (r & 1) ? BJ : BI, yl = w / wr, xl = w % wr;
+            const int kk = k0 + k;
+            if (kk >= Q.nzh) continue;
+            const int xg = (r == 0 ? i0 : r == 1 ? P.nx - BJ - j0 : r == 2 ? P.nx - BI - i0 : j0) + xl;
+            const int yg = (r == 0 ? j0 : r == 1 ? i0 : r == 2 ? P.ny - BJ - j0 : P.ny - BI - i0) + yl;
+            const int zg = img >= 4 ? P.nz - 1 - kk : kk;
+            const size_t o = ((size_t)zg * P.ny + yg) * P.nx + xg;
+            float4 v = *reinterpret_cast<const float4 *>(s_out + e);
+            if (f) {
+                const float4 fv = __ldg(reinterpret_cast<const float4 *>(f + o));
+                v.x = fmaf(-coef, v.x, fv.x); v.y = fmaf(-coef, v.y, fv.y); v.z = fmaf(-coef, v.z, fv.z); v.w = fmaf(-coef, v.w, fv.w);
+            }
+            *reinterpret_cast<float4 *>(out + o) = v;
+        }
+    } else {
+        constexpr int NE = 8 * 32 * NIJ;
+        for (int e = threadIdx.x; e < NE; e += blockDim.x) {
+            const int img = e / (32 * NIJ), k = (e / NIJ) % 32, w = e % NIJ;
+            const int r = img & 3, wr = (r & 1) ? BJ : BI, yl = w / wr, xl = w % wr;
+            // back to the brick's own column (ii, jj): is it inside the quadrant?
+            const int ii = r == 0 ? xl : r == 1 ? yl : r == 2 ? BI - 1 - xl : BI - 1 - yl;
+            const int jj = r == 0 ? yl : r == 1 ? BJ - 1 - xl : r == 2 ? BJ - 1 - yl : xl;
+            const int kk = k0 + k;
+            if (kk >= Q.nzh || i0 + ii >= ni || j0 + jj >= nj) continue;
+            int xg, yg;
+            bt_image(r, i0 + ii, j0 + jj, n1, xg, yg);
+            const int zg = img >= 4 ? P.nz - 1 - kk : kk;
+            const size_t o = ((size_t)zg * P.ny + yg) * P.nx + xg;
+            const float v = s_out[e];
+            out[o] = f ? fmaf(-coef, v, __ldg(f + o)) : v;
+        }
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
+cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out, unsigned int *errflag, cudaStream_t st)
+{
+    const LevelParams &P = L.p;
+    const BtPlan &B = L.bt;
+    auto kern = back_tma_kernel<BI, BJ, CPW, NSLOT, TP, MINB>;
+    static bool attr_set = false;       // per instantiation; the value only grows
+    static int attr_bytes = 0;
+    if (!attr_set || B.q.total > attr_bytes) {
+        CBCT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, B.q.total));
+        attr_set = true; attr_bytes = B.q.total;
+    }
+    const int ni = P.nx / 2, nj = P.ny / 2;
+    dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 31) / 32), b((BI * BJ / CPW + 1) * 32);
+    kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag);
+    return CBCT_OK;
+}
+
+}  // namespace
+
+// Plan of the TMA back-projector for one level, made once at create: which layout the residual stack takes, the tile
+// sizes that hold every stage of every brick (found by walking all bricks and views in fp64, with a margin; the kernel
+// counts violations in cbct_geometry::d_errflag), and the tensor maps.  plan.ok == false leaves the level to back.cu.
+cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
+{
+    const cbct_geometry_desc &d = g->desc;
+    LevelParams &P = L.p;
+    BtPlan &B = L.bt;
+    B.ok = false;
+    if (g->disable_tma || P.nsym != 4 || P.nmir != 2) return CBCT_OK;
+    if (L.back_maxc > BT_MAXC) return CBCT_OK;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return CBCT_OK;
+    const int BI = 4, BJ = 4;
+    const int ni = P.nx / 2, nj = P.ny / 2, nzh = P.nz / 2;
+    const double K = L.hz * d.sdd / L.dv;                               // K / depth = detector rows per z-index
+    const double u0 = -0.5 * (P.nu - 1) * L.du + d.det_off_u;
+    const double c0v_m = -(-0.5 * (P.nv - 1) * L.dv + d.det_off_v) / L.dv - 2.0e-3;
+    // the first-quadrant bricks under every view = their four images under the base views
+    double len_max = 0.0;
+    int span_max = 0, ncols_max = 0;
+    for (int a = 0; a < P.np; ++a) {
+        const double c = cos(g->angles[a]), s = sin(g->angles[a]);
+        const double dn = 1.01 * 0.5 * (fabs(c) * L.hx + fabs(s) * L.hy), du = 1.003 * 0.5 * (fabs(s) * L.hx + fabs(c) * L.hy);
+        for (int bj = 0; bj < nj; bj += BJ)
+            for (int bi = 0; bi < ni; bi += BI) {
+                double lo = 1e300, hi = -1e300, rn_lo = 1e300, rn_hi = -1e300;
+                for (int cj = 0; cj < 2; ++cj)
+                    for (int ci = 0; ci < 2; ++ci) {
+                        const int i = ci ? (bi + BI - 1 < ni ? bi + BI - 1 : ni - 1) : bi, j = cj ? (bj + BJ - 1 < nj ? bj + BJ - 1 : nj - 1) : bj;
+                        const double xc = (i - 0.5 * (P.nx - 1)) * L.hx, yc = (j - 0.5 * (P.ny - 1)) * L.hy;
+                        const double rn = xc * c + yc * s + d.sad, ru = xc * s - yc * c;
+                        const double mag = d.sdd / rn, uc = mag * ru, W = mag * (fabs(ru / rn) * dn + du);
+                        lo = fmin(lo, uc - W); hi = fmax(hi, uc + W);
+                        rn_lo = fmin(rn_lo, rn); rn_hi = fmax(rn_hi, rn);
+                    }
+                int iu_lo = (int)ceil((lo - u0) / L.du - 0.02), iu_hi = (int)floor((hi - u0) / L.du + 0.02);
+                if (iu_lo < 0) iu_lo = 0;
+                if (iu_hi > P.nu - 1) iu_hi = P.nu - 1;
+                if (iu_hi - iu_lo + 1 > ncols_max) ncols_max = iu_hi - iu_lo + 1;
+                // rows of one voxel (lowest slice, nearest depth of the brick) and of the brick's lowest 32 slices
+                const double len = K * ((double)nzh / (rn_lo - dn) - (double)(nzh - 1) / (rn_lo + dn)) + 5.0e-3;
+                if (len > len_max) len_max = len;
+                const int klast = nzh < 32 ? nzh - 1 : 31;
+                const double rfirst = ceil(-(double)nzh * K / (rn_lo - dn) + c0v_m) - 1.0;
+                const double rlast = ceil(-(double)(nzh - klast) * K / (rn_hi + dn) + c0v_m);
+                if ((int)(rlast - rfirst) > span_max) span_max = (int)(rlast - rfirst);
+            }
+    }
+    const int nslot = (int)floor(len_max) + 1;
+    if (nslot > 4) return CBCT_OK;
+    const int NSLOT = nslot <= 2 ? 2 : nslot;
+    const int TP = (K / d.sad >= 1.5 && P.nv % 2 == 0) ? 2 : 1;
+    // window: rows rfirst .. rlast + NSLOT, one row of alignment, the odd plane's shift, and a row of margin at each end
+    const int rows = span_max + NSLOT + 1 + 1 + (TP == 2 ? 3 : 1) + 2;
+    const int XB = ((rows + TP - 1) / TP + 7) / 8 * 8;
+    if (2 * XB > 256) return CBCT_OK;
+    const int ncols = ncols_max + 1;
+    if (ncols >= (1 << BT_NMAPS)) return CBCT_OK;
+
+    BtParams &q = B.q;
+    q.XB = XB; q.ncols = ncols; q.nzh = nzh;
+    q.plane_bytes = ncols * XB * 16;
+    q.half_bytes = TP * q.plane_bytes;
+    q.stage_bytes = 2 * q.half_bytes;
+    q.ic_scale = (float)K;
+    q.c0v_m = (float)c0v_m;
+    const int nw = BI * BJ;
+    int off = BT_NST * q.stage_bytes;
+    const int out_bytes = 8 * 32 * BI * BJ * 4;
+    if (off < out_bytes) off = out_bytes;
+    q.list_off = off; off += nw * 64 * 16;
+    q.view_off = off; off += P.nbase * 16;
+    q.hdr_off = off; off += BT_NST * 16;
+    q.bar_off = off; off += 2 * BT_NST * 8;
+    q.total = off;
+    q.vec4 = (P.nx % 4 == 0 && BI % 4 == 0 && BJ % 4 == 0) ? 1 : 0;
+    if (q.total > 227 * 1024) return CBCT_OK;
+    B.BI = BI; B.BJ = BJ; B.CPW = 1; B.NSLOT = NSLOT; B.TP = TP;
+    B.minb = 2 * (q.total + 1024) <= 228 * 1024 ? 2 : 1;
+
+    // the residual stack as a 4-d tensor of 8-byte elements: (2 x entry index within a plane, plane, column, base view)
+    const int tXP = P.nv / TP;
+    for (int b = 0; b < BT_NMAPS; ++b) {
+        cuuint64_t dims[4] = {(cuuint64_t)2 * tXP, (cuuint64_t)TP, (cuuint64_t)P.nu, (cuuint64_t)P.nbase};
+        cuuint64_t strides[3] = {(cuuint64_t)tXP * 16, (cuuint64_t)P.nv * 16, (cuuint64_t)P.nu * P.nv * 16};
+        cuuint32_t box[4] = {(cuuint32_t)2 * XB, 1u, 1u << b, 1u};
+        cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+        CUresult r = enc(&B.maps.m[b], CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, L.d_T, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cbct_fail(CBCT_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    }
+    P.tP = TP; P.tXP = tXP;
+    B.ok = true;
+    return CBCT_OK;
+}
+
+cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st)
+{
+    const BtPlan &B = L.bt;
+    cbct_status s = CBCT_ERR_INVALID_ARG;
+#define BT_CASE(NS, TPV)                                                                                         \
+    if (B.NSLOT == NS && B.TP == TPV)                                                                            \
+        s = B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2>(L, d_f, coef, d_out, g->d_errflag, st)                   \
+                        : bt_launch<4, 4, 1, NS, TPV, 1>(L, d_f, coef, d_out, g->d_errflag, st);
+    BT_CASE(2, 1) BT_CASE(3, 1) BT_CASE(4, 1) BT_CASE(2, 2) BT_CASE(3, 2) BT_CASE(4, 2)
+#undef BT_CASE
+    if (s != CBCT_OK) return s == CBCT_ERR_INVALID_ARG ? cbct_fail(s, "launch_back_tma: no kernel for this plan") : s;
+    CBCT_LAUNCH_CHECK(g);
+    return CBCT_OK;
+}

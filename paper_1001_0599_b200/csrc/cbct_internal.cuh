@@ -1,6 +1,7 @@
 // cbct_internal.cuh -- shared declarations of the CUDA product path (libcbct).
 // Nothing here is used by, or uses, the CPU oracle under oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <vector>
@@ -43,6 +44,8 @@ struct LevelParams {
     int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
     int nmir;                  // 2 when the z-mirror image of every ray / voxel shares its weights, else 1
     int stage_cells, t_entries; // cells of the staged copy / entries (R floats) of the residual stack: bounds of the gathers
+    int tP, tXP;               // residual stack: rows of a detector column stored in tP planes by row % tP (1 = plain), tXP = nv / tP
+                               // entries each: row iv sits at (iv % tP) * tXP + iv / tP of its column (back_tma.cu)
     int nyP, nzP;              // padded extents of the staged volume [i + PM][j + PM][k + PZ] (k fastest)
     int istride, jstride;      // its element strides along i and j (nyP * nzP, nzP)
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
@@ -55,8 +58,32 @@ struct LevelParams {
     int bc_xy, bc_z;
 };
 
+// ---- back_tma.cu: the TMA / shared-memory back-projector's per-level plan ----
+constexpr int BT_MAXC = 8;      // candidate detector columns per (voxel column, base view, image)
+constexpr int BT_NST = 2;       // depth of the tile ring
+constexpr int BT_NMAPS = 5;     // tensor maps with boxes of 1, 2, 4, 8, 16 detector columns
+struct BtMaps { CUtensorMap m[BT_NMAPS]; };
+struct BtParams {
+    int XB;                     // entries (rows) per plane of a tile column; a multiple of 8
+    int ncols;                  // tile columns: the widest brick shadow of the level
+    int plane_bytes, half_bytes, stage_bytes;   // ncols * XB * 16; x tP (the rows of one volume half); x 2
+    int list_off, view_off, hdr_off, bar_off, total;   // shared-memory carve-up (bytes)
+    int nzh;                    // nz / 2
+    int vec4;                   // results may leave with 16-byte stores
+    float ic_scale;             // hz * sdd / dv: detector rows per z-index at unit depth
+    float c0v_m;                // -v0 / dv - 2e-3: row index of v = 0, minus the range tolerance
+};
+struct BtConsts { float c0v_m, dv, v0; int rr_max; };
+struct BtPlan {
+    bool ok = false;
+    int BI = 0, BJ = 0, CPW = 0, NSLOT = 0, TP = 1, minb = 1;
+    BtParams q;
+    BtMaps maps;
+};
+
 struct Level {
     LevelParams p;
+    BtPlan bt;
     double hx, hy, hz, du, dv;
     size_t nvox, nray;
     RayU *d_rayu = nullptr;     // [np][nu]
@@ -97,6 +124,8 @@ struct cbct_geometry {
     mutable unsigned long long stage_calls[CBCT_N_STAGES] = {0};
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // 0,1 whole call; 2,3 stage timers; 4 first TV trial
     int sm_count = 148;
+    int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
+    unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always
 };
 
 // Debug builds (-DCBCT_ASSERT): device-side bounds checks of every gather index (compute-sanitizer stand-in).
@@ -169,6 +198,9 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
 //           out = f - coef * P^T in (f may be NULL: out = P^T in)
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
                         const float *d_f, float coef, float *d_out, cudaStream_t st);
+// back_tma.cu : plan of the TMA back-projector for a level (create time; needs L.d_T), and its launch (input = L.d_T)
+cbct_status bt_plan_level(const cbct_geometry *g, Level &L);
+cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st);
 // back_eq6.cu : out = f - coef * b6(T) with T in the plain [view][row][column] layout (f may be NULL: out = b6(T))
 cbct_status launch_back_eq6(const cbct_geometry *g, const Level &L, const float *d_T, const float *d_f, float coef,
                             float *d_out, cudaStream_t st);

@@ -220,15 +220,15 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                     out[o1] = T;
                     sq += (double)T * (double)T;
                 } else if (MODE == 2) {
-                    res[q] = pr * Lr;                  // L * (P f): input of the transpose without a residual
+                    res[q] = pr * scale;               // L inv_dd * (P f): input of the transpose without a residual
                 } else {
                     const float T = pr - __ldg(y + o1);
-                    res[q] = T * Lr;                   // what the transpose consumes (see back.cu)
+                    res[q] = T * scale;                // what the transpose consumes (see back.cu)
                     sq += (double)T * (double)T;
                 }
             }
             if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
-                const size_t ot = ((size_t)a * P.nu + iu) * P.nv + ivm;
+                const size_t ot = ((size_t)a * P.nu + iu) * P.nv + t_row_slot(P, ivm);
                 if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
                 else out[ot] = res[0];
             }

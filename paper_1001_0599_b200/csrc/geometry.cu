@@ -116,7 +116,7 @@ static void free_all(cbct_geometry *g)
         cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_cs); cudaFree(L.d_stage); cudaFree(L.d_T);
         cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_prev); cudaFree(L.d_y);
     }
-    cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter);
+    cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter); cudaFree(g->d_errflag);
     if (g->h_scalars) cudaFreeHost(g->h_scalars);
     for (int i = 0; i < 5; ++i) if (g->ev[i]) cudaEventDestroy(g->ev[i]);
     delete g;
@@ -147,12 +147,15 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     if (!g) return cbct_fail(CBCT_ERR_OOM, "host allocation failed");
     g->desc = *desc;
     g->allow_symmetry = desc->no_symmetry ? 0 : 1;
+    g->disable_tma = (desc->kernel_flags & CBCT_KERNEL_NO_TMA) ? 1 : 0;
     g->sm_count = prop.multiProcessorCount;
     g->angles.resize(desc->n_proj);
     for (int a = 0; a < desc->n_proj; ++a)
         g->angles[a] = desc->angles_rad ? desc->angles_rad[a] : 2.0 * M_PI * a / desc->n_proj;
     g->desc.angles_rad = nullptr;
 
+    st = dev_alloc(g, &g->d_errflag, (size_t)1);
+    if (st != CBCT_OK) { free_all(g); return st; }
     g->levels.resize(desc->max_levels);
     for (int l = 0; l < desc->max_levels; ++l) {
         Level &L = g->levels[l];
@@ -198,6 +201,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP * p.nmir;
         p.stage_cells = (int)(L.stage_elems / p.nmir);
         p.t_entries = (int)(L.nray / p.nsym);
+        p.tP = 1; p.tXP = p.nv;
         if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }
 
         std::vector<RayU> rays;
@@ -236,6 +240,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
             e = cudaMemcpy(L.d_cs, cs.data(), cs.size() * sizeof(double2), cudaMemcpyHostToDevice);
         }
         if (e != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "table upload: %s", cudaGetErrorString(e)); }
+        TRY(bt_plan_level(g, L));       // the TMA back-projector's tiles and the residual stack's layout (back_tma.cu)
     }
     {
         size_t need = 1024;
@@ -253,6 +258,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     TRY(dev_alloc(g, &g->d_partials, (size_t)4 * g->partials_stride));
     TRY(dev_alloc(g, &g->d_scalars, (size_t)kScalars));
     TRY(dev_alloc(g, &g->d_counter, (size_t)1));
+    if (cudaMemset(g->d_errflag, 0, sizeof(unsigned int)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset failed"); }
     if (cudaMemset(g->d_counter, 0, sizeof(unsigned int)) != cudaSuccess || cudaMemset(g->d_scalars, 0, sizeof(double) * kScalars) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the reduction scalars failed"); }
     g->objective_cap = 4096;
     TRY(dev_alloc(g, &g->d_objective, (size_t)2 * g->objective_cap));
@@ -272,6 +278,23 @@ extern "C" int cbct_geometry_symmetry(const cbct_geometry *g, int level)
 {
     const Level *L = get_level(g, level);
     return L ? L->p.nsym * L->p.nmir : 0;
+}
+
+extern "C" int cbct_geometry_back_path(const cbct_geometry *g, int level)
+{
+    const Level *L = get_level(g, level);
+    if (!L) return -1;
+    if (L->bt.ok) return CBCT_BACK_PATH_TMA;
+    return L->back_maxc <= 5 ? CBCT_BACK_PATH_LIST : CBCT_BACK_PATH_GATHER;
+}
+
+extern "C" cbct_status cbct_bound_violations(const cbct_geometry *g, unsigned int *count, void *cuda_stream)
+{
+    if (!g || !count) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_bound_violations: NULL argument");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CBCT_CUDA(cudaMemcpyAsync(count, g->d_errflag, sizeof(unsigned int), cudaMemcpyDeviceToHost, st));
+    CBCT_CUDA(cudaStreamSynchronize(st));
+    return CBCT_OK;
 }
 
 extern "C" unsigned long long cbct_geometry_device_bytes(const cbct_geometry *g) { return g ? g->device_bytes : 0ULL; }

@@ -39,6 +39,14 @@ __device__ __forceinline__ RayZ ray_z(const RayU &r, float v, float sz)
 // length in mm of the whole ray source -> pixel; one unit slab holds L * inv_dd of it
 __device__ __forceinline__ float ray_len_L(const RayU &r, float v) { return sqrtf(fmaf(v, v, r.c_l)); }
 
+// Position of detector row iv inside its column of the residual stack: plain, or split by row parity (LevelParams::tP,
+// back_tma.cu).  The stack holds L(u,v) * inv_dd(view, iu) * T: the length of one unit slab of the ray times the residual,
+// so that a back-projector's weight is the bare overlap of crossing parameters.
+__device__ __forceinline__ int t_row_slot(const LevelParams &P, int iv)
+{
+    return P.tP == 2 ? (iv & 1) * P.tXP + (iv >> 1) : iv;
+}
+
 __device__ __forceinline__ RayU load_rayu(const RayU *__restrict__ t, int idx)
 {
     const float4 *p = reinterpret_cast<const float4 *>(t + idx);
