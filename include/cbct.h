@@ -170,7 +170,8 @@ cbct_status cbct_tv_energy(const cbct_geometry *g, int level, const float *d_f, 
 cbct_status cbct_quality_metrics(const cbct_geometry *g, int level, const float *d_f, const float *d_f0,
                                  double *rel_error, double *correlation, void *cuda_stream);
 
-/* A8 grid transfers (L215-L223; readings S12, S13).  `level` is the FINE level of the pair.
+/* A8 grid transfers (L215-L223; readings S12, S13).  `level` is the FINE level of the pair.  Buffers need only
+ * their natural 4-byte alignment (8-byte aligned fine buffers take a faster load path).
  *   restrict: fine volume -> 2x2x2 mean on level+1.   bin: fine projections -> 2x2 mean.
  *   prolong : coarse volume (level+1) -> fine, cell-centred trilinear (3/4, 1/4); a missing
  *             neighbour is 0 under BC_ZERO and the edge value under BC_REFLECT. */
@@ -209,7 +210,9 @@ typedef struct {
 typedef struct {
     int n_iters_total;
     double *objective;   /* caller-owned HOST array of sum(iters) doubles or NULL:
-                            objective[it] = tv_weight*E1(f) + E2(f) of the f entering iteration it */
+                            objective[it] = tv_weight*E1(f) + E2(f) of the f entering iteration it.
+                            A monitored call (non-NULL) may run at most 4096 iterations in total
+                            (CBCT_ERR_INVALID_ARG beyond); unmonitored calls are not limited. */
     double *step_abs;    /* caller-owned HOST array of n_levels doubles or NULL: tau per level */
     int *iters_done;     /* caller-owned HOST array of n_levels ints or NULL: iterations run per level, coarsest ->
                             finest (= iters_per_level[] unless conv_tol stopped a level early); objective[] holds

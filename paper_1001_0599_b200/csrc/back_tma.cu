@@ -97,21 +97,23 @@ __device__ __forceinline__ void bt_shadow(const LevelParams &P, const float4 vw,
     iu_hi = min(P.nu - 1, __float2int_rd((uc + W - P.u0) * P.inv_du + 0.02f));
 }
 
-// One detector column's contribution to a voxel and its 7 images.  e0 = (s_lo, s_hi, e, q) as in back.cu; icn = 1/c at
-// the strip end nearer to the source, in detector rows per z-index; colA = the column's first entry in the stage's A
-// tile.  The voxel lies below the source plane (zlo + 1 <= 0): its rows have v < 0, so the two z-plane crossings come in
-// a known order -- plane zlo + 1 first when q > 0 -- and rows with v > 0 clip to weight 0 by the same expressions.
+// One detector column's contribution to a voxel and its 7 images.  e0 = (s_lo, s_hi, e, q) as in back.cu; e1 = (1/c at
+// the strip end nearer to the source in detector rows per z-index, the column's byte offset in the stage's A tile, and
+// the z-planes of the voxel -- as offsets from zlo -- that the rows cross first and second).  The voxel lies below the
+// source plane (zlo + 1 <= 0): its rows have v < 0, so the two crossings come in a known order -- plane zlo + 1 first
+// when q > 0 -- and rows with v > 0 clip to weight 0 by the same expressions.  A lane whose rows all lie below the
+// detector (the truncated bottom of the volume) does nothing.
 template <int SG, int NSLOT, int TP>
-__device__ __forceinline__ void bt_visit(float (&acc)[8], const char *__restrict__ colA, int KB, int plane_bytes,
-                                         float zlo, const float4 e0, float icn, int r0A, const BtConsts C)
+__device__ __forceinline__ void bt_visit(float (&acc)[8], const char *__restrict__ tile, int KB, int plane_bytes,
+                                         float zlo, const float4 e0, const float4 e1, int r0A, const BtConsts C)
 {
-    const int r = __float2int_ru(fmaf(zlo, icn, C.c0v_m));
+    const int r = __float2int_ru(fmaf(zlo, e1.x, C.c0v_m));
+    if (r + NSLOT <= 0) return;
     const int rr = r - r0A;
     CBCT_DEV_ASSERT(rr >= 0 && rr + NSLOT - 1 <= C.rr_max);
     const float q = e0.w, e = e0.z;
-    const bool qpos = q > 0.0f;
-    const float zA = qpos ? zlo + 1.0f : zlo, zB = qpos ? zlo : zlo + 1.0f;
-    const float tiny = copysignf(1.0e-37f, q);
+    const float zA = zlo + e1.z, zB = zlo + e1.w;
+    const char *colA = tile + __float_as_int(e1.y);
     int o0, d1;
     if (TP == 2) {
         const int p = rr & 1;
@@ -125,7 +127,7 @@ __device__ __forceinline__ void bt_visit(float (&acc)[8], const char *__restrict
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
         const float v = fmaf(rf + (float)s, C.dv, C.v0);
-        const float inv = rcp_approx(fmaf(v, q, tiny));
+        const float inv = rcp_approx(v * q);           // v != 0: the detector is centred in v with an even row count
         const float qa = fmaf(zA, inv, -e), qb = fmaf(zB, inv, -e);
         const float w = fmaxf(fminf(qb, e0.y) - fmaxf(qa, e0.x), 0.0f);
         const int os = TP == 2 ? o0 + (s & 1) * d1 + (s >> 1) * 16 : o0 + 16 * s;
@@ -179,76 +181,81 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[cp][q] = 0.0f;
 
+    // ---------------- every stage's detector rectangle, by all warps, before the ring starts ----------------
+    // header = (skip, first detector column, first row of the A window, columns)
+    for (int s = warp; s < n_stages; s += NW + 1) {
+        const int a = s >> 2, sg = s & 3;
+        const float4 vw = s_view[a];
+        int cmin = 1 << 30, cmax = -1;
+        float rn_lo = 3.0e38f, rn_hi = -3.0e38f;
+        for (int v = lane; v < NIJ; v += 32) {
+            const int i = i0 + v % BI, j = j0 + v / BI;
+            if (i < ni && j < nj) {
+                int mi, mj, lo, hi;
+                float rn;
+                bt_image(sg, i, j, n1, mi, mj);
+                bt_shadow(P, vw, mi, mj, lo, hi, rn);
+                if (lo <= hi) { cmin = min(cmin, lo); cmax = max(cmax, min(hi, lo + BT_MAXC - 1)); }
+                rn_lo = fminf(rn_lo, rn); rn_hi = fmaxf(rn_hi, rn);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            cmin = min(cmin, __shfl_xor_sync(0xffffffffu, cmin, o));
+            cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
+            rn_lo = fminf(rn_lo, __shfl_xor_sync(0xffffffffu, rn_lo, o));
+            rn_hi = fmaxf(rn_hi, __shfl_xor_sync(0xffffffffu, rn_hi, o));
+        }
+        // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
+        // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
+        const int klast = min(k0 + 31, Q.nzh - 1);
+        const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
+        const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
+        const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
+        const int rlast = __float2int_ru(fmaf(zl, ic_min, Q.c0v_m)) + NSLOT;
+        int ncols = cmax - cmin + 1;
+        const bool skip = ncols <= 0 || rlast < 0 || rmin > P.nv - 1;
+        const int x0 = TP == 2 ? (rmin >> 1) : rmin, r0A = TP * x0;
+        if (!skip && (ncols > Q.ncols || rlast - r0A > C.rr_max)) {   // the bounds of create do not hold: flag, stay in bounds
+            if (lane == 0) atomicAdd(errflag, 1u);
+            ncols = min(ncols, Q.ncols);
+        }
+        if (lane == 0) s_hdr[s] = make_int4(skip ? 1 : 0, cmin, r0A, ncols);
+    }
+    __syncthreads();
+
     if (warp == NW) {
-        // ---------------- producer: the stage's detector rectangle, then the tile copies ----------------
-        for (int s = 0; s < n_stages; ++s) {
-            const int a = s >> 2, sg = s & 3, slot = s % BT_NST, use = s / BT_NST;
-            if (use > 0) mbar_wait(bar0 + 8 * (BT_NST + slot), (use - 1) & 1);
-            const float4 vw = s_view[a];
-            int cmin = 1 << 30, cmax = -1;
-            float rn_lo = 3.0e38f, rn_hi = -3.0e38f;
-            for (int v = lane; v < NIJ; v += 32) {
-                const int i = i0 + v % BI, j = j0 + v / BI;
-                if (i < ni && j < nj) {
-                    int mi, mj, lo, hi;
-                    float rn;
-                    bt_image(sg, i, j, n1, mi, mj);
-                    bt_shadow(P, vw, mi, mj, lo, hi, rn);
-                    if (lo <= hi) { cmin = min(cmin, lo); cmax = max(cmax, min(hi, lo + BT_MAXC - 1)); }
-                    rn_lo = fminf(rn_lo, rn); rn_hi = fmaxf(rn_hi, rn);
-                }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                cmin = min(cmin, __shfl_xor_sync(0xffffffffu, cmin, o));
-                cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
-                rn_lo = fminf(rn_lo, __shfl_xor_sync(0xffffffffu, rn_lo, o));
-                rn_hi = fmaxf(rn_hi, __shfl_xor_sync(0xffffffffu, rn_hi, o));
-            }
-            // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
-            // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
-            const int klast = min(k0 + 31, Q.nzh - 1);
-            const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
-            const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
-            const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
-            const int rlast = __float2int_ru(fmaf(zl, ic_min, Q.c0v_m)) + NSLOT;
-            int ncols = cmax - cmin + 1;
-            const bool skip = ncols <= 0 || rlast < 0 || rmin > P.nv - 1;
-            const int x0 = TP == 2 ? (rmin >> 1) : rmin, r0A = TP * x0;
-            if (!skip && (ncols > Q.ncols || rlast - r0A > C.rr_max)) {   // the bounds of create do not hold: flag, stay in bounds
-                if (lane == 0) atomicAdd(errflag, 1u);
-                ncols = min(ncols, Q.ncols);
-            }
-            if (lane == 0) {
-                s_hdr[slot] = make_int4(skip ? 1 : 0, cmin, r0A, ncols);
+        // ---------------- producer: the tile copies, one stage ahead of the consumers ----------------
+        if (lane == 0) {
+            for (int s = 0; s < n_stages; ++s) {
+                const int a = s >> 2, slot = s % BT_NST, use = s / BT_NST;
+                if (use > 0) mbar_wait(bar0 + 8 * (BT_NST + slot), (use - 1) & 1);
+                const int4 hdr = s_hdr[s];
                 const uint32_t full = bar0 + 8 * slot;
-                if (skip) {
-                    mbar_arrive(full);
-                } else {
-                    const uint32_t tile = smem_u32(smem + slot * Q.stage_bytes);
-                    const uint32_t col_bytes = Q.XB * 16;
-                    mbar_arrive_expect_tx(full, (uint32_t)(2 * TP * ncols) * col_bytes);
-                    int c = 0;
+                if (hdr.x) { mbar_arrive(full); continue; }
+                const int cmin = hdr.y, ncols = hdr.w, x0 = hdr.z / TP;
+                const uint32_t tile = smem_u32(smem + slot * Q.stage_bytes);
+                const uint32_t col_bytes = Q.XB * 16;
+                mbar_arrive_expect_tx(full, (uint32_t)(2 * TP * ncols) * col_bytes);
+                int c = 0;
 #pragma unroll
-                    for (int b = BT_NMAPS - 1; b >= 0; --b) {
-                        if (ncols & (1 << b)) {
-                            const uint32_t dst = tile + c * col_bytes;
-                            if (TP == 2) {
-                                const int xb1 = P.nv / 2 - x0 - Q.XB;      // origin of the mirror rows' odd plane
-                                tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
-                                tma_load_4d(dst + Q.plane_bytes, &maps.m[b], 2 * (x0 - 1), 1, cmin + c, a, full);
-                                tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (xb1 + 1), 0, cmin + c, a, full);
-                                tma_load_4d(dst + Q.half_bytes + Q.plane_bytes, &maps.m[b], 2 * xb1, 1, cmin + c, a, full);
-                            } else {
-                                tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
-                                tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (P.nv - x0 - Q.XB), 0, cmin + c, a, full);
-                            }
-                            c += 1 << b;
+                for (int b = BT_NMAPS - 1; b >= 0; --b) {
+                    if (ncols & (1 << b)) {
+                        const uint32_t dst = tile + c * col_bytes;
+                        if (TP == 2) {
+                            const int xb1 = P.nv / 2 - x0 - Q.XB;      // origin of the mirror rows' odd plane
+                            tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
+                            tma_load_4d(dst + Q.plane_bytes, &maps.m[b], 2 * (x0 - 1), 1, cmin + c, a, full);
+                            tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (xb1 + 1), 0, cmin + c, a, full);
+                            tma_load_4d(dst + Q.half_bytes + Q.plane_bytes, &maps.m[b], 2 * xb1, 1, cmin + c, a, full);
+                        } else {
+                            tma_load_4d(dst, &maps.m[b], 2 * x0, 0, cmin + c, a, full);
+                            tma_load_4d(dst + Q.half_bytes, &maps.m[b], 2 * (P.nv - x0 - Q.XB), 0, cmin + c, a, full);
                         }
+                        c += 1 << b;
                     }
                 }
             }
-            __syncwarp();
         }
     } else {
         // ---------------- consumers ----------------
@@ -289,7 +296,10 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                         const float e = d0 - r.sd;
                         const float icA = rcp_approx(r.q * (e + s_lo)), icB = rcp_approx(r.q * (e + s_hi));
                         e0 = make_float4(s_lo, s_hi, e, r.q);
-                        e1 = make_float4(fmaxf(icA, icB) * P.inv_dv, __int_as_float(iu), 0.f, 0.f);
+                        const int cidx = iu - s_hdr[4 * a + sg].y;
+                        CBCT_DEV_ASSERT(s_hdr[4 * a + sg].x || (cidx >= 0 && cidx < s_hdr[4 * a + sg].w));
+                        e1 = make_float4(fmaxf(icA, icB) * P.inv_dv, __int_as_float(cidx * (Q.XB * 16)),
+                                         r.q > 0.0f ? 1.0f : 0.0f, r.q > 0.0f ? 0.0f : 1.0f);
                     }
                 }
                 const unsigned hit = __ballot_sync(0xffffffffu, ok);
@@ -304,7 +314,7 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                     const int sg = rd * SPR + t;
                     const int s = 4 * a + sg, slot = s % BT_NST, use = s / BT_NST;
                     mbar_wait(bar0 + 8 * slot, use & 1);
-                    const int4 hdr = s_hdr[slot];
+                    const int4 hdr = s_hdr[s];
                     if (!hdr.x) {
                         const char *tile = smem + slot * Q.stage_bytes;
 #pragma unroll
@@ -313,13 +323,10 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                             const int n_u = __popc(hit & (0xffu << (8 * uu)));
                             for (int n = 0; n < n_u; ++n) {
                                 const float4 E0 = l0[uu * 8 + n], E1 = l1[uu * 8 + n];
-                                const int cidx = __float_as_int(E1.y) - hdr.y;
-                                CBCT_DEV_ASSERT(cidx >= 0 && cidx < hdr.w);
-                                const char *colA = tile + cidx * (Q.XB * 16);
-                                if (sg == 0) bt_visit<0, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
-                                else if (sg == 1) bt_visit<1, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
-                                else if (sg == 2) bt_visit<2, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
-                                else bt_visit<3, NSLOT, TP>(acc[cp], colA, KB, Q.plane_bytes, zlo, E0, E1.x, hdr.z, C);
+                                if (sg == 0) bt_visit<0, NSLOT, TP>(acc[cp], tile, KB, Q.plane_bytes, zlo, E0, E1, hdr.z, C);
+                                else if (sg == 1) bt_visit<1, NSLOT, TP>(acc[cp], tile, KB, Q.plane_bytes, zlo, E0, E1, hdr.z, C);
+                                else if (sg == 2) bt_visit<2, NSLOT, TP>(acc[cp], tile, KB, Q.plane_bytes, zlo, E0, E1, hdr.z, C);
+                                else bt_visit<3, NSLOT, TP>(acc[cp], tile, KB, Q.plane_bytes, zlo, E0, E1, hdr.z, C);
                             }
                         }
                     }
@@ -499,7 +506,7 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     if (off < out_bytes) off = out_bytes;
     q.list_off = off; off += nw * 64 * 16;
     q.view_off = off; off += P.nbase * 16;
-    q.hdr_off = off; off += BT_NST * 16;
+    q.hdr_off = off; off += 4 * P.nbase * 16;
     q.bar_off = off; off += 2 * BT_NST * 8;
     q.total = off;
     q.vec4 = (P.nx % 4 == 0 && BI % 4 == 0 && BJ % 4 == 0) ? 1 : 0;

@@ -58,8 +58,7 @@ cbct_status check_params(const cbct_geometry *g, const cbct_fbs_params *p)
         if (p->iters_per_level[l] < 0) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: negative iteration count");
         total += p->iters_per_level[l];
     }
-    if (total > g->objective_cap)
-        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: more than %d iterations in one call", g->objective_cap);
+    (void)total;
     if (!(p->tv_weight >= 0.0) || !(p->step > 0.0 && p->step < 2.0))
         return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: need tv_weight >= 0 and 0 < step < 2");
     if (!(p->conv_tol >= 0.0)) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: conv_tol must be >= 0");
@@ -77,6 +76,16 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
     cbct_status s;
     const int nl = p->n_levels;
     const bool want_obj = rep && rep->objective;
+    {   // the objective monitor keeps one (E1, E2) pair per iteration on the device: its capacity bounds monitored calls only
+        long total = 0;
+        for (int l = 0; l < nl; ++l) total += p->iters_per_level[l];
+        if (want_obj && total > g->objective_cap)
+            return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: more than %d iterations in one call with the "
+                             "objective monitor on (report->objective != NULL)", g->objective_cap);
+    }
+    // slot of iteration n's (E1, E2) pair: its own when monitored, else two scratch pairs taken in turn (the next
+    // iteration's forward projection may be queued while this one's pair is still unread)
+    auto obj_slot = [&](int n) { return g->d_objective + 2 * (want_obj ? n : (n & 1)); };
     CBCT_CUDA(cudaEventRecord(g->ev[0], st));
 
     // data pyramid: y_l = 2x2 mean of y_{l-1}  (S12)
@@ -119,11 +128,11 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
             if (p->conv_tol > 0.0)      // keep the volume that enters the iteration for the convergence test
                 CBCT_CUDA(cudaMemcpyAsync(L.d_prev, f, L.nvox * sizeof(float), cudaMemcpyDeviceToDevice, st));
             if (!fwd_queued) {
-                if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, g->d_objective + 2 * done + 1, st)) != CBCT_OK) return s;
+                if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, obj_slot(done) + 1, st)) != CBCT_OK) return s;
             }
             fwd_queued = false;
             if (want_obj) {
-                if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, g->d_objective + 2 * done, st)) != CBCT_OK) return s;
+                if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, obj_slot(done), st)) != CBCT_OK) return s;
             }
             {
                 if (eq6) s = launch_back_eq6(g, L, L.d_T, f, (float)(tau * c_norm), L.d_g, st);
@@ -132,7 +141,7 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
             }
             {
                 cbct_tv_report tr;
-                ForwardAhead fa = {g, &L, f, y, eq6 ? 4 : 1, g->d_objective + 2 * (done + 1) + 1, st};
+                ForwardAhead fa = {g, &L, f, y, eq6 ? 4 : 1, obj_slot(done + 1) + 1, st};
                 TvAhead ah = {forward_ahead, &fa, false};
                 const bool look_ahead = !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
                 if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st, look_ahead ? &ah : nullptr)) != CBCT_OK) return s;

@@ -436,6 +436,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         }
         double lam = 1.0 / beta, Enew = E0, Dm = 0.0;
         bool accepted = false;
+        int accepted_bt = -1;
         for (int bt = 0; bt <= tp.max_backtracks; ++bt) {
             {
                 StageTimer t(g, st, ST_TV_TRIAL);
@@ -460,7 +461,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
             }
             Enew = hs[4] / N + 0.5 * beta * hs[5] / N;
             ++r.trials;
-            if (Enew <= E0 - tp.armijo_c * lam * Dm) { accepted = true; break; }
+            if (Enew <= E0 - tp.armijo_c * lam * Dm) { accepted = true; accepted_bt = bt; break; }
             lam *= tp.shrink_alpha;
         }
         if (!accepted) break;
@@ -468,7 +469,9 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         const bool last = rel < tp.rel_tol || it + 1 == tp.max_inner;
         float *nxt = last ? d_f : bufs[which];      // d_f, d_f2, d_f, ...: never cur unless last (in place is fine)
         which ^= 1;
-        if (ahead && it == 0 && last) ahead->valid = true;      // d_f holds the candidate and stays as it is
+        // the work queued behind the FIRST trial saw that trial's candidate: it is good only if that very trial was the
+        // accepted one (a backtracked step has since overwritten d_f with another candidate) and the step is the last
+        if (ahead && it == 0 && last && accepted_bt == 0) ahead->valid = true;
         if (!(last && cur != d_f)) {                 // else the accepted trial already wrote max(f - lam d, 0) to d_f
             StageTimer t(g, st, ST_TV_UPDATE);
             if ((s = launch_update(g, n, cur, L.d_d, (float)lam, last ? nonneg : 0, nxt, st)) != CBCT_OK) return s;

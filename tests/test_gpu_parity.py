@@ -418,3 +418,52 @@ def test_fbs_look_ahead_projection_changes_nothing(torch, cbct, orc, tv_weight):
     assert (reps[0].inner_total > 10) == (tv_weight > 1.0)           # the two regimes the test is about
     want = orc.fbs(g, y, setup)
     assert rel_l2(outs[1], want.f) <= TOL_VOL
+
+
+def _noisy_48():
+    g = I.Geometry(nx=48, ny=48, nz=32, hx=2.0, hy=2.0, hz=2.5, nu=64, nv=48, du=2.4, dv=2.4, sad=1000.0,
+                   sdd=1500.0, n_proj=12)
+    ell = [I.Ellipsoid((0.0, 0.0, 0.0), (40.0, 34.0, 36.0), 0.0, 0.02)] + \
+        I.random_ellipsoids(np.random.default_rng(111), 6, (48.0, 48.0, 40.0), axes_range=(4.0, 14.0))
+    return g, I.poisson_log(I.analytic_projections(ell, g), 1e5, 112).astype(np.float32)
+
+
+def test_fbs_look_ahead_backtracked_and_last(torch, cbct, orc):
+    """The look-ahead projection is queued behind the FIRST trial of a prox call; when that trial is rejected and a
+    shrunken step is accepted AND is the last (max_inner = 1), the queued projection saw a rejected volume and must be
+    redone.  Bitwise equality with the plain sequence (objective monitor on), and parity with the oracle."""
+    g, y = _noisy_48()
+    setup = I.FbsSetup(iters_per_level=(3, 5), tv_weight=3000.0, max_inner=1)
+    outs, reps = [], []
+    with cbct.geometry_create(g, max_levels=2) as h:
+        for objective in (True, False, False):
+            f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+            reps.append(h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective))
+            outs.append(f.cpu().numpy())
+    assert reps[1].trials_total > reps[1].inner_total          # some accepted step had been backtracked to
+    assert reps[1].inner_total == 8                             # one descent step per prox call
+    assert outs[0].tobytes() == outs[1].tobytes() == outs[2].tobytes()
+    want = orc.fbs(g, y, setup)
+    assert (reps[1].inner_total, reps[1].trials_total) == (want.inner_total, want.trials_total)
+    assert rel_l2(outs[1], want.f) <= TOL_VOL
+
+
+@pytest.mark.parametrize("objective", [True, False])
+@pytest.mark.parametrize("kw", [dict(max_inner=1, tv_weight=300.0), dict(max_backtracks=0, tv_weight=3000.0),
+                                dict(max_backtracks=1, tv_weight=3000.0)])
+def test_fbs_short_prox_budgets_match_oracle(torch, cbct, orc, kw, objective):
+    """The ROF sub-solver cut short inside the FBS driver: a single descent step per call, and a backtracking budget
+    that runs out (the prox call then keeps f = g: PAPER.md:L155-L159, reading S8) -- with and without the monitor."""
+    g, y = _noisy_48()
+    setup = I.FbsSetup(iters_per_level=(3, 4), **kw)
+    want = orc.fbs(g, y, setup)
+    with cbct.geometry_create(g, max_levels=2) as h:
+        f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+        rep = h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective)
+        got = f.cpu().numpy()
+    assert (rep.inner_total, rep.trials_total) == (want.inner_total, want.trials_total)
+    if "max_backtracks" in kw and kw["max_backtracks"] == 0:
+        assert rep.trials_total > rep.inner_total               # the budget did run out in some call
+    assert rel_l2(got, want.f) <= TOL_VOL, rel_l2(got, want.f)
+    if objective:
+        np.testing.assert_allclose(rep.objective, want.objective, rtol=1e-4)
