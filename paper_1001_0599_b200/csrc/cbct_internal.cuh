@@ -73,7 +73,7 @@ struct BtParams {
     float ic_scale;             // hz * sdd / dv: detector rows per z-index at unit depth
     float c0v_m;                // -v0 / dv - 2e-3: row index of v = 0, minus the range tolerance
 };
-struct BtConsts { float c0v_m, dv, v0; int rr_max; };
+struct BtConsts { float c0v_m, dv, v0; int rr_max, plane_step8, step_even, step_odd, KB; };
 struct BtPlan {
     bool ok = false;
     int BI = 0, BJ = 0, CPW = 0, NSLOT = 0, TP = 1, minb = 1;
