@@ -461,9 +461,9 @@ def run_sweep(args):
         for nv in views:
             g = I.sweep_geometry(n, nv)
             with cbct.geometry_create(g) as h:
-                gen = torch.Generator(device="cuda").manual_seed(I.SEED_BASE + 5)
-                f = torch.rand(g.vol_shape, device="cuda", generator=gen) * 0.03
-                q = torch.rand(g.proj_shape, device="cuda", generator=gen)
+                # the seeded host generators of SURVEY.md section 8(d): the inputs tests/test_gpu_fullsize.py checks against the oracle
+                f = torch.from_numpy(I.uniform_volume(g, I.SEED_BASE + 5, hi=0.03)).cuda()
+                q = torch.from_numpy(I.uniform_projections(g, I.SEED_BASE + 6)).cuda()
                 p, b = torch.empty_like(q), torch.empty_like(f)
                 S = h.count_samples()
                 reps = max(3, min(args.steps, 10))

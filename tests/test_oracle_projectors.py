@@ -268,3 +268,34 @@ def test_eq6_taps_outside_the_detector_are_zero(orc):
                    n_proj=1)
     b = orc.back_eq6(g, np.ones(g.proj_shape))
     assert b[4, 4, 4] > 0 and b[0, 4, 4] == 0.0 and b[4, 0, 4] == 0.0 and b[8, 8, 4] == 0.0
+
+
+def test_P1_sample_count_equals_brute_force_count(orc):
+    """S, the unit of the GUPS metric ("ray-tracing"; reading S2: one (ray, voxel) pair with positive
+    length): the traversal's count equals the number of (ray, voxel) pairs whose slab-method length
+    (`ray_box_len`, pinned by the hand surds) is positive, on a small off-centre anisotropic grid with generic angles
+    (no ray lies in a voxel face: the shortest positive length is far from 0)."""
+    g = I.Geometry(nx=9, ny=11, nz=7, hx=1.7, hy=1.3, hz=2.1, nu=10, nv=8, du=2.3, dv=2.9, sad=80.0, sdd=130.0,
+                   n_proj=4, vol_off=(0.7, -0.4, 0.3), det_off_u=0.31, det_off_v=-0.17,
+                   angles=np.deg2rad([13.0, 101.5, 222.2, 341.0]))
+    _, S = orc.forward(g, np.ones(g.vol_shape), return_samples=True)
+    h = 0.5 * np.array([g.hx, g.hy, g.hz])
+    centres = [np.array([(i - (g.nx - 1) / 2) * g.hx + g.vol_off[0], (j - (g.ny - 1) / 2) * g.hy + g.vol_off[1],
+                         (k - (g.nz - 1) / 2) * g.hz + g.vol_off[2]])
+               for k in range(g.nz) for j in range(g.ny) for i in range(g.nx)]
+    count, shortest, per_ray = 0, np.inf, []
+    for a in range(g.n_proj):
+        for iv in range(g.nv):
+            for iu in range(g.nu):
+                S0, D = orc.ray(g, a, iu, iv)
+                n = 0
+                for c in centres:
+                    ln = orc.ray_box_len(S0, D, c - h, c + h)
+                    if ln > 0.0:
+                        n += 1
+                        shortest = min(shortest, ln)
+                per_ray.append(n)
+                count += n
+    assert shortest > 1e-6                      # no grazing pair decides the count
+    assert S == count == 3882
+    assert max(per_ray) <= g.nx + g.ny + g.nz   # a ray crosses at most nx + ny + nz - 2 voxels

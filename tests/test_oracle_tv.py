@@ -153,3 +153,87 @@ def test_P13_grid_transfers(orc):
     # prolongation preserves the mean of interior-supported volumes (zero BC)
     blob = np.zeros((4, 6, 6)); blob[1:3, 2:4, 2:4] = rng.random((2, 2, 2))
     assert orc.prolong(blob, I.BC_ZERO, I.BC_ZERO).mean() == pytest.approx(blob.mean(), rel=1e-13)
+
+
+def _replay_prox(orc, g, gg, w, c, alpha, eps, max_inner, delta, max_bt=20):
+    """The loop of PAPER.md:L155-L159 spelled out once more on top of the two pinned primitives (rof_energy: P8 and
+    the numpy definition; rof_gradient: P7 finite differences): start at f = g, first trial step 1/beta, Eq. 5
+    `E_new <= E0 - c lam mean(d^2)` else lam <- alpha lam, stop when |E_new - E0| / E0 < eps.  Returns the counts, the
+    relative distance of every trial from the Armijo threshold and the relative decrease of every accepted step."""
+    beta = 1.0 / w
+    f = gg.copy()
+    e0 = orc.rof_energy(g, f, gg, beta, delta)
+    inner = trials = 0
+    margins, rels = [], []
+    for _ in range(max_inner):
+        d = orc.rof_gradient(g, f, gg, beta, delta)
+        dm = float(np.mean(d * d))
+        lam, ok = w, False
+        for _bt in range(max_bt + 1):
+            en = orc.rof_energy(g, f - lam * d, gg, beta, delta)
+            trials += 1
+            margins.append((en - (e0 - c * lam * dm)) / e0)
+            if en <= e0 - c * lam * dm:
+                ok = True
+                break
+            lam *= alpha
+        if not ok:
+            break
+        f = f - lam * d
+        inner += 1
+        rels.append(abs(en - e0) / e0)
+        e0 = en
+        if rels[-1] < eps:
+            break
+    return inner, trials, margins, rels, f
+
+
+@pytest.mark.parametrize("w,c,alpha", [(2e-3, 0.01, 0.6), (2e-2, 0.01, 0.6), (2e-2, 0.5, 0.6), (0.2, 0.9, 0.6), (2e-2, 0.5, 0.3)])
+def test_P9b_armijo_constant_and_shrink_decide_the_trial_count(orc, w, c, alpha):
+    """Eq. 5 with its constant c and the shrink factor alpha (L159): the first trial step 1/beta
+    overshoots, so the accepted step is reached after a KNOWN number of rejected trials, each of which misses the
+    threshold E0 - c lam mean(d^2) by a margin far from a tie.  An oracle that dropped c (accepted any decrease), put it
+    on the wrong term or shrank by another factor returns other counts."""
+    g = vol_geom(n=(12, 10, 8))
+    gg = np.random.default_rng(3).random(g.vol_shape) * 0.03
+    inner, trials, margins, _, f_want = _replay_prox(orc, g, gg, w, c, alpha, 0.0, 3, 1e-4)
+    assert inner == 3 and trials > inner                       # backtracking happened
+    assert min(abs(m) for m in margins) > 5e-5                 # no trial sits on the threshold
+    f, rep = orc.tv_prox(g, gg, w, I.FbsSetup(eps_delta=1e-4, rel_tol=0.0, max_inner=3, armijo_c=c, shrink_alpha=alpha))
+    assert (rep.inner_iters, rep.trials) == (inner, trials)
+    np.testing.assert_allclose(f, f_want, rtol=0, atol=1e-15)
+
+
+def test_P9b_the_constant_matters(orc):
+    """Same problem, c = 0.01 (L159) against c = 0.9: some trials decrease the energy but not by c lam mean(d^2)."""
+    g = vol_geom(n=(12, 10, 8))
+    gg = np.random.default_rng(3).random(g.vol_shape) * 0.03
+    t = {}
+    for c in (0.0, 0.01, 0.9):
+        _, rep = orc.tv_prox(g, gg, 2e-3, I.FbsSetup(eps_delta=1e-4, rel_tol=0.0, max_inner=3, armijo_c=c))
+        t[c] = rep.trials
+    assert t[0.0] <= t[0.01] < t[0.9]
+    assert (t[0.01], t[0.9]) == (5, 15)
+
+
+def test_P9c_epsilon_stop_uses_the_relative_decrease_of_the_step(orc):
+    """The stop |E_new - E0| / E0 < eps (eps = 1e-3 there): eps placed between the relative decreases
+    of two known accepted steps stops exactly there; and the denominator is the energy BEFORE the step -- an eps between
+    |dE|/E0 and |dE|/E_new tells the two apart."""
+    g = vol_geom(n=(12, 10, 8))
+    gg = np.random.default_rng(3).random(g.vol_shape) * 0.03
+    w = 2e-2
+    _, _, _, rels, _ = _replay_prox(orc, g, gg, w, 0.01, 0.6, 0.0, 12, 1e-4)
+    assert rels[1] < 0.07 < rels[0] and min(rels[:5]) > 0.05 > rels[5]      # the fixture this test is built on
+    for eps, want in ((0.07, 2), (0.05, 6)):
+        inner, trials, _, _, f_want = _replay_prox(orc, g, gg, w, 0.01, 0.6, eps, 50, 1e-4)
+        assert inner == want
+        f, rep = orc.tv_prox(g, gg, w, I.FbsSetup(eps_delta=1e-4, rel_tol=eps, max_inner=50))
+        assert (rep.inner_iters, rep.trials) == (inner, trials)
+        np.testing.assert_allclose(f, f_want, rtol=0, atol=1e-15)
+    # between |dE|/E0 = rels[1] and |dE|/E_new = rels[1] / (1 - rels[1]): stops at step 2 only with E0 below the line
+    eps = 0.5 * (rels[1] + rels[1] / (1.0 - rels[1]))
+    _, rep = orc.tv_prox(g, gg, w, I.FbsSetup(eps_delta=1e-4, rel_tol=eps, max_inner=50))
+    assert rep.inner_iters == 2
+    _, rep = orc.tv_prox(g, gg, w, I.FbsSetup(eps_delta=1e-4, rel_tol=0.999 * rels[1], max_inner=50))
+    assert rep.inner_iters > 2
