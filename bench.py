@@ -37,16 +37,22 @@ from paper_1001_0599_b200 import inputs as I  # noqa: E402
 METRIC = "fbs_iterations_per_second"
 UNIT = "iter/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch at config 3, from the committed `ncu --set full`
-# capture of this command (profiles/r01e_ncu_full_summary.txt); None = not captured for that kernel.
-# L1 / L2 sector hit rates (%) and DRAM GB/s under ncu of the same capture (cold-cache, serialised launches): evidence for
-# the memory-path design of each kernel, not a timing
-NCU_COUNTERS = {"forward": {"l1_hit_pct": 68.1, "l2_hit_pct": 91.0, "l1tex_throughput_pct": 59.2},
-                "back": {"l1_hit_pct": 54.1, "l2_hit_pct": 95.1, "l1tex_throughput_pct": 83.4},
-                "tv_grad": {"l1_hit_pct": 18.4, "l2_hit_pct": 28.4}, "tv_trial": {"l1_hit_pct": 35.9, "l2_hit_pct": 27.4},
-                "tv_update": {"l1_hit_pct": 0.0, "l2_hit_pct": 0.0}}
-NCU_DRAM_BYTES_PER_LAUNCH = {"back": 149.91e6, "forward": 120.75e6, "tv_grad": 98.30e6, "tv_trial": 178.88e6,
-                             "tv_update": None}
+COUNTERS_FILE = os.path.join(ROOT, "profiles", "r02_counters.json")
+
+
+def _load_counters():
+    """ncu counters per kernel of the FBS step (DRAM bytes per launch, L1 / L2 hit rates, ...) from the tracked record the
+    capture step wrote (`python -m paper_1001_0599_b200.ncu_counters`): evidence for each kernel's memory path, not a timing.
+    The record carries a hash of the kernel sources it was captured from; when the sources have changed since, the
+    counters are stale and are NOT quoted (roofline.traffic = null)."""
+    from paper_1001_0599_b200 import ncu_counters
+    if not os.path.exists(COUNTERS_FILE):
+        return {}, {"counters_file": None}
+    rec = json.load(open(COUNTERS_FILE))
+    fresh = rec.get("kernel_sources_sha256") == ncu_counters.kernel_sources_sha256()
+    meta = {"counters_file": os.path.relpath(COUNTERS_FILE, ROOT), "counters_commit": rec.get("counters_commit"),
+            "counters_match_kernel_sources": fresh}
+    return (rec.get("kernels", {}) if fresh else {}), meta
 
 
 def _peaks():
@@ -135,6 +141,26 @@ def max_over_ranks(ms: float, world: int, device="cuda") -> float:
 def aggregate_value(steps: int, world: int, ms_total: float) -> float:
     """Whole-job throughput: every rank did `steps` units in `ms_total` (max over ranks)."""
     return world * steps / (ms_total / 1e3)
+
+
+def fov_mask(g) -> np.ndarray:
+    """Voxels whose centre every view sees: (u*, v*) of Eq. A6 inside the detector for all angles.
+    Measurement-side helper for the error restricted to the field of view (reading R4)."""
+    x = (np.arange(g.nx) - 0.5 * (g.nx - 1)) * g.hx + g.vol_off[0]
+    yy = (np.arange(g.ny) - 0.5 * (g.ny - 1)) * g.hy + g.vol_off[1]
+    z = (np.arange(g.nz) - 0.5 * (g.nz - 1)) * g.hz + g.vol_off[2]
+    umax, vmax = 0.5 * g.nu * g.du, 0.5 * g.nv * g.dv
+    inplane = np.ones((g.ny, g.nx), dtype=bool)
+    mag_min = np.full((g.ny, g.nx), np.inf)
+    X, Y = np.meshgrid(x, yy)
+    for t in g.angles_rad():
+        c, s_ = np.cos(t), np.sin(t)
+        rn = X * c + Y * s_ + g.sad
+        u = g.sdd * (X * s_ - Y * c) / rn
+        inplane &= np.abs(u - g.det_off_u) <= umax
+        mag_min = np.minimum(mag_min, rn / g.sdd)          # |z| <= vmax rn / sdd for the view that sees least of the column
+    zlim = vmax * mag_min                                       # (det_off_v = 0 in every config)
+    return inplane[None, :, :] & (np.abs(z)[:, None, None] <= zlim[None, :, :])
 
 
 def workload(name: str):
@@ -268,6 +294,18 @@ def run_ours(args):
         S = h.count_samples()
         h.step_bound()
         f_start = f.clone()
+        back_path = h.back_path(0)
+
+        # ---- measured gather ceilings: the calibration kernel over a buffer the size of the staged
+        # volume copy, each pattern from L2 (every run new to the SM) and from L1 (a 16 KB tile re-read 256 times), and the
+        # shared-memory patterns of the TMA back-projector
+        cal = torch.rand(70 * 2 ** 20 // 4, device="cuda")
+        ceilings = {}
+        for key, variant, reuse, iters in (("ldg4_run128B_from_l2", 0, 1, 128), ("ldg4_run128B_from_l1", 0, 256, 256),
+                                           ("ldg16_stride2_from_l2", 1, 1, 64), ("ldg16_stride2_from_l1", 1, 256, 128),
+                                           ("lds16_stride2_plain", 2, 1, 512), ("lds16_stride2_parity_split", 3, 1, 512)):
+            ceilings[key] = max(cbct.gather_ceiling(cal, variant, reuse, iters, stream=stream)[0] for _ in range(3))
+        del cal
 
         def step_device():
             return h.fbs_reconstruct(y, f, one, use_initial=True, objective=False, stream=stream)
@@ -326,6 +364,7 @@ def run_ours(args):
 
         # ---- whole reconstruction: all levels, all iterations (rank 0 reports) ---------------
         recon = None
+        recon_extra = {}
         if not args.no_recon:
             f.zero_()
             barrier()
@@ -343,11 +382,61 @@ def run_ours(args):
                      "rel_error_vs_phantom": e_rec, "correlation_vs_phantom": c_rec,
                      "rel_error_vs_phantom_host_entry": float(np.linalg.norm(vol_host - truth) / np.linalg.norm(truth))}
             del hr
+            # ---- beside the headline: the error inside the field of view, and the regime where the TV step does work ----
+            # (reading R4: under the normalisation S5 the configs' TV weight 0.01 is a very weak regulariser -- every
+            # prox call is one accepted step.  A coarse scan of the weight finds the one with the lowest error against the
+            # phantom; K finest-level iterations are then timed at that weight.  Reported, never the headline `value`.)
+            recon_extra = {}
+            if rank == 0 and not args.no_extra:
+                mask = fov_mask(g)
+                t_dev = torch.from_numpy(truth).cuda()
+                m_dev = torch.from_numpy(mask).cuda()
+
+                def errors(vol):
+                    d2 = (vol - t_dev) ** 2
+                    return (float(torch.sqrt(d2.sum() / (t_dev ** 2).sum())),
+                            float(torch.sqrt(d2[m_dev].sum() / (t_dev[m_dev] ** 2).sum())))
+
+                scan = []
+                for lam in (fbs.tv_weight, 1.0, 10.0, 100.0, 1000.0, 10000.0):
+                    sl = I.FbsSetup(**{**fbs.__dict__, "tv_weight": lam})
+                    f.zero_()
+                    rl = h.fbs_reconstruct(y, f, sl, objective=False, stream=stream)
+                    e_all, e_fov = errors(f)
+                    scan.append({"tv_weight": lam, "rel_error_vs_phantom": e_all, "rel_error_inside_fov": e_fov,
+                                 "recon_seconds": rl.ms_total / 1e3, "tv_inner_total": int(rl.inner_total),
+                                 "tv_trials_total": int(rl.trials_total)})
+                best = min(scan, key=lambda r_: r_["rel_error_inside_fov"])
+                sb = I.FbsSetup(**{**fbs.__dict__, "tv_weight": best["tv_weight"]})
+                f.zero_()
+                h.fbs_reconstruct(y, f, I.FbsSetup(**{**sb.__dict__, "iters_per_level": tuple(fbs.iters_per_level[:-1]) + (0,)}),
+                                  objective=False, stream=stream)
+                kb = I.FbsSetup(**{**sb.__dict__, "iters_per_level": (args.steps,)})
+                h.fbs_reconstruct(y, f, kb, use_initial=True, objective=False, stream=stream)     # warm-up
+                h.set_stage_timing(True)
+                rb = h.fbs_reconstruct(y, f, kb, use_initial=True, objective=False, stream=stream)
+                st_b = h.stage_ms()
+                h.set_stage_timing(False)
+                rb2 = h.fbs_reconstruct(y, f, kb, use_initial=True, objective=False, stream=stream)
+                tv_ms = sum(st_b[n][0] for n in ("tv_grad", "tv_trial", "tv_update")) / args.steps
+                all_ms = sum(v_[0] for v_ in st_b.values()) / args.steps
+                recon_extra = {"fov_voxel_fraction": float(mask.mean()),
+                               "rel_error_inside_fov": scan[0]["rel_error_inside_fov"],
+                               "tv_weight_scan": scan,
+                               "tv_active_regime": {"tv_weight": best["tv_weight"], "ms_per_step": rb2.ms_total / args.steps,
+                                                    "tv_inner_per_step": rb.inner_total / args.steps,
+                                                    "tv_trials_per_step": rb.trials_total / args.steps,
+                                                    "tv_ms_per_step": tv_ms, "tv_share_of_step": tv_ms / all_ms,
+                                                    "note": "config 3 at the TV weight with the lowest in-FOV error of the scan; "
+                                                            "an extra row, not the headline"}}
+                del t_dev, m_dev
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
+    if recon:
+        recon.update(recon_extra)
 
     K = args.steps
     sec_step = ms_total / 1e3 / K
@@ -358,6 +447,12 @@ def run_ours(args):
     # data path: the gather roofline is 128 B/clk/SM x 148 SMs x f_clk = 32 samples/clk/SM.  The TV passes stream
     # the volume arrays once: HBM roofline (measured copy bandwidth).
     l1_peak_gbs = 148 * 128 * sm_max_mhz * 1e6 / 1e9
+    counters, counters_meta = _load_counters() if args.workload == "config3" else ({}, {"counters_file": None})
+    # the measured ceiling of each projector's own pattern: the forward projector's 4-byte loads of contiguous runs served
+    # from L1; the back-projector's 16-byte loads two entries apart, from shared memory (TMA path) or from L1 (list kernel)
+    measured = {"forward": ("ldg4_run128B_from_l1", ceilings["ldg4_run128B_from_l1"]),
+                "back": (("lds16_stride2_parity_split", ceilings["lds16_stride2_parity_split"]) if back_path == "tma"
+                         else ("ldg16_stride2_from_l1", ceilings["ldg16_stride2_from_l1"]))}
     first = abs(inner / K - 1.0) < 1e-9          # one descent step per prox call: f is g itself in both passes
     # the trial pass also writes its volume (the result, when the step is accepted and last): + 4 bytes per voxel
     tv_bytes = {"tv_grad": 8.0 if first else 12.0, "tv_trial": 12.0 if first else 16.0, "tv_update": 12.0}
@@ -367,16 +462,17 @@ def run_ours(args):
             t = per[name]["ms_per_launch"] / 1e3
             kern[name] = {"bound": "l1-gather", "gups": S / t / 1e9, "achieved": 4.0 * S / t / 1e9, "peak": l1_peak_gbs,
                           "unit": "GB/s", "frac": 4.0 * S / t / 1e9 / l1_peak_gbs,
-                          "peak_source": "148 SMs x 128 B/clk x %.0f MHz (DESIGN.md section 7)" % sm_max_mhz}
+                          "peak_source": "analytic: 148 SMs x 128 B/clk x %.0f MHz (DESIGN.md section 7)" % sm_max_mhz,
+                          "peak_measured": measured[name][1], "frac_measured": 4.0 * S / t / 1e9 / measured[name][1],
+                          "peak_measured_source": "cbct_gather_ceiling: " + measured[name][0]}
     for name, bpv in tv_bytes.items():
         if per[name]["ms_per_launch"]:
             t = per[name]["ms_per_launch"] / 1e3
             kern[name] = {"bound": "hbm", "achieved": bpv * nvox / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
                           "frac": bpv * nvox / t / 1e9 / hbm_peak, "bytes_per_voxel": bpv, "peak_source": peak_src}
     for name in kern:
-        if args.workload == "config3":          # the committed capture is of this workload
-            kern[name]["ncu"] = dict(NCU_COUNTERS.get(name, {}), dram_bytes_per_launch=NCU_DRAM_BYTES_PER_LAUNCH.get(name),
-                                     source="profiles/r01e_ncu_full_summary.txt")
+        if name in counters:                    # the tracked capture is of this workload and of these kernel sources
+            kern[name]["ncu"] = counters[name]
     dominant = max((n for n in kern), key=lambda n: per[n]["ms_per_step"])
     roof = dict(kern[dominant])
     # the same kernel against the HBM roofline, for reference: algorithmic HBM bytes per launch
@@ -385,8 +481,10 @@ def run_ours(args):
         t = per[dominant]["ms_per_launch"] / 1e3
         roof["hbm"] = {"algorithmic_bytes": alg_hbm, "achieved": alg_hbm / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
                        "frac": alg_hbm / t / 1e9 / hbm_peak, "peak_source": peak_src}
-    roof.update({"kernel": dominant, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dominant) if args.workload == "config3" else None,
+    roof.update({"kernel": dominant, "traffic": counters.get(dominant, {}).get("dram_bytes_per_launch"),
                  "share_of_step": per[dominant]["ms_per_step"] / sum(v["ms_per_step"] for v in per.values())})
+    roof.update(counters_meta)
+    roof["back_path"] = back_path
 
     base = cpu_baseline(cfg, y_host)
     line = {
@@ -409,6 +507,7 @@ def run_ours(args):
                 "d2h_bytes_per_step": 4 * nvox, "ms_per_step": ms_e2e / K},
         "gpu_launches": int(launches),
         "roofline": roof,
+        "gather_ceilings_gbs": {k: round(v, 1) for k, v in ceilings.items()},
         "kernels": kern,
         "stage_ms_per_step": {n: round(v["ms_per_step"], 4) for n, v in per.items()},
         "projector_gups": {"samples_per_projection": int(S),
@@ -549,6 +648,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--no-recon", action="store_true", help="skip the whole-reconstruction timing")
+    ap.add_argument("--no-extra", action="store_true", help="skip the TV-weight scan / field-of-view error beside the headline")
     ap.add_argument("--sweep", action="store_true", help="config 5: operator microbenchmarks instead of the FBS step")
     ap.add_argument("--sweep-sizes", default="64,128,256,512")
     ap.add_argument("--sweep-views", default="1,40,360")

@@ -249,6 +249,17 @@ cbct_status cbct_set_stage_timing(cbct_geometry *g, int enable);
 cbct_status cbct_get_stage_ms(const cbct_geometry *g, float out_ms[CBCT_N_STAGES],
                               unsigned long long out_calls[CBCT_N_STAGES]);
 
+/* Measured ceiling of the gather patterns the projectors are made of: a calibration kernel
+ * issues blocks x 256 threads x iters x 8 independent loads from d_buf (n_floats floats, 16-byte aligned, caller-owned,
+ * any finite contents) and reports its device time and the bytes the lanes asked for.  variant 0: 4-byte loads, a warp
+ * reads one contiguous 128-byte run (forward projector); 1: 16-byte loads two entries apart (back-projector, L1 path);
+ * 2 / 3: 16-byte loads two entries apart from a shared-memory tile, plain / split by entry parity (back_tma.cu).
+ * The run's position is pseudo-random inside a 16 KB tile that moves every `reuse` loads (variants 0, 1): reuse = 1
+ * gathers from L2, a large reuse from L1.  d_sink: one float the kernel may write.  Synchronises the stream.
+ * Not part of the hot path: bench.py quotes the projectors' GUPS against it. */
+cbct_status cbct_gather_ceiling(const float *d_buf, unsigned long long n_floats, int variant, int reuse, int iters,
+                                float *d_sink, float *ms, unsigned long long *bytes, void *cuda_stream);
+
 /* Thread-local message of the last failing call on this thread ("" if none). */
 const char *cbct_last_error(void);
 const char *cbct_version(void);

@@ -33,7 +33,7 @@ EXPORTS = [
     "cbct_quality_metrics",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
-    "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_last_error", "cbct_version",
+    "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_gather_ceiling", "cbct_last_error", "cbct_version",
 ]
 
 
@@ -136,6 +136,7 @@ def load_library():
     lib.cbct_launch_count.restype = C.c_ulonglong
     lib.cbct_set_stage_timing.argtypes = [vp, ip]
     lib.cbct_get_stage_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_ulonglong)]
+    lib.cbct_gather_ceiling.argtypes = [vp, C.c_ulonglong, ip, ip, ip, vp, C.POINTER(C.c_float), C.POINTER(C.c_ulonglong), vp]
     lib.cbct_last_error.restype = C.c_char_p
     lib.cbct_version.restype = C.c_char_p
     for name in EXPORTS:
@@ -375,6 +376,18 @@ class Geometry:
         calls = (C.c_ulonglong * len(self.STAGES))()
         _check(load_library().cbct_get_stage_ms(self._h, ms, calls))
         return {k: (float(m), int(c)) for k, m, c in zip(self.STAGES, ms, calls)}
+
+
+def gather_ceiling(buf, variant: int, reuse: int = 1, iters: int = 64, stream=None):
+    """cbct_gather_ceiling: (GB/s the lanes were served, milliseconds) of one calibration launch over `buf`."""
+    import torch
+    if not (isinstance(buf, torch.Tensor) and buf.is_cuda and buf.dtype == torch.float32 and buf.is_contiguous()):
+        raise TypeError("buf: need a contiguous float32 CUDA tensor")
+    sink = torch.zeros(1, device=buf.device, dtype=torch.float32)
+    ms, nbytes = C.c_float(0.0), C.c_ulonglong(0)
+    _check(load_library().cbct_gather_ceiling(C.c_void_p(buf.data_ptr()), buf.numel(), variant, reuse, iters,
+                                              C.c_void_p(sink.data_ptr()), C.byref(ms), C.byref(nbytes), _stream_ptr(stream)))
+    return nbytes.value / (ms.value * 1e-3) / 1e9, ms.value
 
 
 def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False) -> Geometry:
