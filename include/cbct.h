@@ -73,6 +73,9 @@ typedef struct {
                                  for A/B measurements and for keeping the other paths under test. */
 } cbct_geometry_desc;
 #define CBCT_KERNEL_NO_TMA 1
+#define CBCT_KERNEL_HOST_ARMIJO 2 /* cbct_tv_prox sequenced by the host (one stream synchronisation per Armijo trial) instead
+                                     of the single cooperative kernel that takes every accept / shrink / stop decision on
+                                     the device; same passes, same decisions.  For A/B measurements and tests. */
 
 /* Validates the description, uploads per-view tables and allocates all scratch for
  * `max_levels` levels.  *out is NULL on failure. */

@@ -175,7 +175,7 @@ class Geometry:
     `desc` is any object with the attributes of `inputs.Geometry`.
     """
 
-    def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False):
+    def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False, host_armijo: bool = False):
         lib = load_library()
         self._h = C.c_void_p()
         self.desc = desc
@@ -192,7 +192,7 @@ class Geometry:
         d.angles_rad = ang.ctypes.data_as(C.POINTER(C.c_double))
         d.bc_xy, d.bc_z, d.max_levels = desc.bc_xy, desc.bc_z, self.max_levels
         d.no_symmetry = int(bool(no_symmetry))
-        d.kernel_flags = 1 if no_tma else 0          # CBCT_KERNEL_NO_TMA
+        d.kernel_flags = (1 if no_tma else 0) | (2 if host_armijo else 0)     # CBCT_KERNEL_NO_TMA | CBCT_KERNEL_HOST_ARMIJO
         _check(lib.cbct_geometry_create(C.byref(d), C.byref(self._h)))
 
     def close(self):
@@ -390,8 +390,9 @@ def gather_ceiling(buf, variant: int, reuse: int = 1, iters: int = 64, stream=No
     return nbytes.value / (ms.value * 1e-3) / 1e9, ms.value
 
 
-def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False) -> Geometry:
-    return Geometry(desc, max_levels, no_symmetry, no_tma)
+def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False,
+                    host_armijo: bool = False) -> Geometry:
+    return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo)
 
 
 def version() -> str:

@@ -125,6 +125,7 @@ struct cbct_geometry {
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // 0,1 whole call; 2,3 stage timers; 4 first TV trial
     int sm_count = 148;
     int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
+    int host_armijo = 0;            // bit 1: the host-sequenced Armijo loop instead of the cooperative TV-prox kernel
     unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always
 };
 
@@ -136,7 +137,7 @@ struct cbct_geometry {
 #define CBCT_DEV_ASSERT(x) ((void)0)
 #endif
 
-constexpr int kScalars = 16;
+constexpr int kScalars = 24;     // 0-2 gradient-pass sums, 4-5 trial sums, 8 E1, 9 Lhat max, 10 S, 16-21 cooperative TV-prox report
 
 // Attribution of device time to one kernel (or a short fixed group): CUDA events around the
 // launches on the library's stream, only when cbct_set_stage_timing switched it on (it adds a

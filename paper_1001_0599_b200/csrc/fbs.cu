@@ -87,6 +87,8 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
     // iteration's forward projection may be queued while this one's pair is still unread)
     auto obj_slot = [&](int n) { return g->d_objective + 2 * (want_obj ? n : (n & 1)); };
     CBCT_CUDA(cudaEventRecord(g->ev[0], st));
+    if (!g->host_armijo)        // the cooperative TV-prox kernel counts its descent steps and trials on the device
+        CBCT_CUDA(cudaMemsetAsync(g->d_scalars + 20, 0, 2 * sizeof(double), st));
 
     // data pyramid: y_l = 2x2 mean of y_{l-1}  (S12)
     {
@@ -143,7 +145,8 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
                 cbct_tv_report tr;
                 ForwardAhead fa = {g, &L, f, y, eq6 ? 4 : 1, obj_slot(done + 1) + 1, st};
                 TvAhead ah = {forward_ahead, &fa, false};
-                const bool look_ahead = !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
+                // (host-sequenced Armijo loop only: the cooperative kernel has no host wait to hide)
+                const bool look_ahead = g->host_armijo && !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
                 if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st, look_ahead ? &ah : nullptr)) != CBCT_OK) return s;
                 fwd_queued = look_ahead && ah.valid;
                 inner_total += tr.inner_iters;
@@ -165,10 +168,12 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
     }
     CBCT_CUDA(cudaEventRecord(g->ev[1], st));
     if (rep) {
+        if (!g->host_armijo) CBCT_CUDA(cudaMemcpyAsync(g->h_scalars + 20, g->d_scalars + 20, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CBCT_CUDA(cudaStreamSynchronize(st));
+        if (!g->host_armijo) { inner_total = (int)(g->h_scalars[20] + 0.5); trials_total = (int)(g->h_scalars[21] + 0.5); }
         rep->n_iters_total = done;
         rep->inner_total = inner_total;
         rep->trials_total = trials_total;
-        CBCT_CUDA(cudaEventSynchronize(g->ev[1]));
         CBCT_CUDA(cudaEventElapsedTime(&rep->ms_total, g->ev[0], g->ev[1]));
         if (want_obj && done > 0) {
             std::vector<double> h(2 * (size_t)done);

@@ -86,6 +86,9 @@ __global__ void stage_volume_packed_kernel(const float *__restrict__ in, float2 
 }
 
 constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x 8 detector columns
+#ifndef FWD_MINB
+#define FWD_MINB 2
+#endif
 
 // One staged cell: a voxel value (M == 1) or the mirror pair (f(k), f(nz-1-k)) (M == 2).
 template <int M> struct StageCell { typedef float type; };
@@ -99,7 +102,7 @@ __device__ __forceinline__ float cell_hi(float2 c) { return c.y; }
 // z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again, and -- the staged
 // copy being mirror-packed -- the same loads.  MODE as in launch_forward.
 template <int R, int M, int MODE>
-__global__ void __launch_bounds__(FWD_BV *FWD_BU, 2)
+__global__ void __launch_bounds__(FWD_BV *FWD_BU, FWD_MINB)
 forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
                unsigned int *__restrict__ counter, double *__restrict__ sum_out)
@@ -157,6 +160,9 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                 t = si; si = -sj; sj = t;
                 t = mi; mi = -mj; mj = t;
             }
+#ifdef FWD_UNROLL
+#pragma unroll FWD_UNROLL
+#endif
             for (int s = s_lo; s < s_hi; ++s) {
                 // crossing parameters of the next minor-axis plane and the next z-plane, clipped to the slab
                 const float sy = __saturatef((nexty - y0) * r.inv_m);

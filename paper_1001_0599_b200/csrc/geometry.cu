@@ -148,6 +148,11 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     g->desc = *desc;
     g->allow_symmetry = desc->no_symmetry ? 0 : 1;
     g->disable_tma = (desc->kernel_flags & CBCT_KERNEL_NO_TMA) ? 1 : 0;
+    g->host_armijo = (desc->kernel_flags & CBCT_KERNEL_HOST_ARMIJO) ? 1 : 0;
+    {   // the cooperative TV-prox kernel needs cooperative launches (every sm_100 device has them; checked all the same)
+        int coop = 0;
+        if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) g->host_armijo = 1;
+    }
     g->sm_count = prop.multiProcessorCount;
     g->angles.resize(desc->n_proj);
     for (int a = 0; a < desc->n_proj; ++a)
@@ -255,11 +260,11 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         }
         g->partials_stride = (int)need;
     }
-    TRY(dev_alloc(g, &g->d_partials, (size_t)4 * g->partials_stride));
+    TRY(dev_alloc(g, &g->d_partials, (size_t)8 * g->partials_stride));
     TRY(dev_alloc(g, &g->d_scalars, (size_t)kScalars));
-    TRY(dev_alloc(g, &g->d_counter, (size_t)1));
+    TRY(dev_alloc(g, &g->d_counter, (size_t)4));        // [0] ticket of the fused reductions, [1..2] tile tickets of the cooperative TV-prox
     if (cudaMemset(g->d_errflag, 0, sizeof(unsigned int)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset failed"); }
-    if (cudaMemset(g->d_counter, 0, sizeof(unsigned int)) != cudaSuccess || cudaMemset(g->d_scalars, 0, sizeof(double) * kScalars) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the reduction scalars failed"); }
+    if (cudaMemset(g->d_counter, 0, 4 * sizeof(unsigned int)) != cudaSuccess || cudaMemset(g->d_scalars, 0, sizeof(double) * kScalars) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the reduction scalars failed"); }
     g->objective_cap = 4096;
     TRY(dev_alloc(g, &g->d_objective, (size_t)2 * g->objective_cap));
 #undef TRY

@@ -8,8 +8,11 @@
 // value (BC_REFLECT) (L161).  div is the exact negative transpose (backward differences,
 // p_{-1} = 0).  Per-voxel terms are fp32, sums are fp64 in a fixed order (reduce.cuh).
 #include <math.h>
+#include <cooperative_groups.h>
 #include "cbct_internal.cuh"
 #include "reduce.cuh"
+
+namespace cg = cooperative_groups;
 
 struct TvDims {
     int nx, ny, nz;
@@ -80,14 +83,15 @@ struct TvTile {
     size_t plane;
 };
 
-__device__ __forceinline__ TvTile tv_tile(const TvDims &D, int zc)
+// tile (bx, by, bz) of the grid tv_grid() lays over the volume, for the warp threadIdx.y of a 32 x TV_WPB block
+__device__ __forceinline__ TvTile tv_tile(const TvDims &D, int zc, int bx, int by, int bz)
 {
     TvTile T;
     T.lane = threadIdx.x;
-    T.i0 = blockIdx.x * 32;
+    T.i0 = bx * 32;
     const int i = T.i0 + T.lane;
-    T.j0 = (blockIdx.y * TV_WPB + threadIdx.y) * TV_R;
-    T.k0 = blockIdx.z * zc;
+    T.j0 = (by * TV_WPB + threadIdx.y) * TV_R;
+    T.k0 = bz * zc;
     T.k1 = min(T.k0 + zc, D.nz);
     T.ks = T.k0 > 0 ? T.k0 - 1 : 0;
     T.hy = T.j0 > 0;
@@ -125,13 +129,10 @@ __device__ __forceinline__ float right_neighbour(float own, float rcol, int src,
 // Gradient pass at u = f:  d = -div p + beta (f - g);  out[0] = sum |grad f|_delta,
 // out[1] = sum (f-g)^2, out[2] = sum d^2.  FIRST: f is g itself (first descent step): no g loads.
 template <bool FIRST>
-__global__ void __launch_bounds__(32 * TV_WPB)
-tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ g, float beta, float delta2,
-               float *__restrict__ d_out, int zc, double *__restrict__ partials, int stride,
-               unsigned int *__restrict__ counter, double *__restrict__ out)
+__device__ __forceinline__ void tv_grad_tile(const TvDims &D, const TvTile &T, const float *__restrict__ f,
+                                             const float *__restrict__ g, float beta, float delta2,
+                                             float *__restrict__ d_out, double &e_tv, double &e_q, double &e_d)
 {
-    __shared__ double slot[32];
-    const TvTile T = tv_tile(D, zc);
     const float *pk = f + T.ks * T.plane;                                    // slice k
     const float *p2 = f + min(T.ks + 1, D.nz - 1) * T.plane;                 // slice k+2 (after the first advance)
     const float *pg = g + min(T.ks + 1, D.nz - 1) * T.plane;
@@ -152,7 +153,6 @@ tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restr
     hA = __ldg(pk + T.hro); hB = __ldg(p2 + T.hro);
     lA = __ldg(pk + T.lco); lB = __ldg(p2 + T.lco);
     rA = __ldg(pk + T.rco); rB = __ldg(p2 + T.rco);
-    double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
 
     auto step = [&](int k, float (&c)[TV_R + 1], float (&cn)[TV_R + 1], float (&cnn)[TV_R + 1], float (&gc)[TV_R],
                     float (&gnn)[TV_R], float hc, float hcn, float &hcnn, float lc, float lcn, float &lcnn, float rc,
@@ -233,6 +233,18 @@ tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restr
         if (k + 2 >= T.k1) break;
         step(k + 2, C, A, B, GC, GB, hC, hA, hB, lC, lA, lB, rC, rB);
     }
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(32 * TV_WPB)
+tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ g, float beta, float delta2,
+               float *__restrict__ d_out, int zc, double *__restrict__ partials, int stride,
+               unsigned int *__restrict__ counter, double *__restrict__ out)
+{
+    __shared__ double slot[32];
+    const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+    double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
+    tv_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
     double s[3];
     s[0] = block_sum(e_tv, slot);
     s[1] = block_sum(e_q, slot);
@@ -243,14 +255,10 @@ tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restr
 // Energy pass at u = f - lam*dir (TRIAL) or u = f:  out[0] = sum |grad u|_delta and, when rows == 2,
 // out[1] = sum (u-g)^2.  Same warp tiles and march; nothing but u(i+1) is exchanged between voxels.
 template <bool TRIAL>
-__global__ void __launch_bounds__(32 * TV_WPB)
-tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
-                 const float *__restrict__ g, float lam, float delta2, int zc, int rows,
-                 double *__restrict__ partials, int stride, unsigned int *__restrict__ counter,
-                 double *__restrict__ out, float *__restrict__ cand, int cand_clip)
+__device__ __forceinline__ void tv_energy_tile(const TvDims &D, const TvTile &T, const float *__restrict__ f,
+                                               const float *__restrict__ dir, const float *__restrict__ g, float lam,
+                                               float delta2, float *__restrict__ cand, int cand_clip, double &e_tv, double &e_q)
 {
-    __shared__ double slot[32];
-    const TvTile T = tv_tile(D, zc);
     const bool hasg = g != nullptr;
     const size_t ok = T.k0 * T.plane;
     size_t ocur = ok;                                             // slice k
@@ -270,7 +278,6 @@ tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__res
         GC[r] = 0.0f;
     }
     rA = field<TRIAL>(f, dir, lam, ok + T.rco); rB = field<TRIAL>(f, dir, lam, o2 + T.rco);
-    double e_tv = 0.0, e_q = 0.0;
 
     auto step = [&](int k, float (&c)[TV_R + 1], float (&cn)[TV_R + 1], float (&cnn)[TV_R + 1], float (&gc)[TV_R],
                     float (&gnn)[TV_R], float rc, float &rcnn) {
@@ -311,9 +318,22 @@ tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__res
         if (k + 2 >= T.k1) break;
         step(k + 2, C, A, B, GC, GB, rC, rB);
     }
+}
+
+template <bool TRIAL>
+__global__ void __launch_bounds__(32 * TV_WPB)
+tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
+                 const float *__restrict__ g, float lam, float delta2, int zc, int rows,
+                 double *__restrict__ partials, int stride, unsigned int *__restrict__ counter,
+                 double *__restrict__ out, float *__restrict__ cand, int cand_clip)
+{
+    __shared__ double slot[32];
+    const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+    double e_tv = 0.0, e_q = 0.0;
+    tv_energy_tile<TRIAL>(D, T, f, dir, g, lam, delta2, cand, cand_clip, e_tv, e_q);
     double s[2];
     s[0] = block_sum(e_tv, slot);
-    s[1] = hasg ? block_sum(e_q, slot) : 0.0;
+    s[1] = g != nullptr ? block_sum(e_q, slot) : 0.0;
     publish_and_finalize<2>(s, rows, partials, stride, counter, out, slot);
 }
 
@@ -345,6 +365,152 @@ __global__ void tv_update_kernel<float4>(size_t n, const float4 *f, const float4
             v.z = v.z < 0.0f ? 0.0f : v.z; v.w = v.w < 0.0f ? 0.0f : v.w;
         }
         out[o] = v;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// The whole TV-prox call as ONE cooperative kernel: the Armijo loop of L155-L159 runs on the device.
+//
+// A persistent grid (as many blocks as fit the GPU at once) walks the tiles of every pass; between passes a grid-wide
+// barrier, after which EVERY block adds the blocks' fp64 partial sums in index order -- the same number in every block, so
+// all blocks take the same accept / shrink / stop decision (Eq. 5; the epsilon rule) without a host round trip and
+// without a second kernel.  Passes, buffers and the order of the decisions are those of the host-sequenced loop
+// (run_tv_prox below): gradient pass, trial passes with lam = 1/beta, alpha/beta, ..., update, and the truncated trial
+// volume doubling as the result when the accepted step is the last.  Sums depend on the grid size only (fixed for a
+// device), never on timing: bitwise reproducible.
+// ---------------------------------------------------------------------------------------------------------------------
+struct TvCoop {
+    TvDims D;
+    const float *g;
+    float *f, *f2, *d;
+    double beta, armijo_c, alpha, rel_tol, n;
+    float delta2;
+    int max_inner, max_bt, nonneg, zc, ntx, nty, ntz;
+    size_t nvox;
+    double *partials;       // 6 rows of `stride` per-TILE partials (two sets of three, used in turn)
+    int stride;
+    unsigned int *ticket;   // two tile counters, used in turn by successive passes; 0 between calls
+    double *report;         // [0] inner, [1] trials, [2] E_first, [3] E_last of this call; [4], [5] += inner, trials
+};
+
+__global__ void __launch_bounds__(32 * TV_WPB, 4)
+tv_prox_coop_kernel(const TvCoop p)
+{
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double slot[32];
+    __shared__ double s_tot[3];
+    const int tid = threadIdx.y * 32 + threadIdx.x, nthr = 32 * TV_WPB;
+    const int ntiles = p.ntx * p.nty * p.ntz;
+    const unsigned nblk = gridDim.x;
+    int pset = 0;
+    __shared__ int s_tile;
+
+    // The tiles of a pass are handed out by a ticket counter (the blocks stay evenly loaded whatever ntiles / gridDim is);
+    // every tile publishes its own partial sums, so which block computed a tile does not enter any sum.
+    auto next_tile = [&]() {
+        __syncthreads();
+        if (tid == 0) s_tile = (int)atomicAdd(p.ticket + pset, 1u);
+        __syncthreads();
+        return s_tile;
+    };
+    auto publish = [&](int t, double a0, double a1, double a2, int rows) {
+        const double v[3] = {a0, a1, a2};
+        for (int r = 0; r < rows; ++r) {
+            const double s = block_sum(v[r], slot);
+            if (tid == 0) p.partials[(size_t)(pset * 3 + r) * p.stride + t] = s;
+        }
+    };
+    // grid barrier, then every block adds all tiles' partials in tile order: the same totals in every thread of the grid
+    auto grid_sums = [&](int rows, double (&tot)[3]) {
+        grid.sync();
+        if (blockIdx.x == 0 && tid == 0) p.ticket[pset] = 0u;        // free again two passes from now
+        for (int r = 0; r < rows; ++r) {
+            double acc = 0.0;
+            for (int i = tid; i < ntiles; i += nthr) acc += __ldcg(p.partials + (size_t)(pset * 3 + r) * p.stride + i);
+            const double s = block_sum(acc, slot);
+            if (tid == 0) s_tot[r] = s;
+        }
+        __syncthreads();
+        for (int r = 0; r < rows; ++r) tot[r] = s_tot[r];
+        __syncthreads();
+        pset ^= 1;
+    };
+    // out = src - lam dir (dir may be NULL: out = src), optionally truncated at 0; then a grid barrier
+    auto update = [&](const float *src, const float *dir, float lam, int clip, float *out) {
+        const size_t i0 = (size_t)blockIdx.x * nthr + tid, step = (size_t)nblk * nthr;
+        const bool vec = p.nvox % 4 == 0 && ((uintptr_t)src % 16 == 0) && ((uintptr_t)out % 16 == 0) && (!dir || (uintptr_t)dir % 16 == 0);
+        if (vec) {
+            for (size_t o = i0; o < p.nvox / 4; o += step) {
+                float4 v = reinterpret_cast<const float4 *>(src)[o];
+                if (dir) {
+                    const float4 w = reinterpret_cast<const float4 *>(dir)[o];
+                    v.x = fmaf(-lam, w.x, v.x); v.y = fmaf(-lam, w.y, v.y); v.z = fmaf(-lam, w.z, v.z); v.w = fmaf(-lam, w.w, v.w);
+                }
+                if (clip) {
+                    v.x = v.x < 0.0f ? 0.0f : v.x; v.y = v.y < 0.0f ? 0.0f : v.y;
+                    v.z = v.z < 0.0f ? 0.0f : v.z; v.w = v.w < 0.0f ? 0.0f : v.w;
+                }
+                reinterpret_cast<float4 *>(out)[o] = v;
+            }
+        } else {
+            for (size_t o = i0; o < p.nvox; o += step) {
+                const float v = dir ? fmaf(-lam, dir[o], src[o]) : src[o];
+                out[o] = (clip && v < 0.0f) ? 0.0f : v;
+            }
+        }
+        grid.sync();
+    };
+
+    const float *cur = p.g;
+    int which = 0, inner = 0, trials = 0;
+    double E0 = 0.0, e_first = 0.0, e_last = 0.0;
+    bool have_E0 = false, clipped = false;
+    for (int it = 0; it < p.max_inner; ++it) {
+        double tot[3];
+        for (int t = next_tile(); t < ntiles; t = next_tile()) {
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+            const TvTile T = tv_tile(p.D, p.zc, t % p.ntx, (t / p.ntx) % p.nty, t / (p.ntx * p.nty));
+            if (cur == p.g) tv_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+            else tv_grad_tile<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+            publish(t, a0, a1, a2, 3);
+        }
+        grid_sums(3, tot);
+        if (!have_E0) { E0 = tot[0] / p.n + 0.5 * p.beta * tot[1] / p.n; e_first = e_last = E0; have_E0 = true; }
+        const double Dm = tot[2] / p.n;
+        double lam = 1.0 / p.beta, Enew = E0;
+        bool accepted = false;
+        float *cand = cur != p.f ? p.f : nullptr;           // the trial also leaves its (truncated) volume in f unless f is what it reads
+        for (int bt = 0; bt <= p.max_bt; ++bt) {
+            for (int t = next_tile(); t < ntiles; t = next_tile()) {
+                double a0 = 0.0, a1 = 0.0;
+                const TvTile T = tv_tile(p.D, p.zc, t % p.ntx, (t / p.ntx) % p.nty, t / (p.ntx * p.nty));
+                tv_energy_tile<true>(p.D, T, cur, p.d, p.g, (float)lam, p.delta2, cand, p.nonneg, a0, a1);
+                publish(t, a0, a1, 0.0, 2);
+            }
+            double tr[3];
+            grid_sums(2, tr);
+            Enew = tr[0] / p.n + 0.5 * p.beta * tr[1] / p.n;
+            ++trials;
+            if (Enew <= E0 - p.armijo_c * lam * Dm) { accepted = true; break; }
+            lam *= p.alpha;
+        }
+        if (!accepted) break;
+        const double rel = fabs(Enew - E0) / E0;
+        const bool last = rel < p.rel_tol || it + 1 == p.max_inner;
+        float *nxt = last ? p.f : (which ? p.f2 : p.f);     // f, f2, f, ...: never cur unless last (in place is fine)
+        which ^= 1;
+        if (!(last && cur != p.f)) update(cur, p.d, (float)lam, last ? p.nonneg : 0, nxt);   // else the accepted trial wrote it
+        cur = nxt;
+        clipped = last;
+        ++inner;
+        E0 = Enew;
+        e_last = Enew;
+        if (last) break;
+    }
+    if (cur != p.f || (p.nonneg && !clipped)) update(cur, nullptr, 0.0f, p.nonneg, p.f);
+    if (blockIdx.x == 0 && tid == 0) {
+        p.report[0] = (double)inner; p.report[1] = (double)trials; p.report[2] = e_first; p.report[3] = e_last;
+        p.report[4] += (double)inner; p.report[5] += (double)trials;
     }
 }
 
@@ -393,6 +559,40 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
     return CBCT_OK;
 }
 
+// The cooperative kernel's launch: a grid of as many blocks as are resident at once.  The report (inner, trials, E_first,
+// E_last) lands in d_scalars[16..19]; d_scalars[20..21] accumulate the counts over calls (cbct_fbs_reconstruct zeroes them).
+static cbct_status launch_tv_prox_coop(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
+                                       int nonneg, const cbct_tv_params &tp, cudaStream_t st)
+{
+    static int occ = 0;
+    if (occ == 0) {
+        CBCT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel, 32 * TV_WPB, 0));
+        if (occ < 1) return cbct_fail(CBCT_ERR_CUDA, "the cooperative TV-prox kernel does not fit an SM");
+    }
+    TvCoop p;
+    p.D = tv_dims(L);
+    p.zc = tv_zchunk(g, p.D);
+    const dim3 tg = tv_grid(p.D, p.zc);
+    p.ntx = tg.x; p.nty = tg.y; p.ntz = tg.z;
+    p.g = d_g; p.f = d_f; p.f2 = L.d_f2; p.d = L.d_d;
+    p.beta = 1.0 / w; p.armijo_c = tp.armijo_c; p.alpha = tp.shrink_alpha; p.rel_tol = tp.rel_tol; p.n = (double)L.nvox;
+    p.delta2 = (float)(tp.eps_delta * tp.eps_delta);
+    p.max_inner = tp.max_inner; p.max_bt = tp.max_backtracks; p.nonneg = nonneg;
+    p.nvox = L.nvox;
+    p.partials = g->d_partials; p.stride = g->partials_stride;
+    p.ticket = g->d_counter + 1;
+    p.report = g->d_scalars + 16;
+    long blocks = (long)g->sm_count * occ;
+    const long ntiles = (long)tg.x * tg.y * tg.z;
+    if (blocks > ntiles) blocks = ntiles;
+    if (ntiles > g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
+    void *args[] = {&p};
+    StageTimer t(g, st, ST_TV_GRAD);
+    CBCT_CUDA(cudaLaunchCooperativeKernel((const void *)tv_prox_coop_kernel, dim3((unsigned)blocks), dim3(32, TV_WPB), args, 0, st));
+    CBCT_LAUNCH_CHECK(g);
+    return CBCT_OK;
+}
+
 // Host-sequenced control loop (the Armijo test needs two global sums per trial).  The gradient pass
 // and the first trial (its step 1/beta is known beforehand) are queued back to back and read with
 // ONE stream synchronisation; the accepted update carries the non-negativity truncation when the
@@ -402,7 +602,6 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
                         int nonneg, const cbct_tv_params &tp, cbct_tv_report *rep, bool sync_report,
                         cudaStream_t st, TvAhead *ahead)
 {
-    (void)sync_report;
     if (ahead) ahead->valid = false;
     cbct_tv_report r = {0, 0, 0.0, 0.0};
     const size_t n = L.nvox;
@@ -410,6 +609,18 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     if (w <= 0.0 || tp.max_inner == 0) {
         StageTimer t(g, st, ST_TV_UPDATE);
         if ((s = launch_update(g, n, d_g, nullptr, 0.0f, nonneg, d_f, st)) != CBCT_OK) return s;
+        if (rep) *rep = r;
+        return CBCT_OK;
+    }
+    if (!g->host_armijo) {
+        // the whole call is one cooperative kernel; its report is read only when the caller wants it now
+        if ((s = launch_tv_prox_coop(g, L, d_g, d_f, w, nonneg, tp, st)) != CBCT_OK) return s;
+        if (rep && sync_report) {
+            CBCT_CUDA(cudaMemcpyAsync(g->h_scalars + 16, g->d_scalars + 16, 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+            CBCT_CUDA(cudaStreamSynchronize(st));
+            r.inner_iters = (int)(g->h_scalars[16] + 0.5); r.trials = (int)(g->h_scalars[17] + 0.5);
+            r.e_first = g->h_scalars[18]; r.e_last = g->h_scalars[19];
+        }
         if (rep) *rep = r;
         return CBCT_OK;
     }

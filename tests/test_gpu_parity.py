@@ -174,8 +174,11 @@ def test_edge_cases_missing_rays_and_unseen_voxels(torch, cbct, orc):
     assert p.item() == pytest.approx(orc.forward(g1, np.full(g1.vol_shape, 2.0)).item(), rel=1e-6)
 
 
+@pytest.mark.parametrize("host_armijo", [False, True])
 @pytest.mark.parametrize("bc", [(I.BC_ZERO, I.BC_REFLECT), (I.BC_REFLECT, I.BC_REFLECT), (I.BC_ZERO, I.BC_ZERO)])
-def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc):
+def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc, host_armijo):
+    """Both control paths of the Armijo loop: the cooperative kernel that decides on the device (default) and the
+    host-sequenced loop (CBCT_KERNEL_HOST_ARMIJO)."""
     g = I.Geometry(nx=37, ny=45, nz=19, hx=1.7, hy=1.3, hz=2.9, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
                    n_proj=1, bc_xy=bc[0], bc_z=bc[1])
     rng = np.random.default_rng(41)
@@ -185,7 +188,7 @@ def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc):
     setup = I.FbsSetup(eps_delta=1e-5, max_inner=8, rel_tol=0.0)
     w = 2e-3
     want, wrep = orc.tv_prox(g, gg, w, setup)
-    with cbct.geometry_create(g) as h:
+    with cbct.geometry_create(g, host_armijo=host_armijo) as h:
         e1 = h.tv_energy(dev(torch, gg), setup.eps_delta)
         f = torch.empty(g.vol_shape, device="cuda", dtype=torch.float32)
         rep = h.tv_prox(dev(torch, gg), f, w, setup)
@@ -204,11 +207,12 @@ def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc):
     assert rep.e_last < rep.e_first
 
 
-def test_tv_prox_degenerate_cases(torch, cbct):
+@pytest.mark.parametrize("host_armijo", [False, True])
+def test_tv_prox_degenerate_cases(torch, cbct, host_armijo):
     g = I.Geometry(nx=16, ny=12, nz=6, hx=1.0, hy=1.0, hz=1.0, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
                    n_proj=1, bc_xy=I.BC_REFLECT, bc_z=I.BC_REFLECT)
     setup = I.FbsSetup()
-    with cbct.geometry_create(g) as h:
+    with cbct.geometry_create(g, host_armijo=host_armijo) as h:
         const = torch.full(g.vol_shape, 0.013, device="cuda", dtype=torch.float32)
         # constant volume, all-reflective BC: zero TV (north_star check), prox leaves it alone
         assert h.tv_energy(const, 0.0) == 0.0
@@ -406,7 +410,7 @@ def test_fbs_look_ahead_projection_changes_nothing(torch, cbct, orc, tv_weight):
     y = I.poisson_log(I.analytic_projections(ell, g), 1e5, 102).astype(np.float32)
     setup = I.FbsSetup(iters_per_level=(4, 6), tv_weight=tv_weight)
     outs, reps = [], []
-    with cbct.geometry_create(g, max_levels=2) as h:
+    with cbct.geometry_create(g, max_levels=2, host_armijo=True) as h:
         for objective in (True, False, False):
             f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
             reps.append(h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective))
@@ -433,7 +437,7 @@ def test_fbs_look_ahead_backtracked_and_last(torch, cbct, orc):
     g, y = _noisy_48()
     setup = I.FbsSetup(iters_per_level=(3, 5), tv_weight=3000.0, max_inner=1)
     outs, reps = [], []
-    with cbct.geometry_create(g, max_levels=2) as h:
+    with cbct.geometry_create(g, max_levels=2, host_armijo=True) as h:
         for objective in (True, False, False):
             f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
             reps.append(h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective))
@@ -446,16 +450,17 @@ def test_fbs_look_ahead_backtracked_and_last(torch, cbct, orc):
     assert rel_l2(outs[1], want.f) <= TOL_VOL
 
 
+@pytest.mark.parametrize("host_armijo", [False, True])
 @pytest.mark.parametrize("objective", [True, False])
 @pytest.mark.parametrize("kw", [dict(max_inner=1, tv_weight=300.0), dict(max_backtracks=0, tv_weight=3000.0),
                                 dict(max_backtracks=1, tv_weight=3000.0)])
-def test_fbs_short_prox_budgets_match_oracle(torch, cbct, orc, kw, objective):
+def test_fbs_short_prox_budgets_match_oracle(torch, cbct, orc, kw, objective, host_armijo):
     """The ROF sub-solver cut short inside the FBS driver: a single descent step per call, and a backtracking budget
     that runs out (the prox call then keeps f = g: PAPER.md:L155-L159, reading S8) -- with and without the monitor."""
     g, y = _noisy_48()
     setup = I.FbsSetup(iters_per_level=(3, 4), **kw)
     want = orc.fbs(g, y, setup)
-    with cbct.geometry_create(g, max_levels=2) as h:
+    with cbct.geometry_create(g, max_levels=2, host_armijo=host_armijo) as h:
         f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
         rep = h.fbs_reconstruct(dev(torch, y), f, setup, objective=objective)
         got = f.cpu().numpy()
@@ -553,3 +558,21 @@ def test_back_projector_paths_agree(torch, cbct, orc):
             assert rel_l2(o, want) <= TOL_PROJ, (name, rel_l2(o, want))
             assert np.abs(o - want).max() <= 1e-4 * np.abs(want).max()
         assert rel_l2(outs[False], outs[True]) <= 1e-6
+
+
+def test_fbs_device_and_host_armijo_agree_bitwise(torch, cbct, orc):
+    """The cooperative TV-prox kernel (every accept / shrink / stop decision taken on the device) against the
+    host-sequenced loop: the same passes in the same order, so the same volume bit for bit and the same counts --
+    in the regime of one descent step per call and in the regime of many backtracked steps."""
+    g, y = _noisy_48()
+    for tv_weight in (0.01, 300.0):
+        setup = I.FbsSetup(iters_per_level=(4, 5), tv_weight=tv_weight)
+        outs, reps = [], []
+        for host in (False, True):
+            with cbct.geometry_create(g, max_levels=2, host_armijo=host) as h:
+                f = torch.zeros(g.vol_shape, device="cuda", dtype=torch.float32)
+                reps.append(h.fbs_reconstruct(dev(torch, y), f, setup, objective=False))
+                outs.append(f.cpu().numpy())
+        assert outs[0].tobytes() == outs[1].tobytes()
+        assert (reps[0].inner_total, reps[0].trials_total) == (reps[1].inner_total, reps[1].trials_total)
+        assert (reps[0].trials_total > reps[0].inner_total) == (tv_weight > 1.0)
