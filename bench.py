@@ -203,8 +203,8 @@ def oracle_sample(cfg, y, views: int, z_div: int):
             "parts_s": {"P": (t1 - t0) * g.n_proj / views, "PT": (t2 - t1) * g.n_proj / views,
                         "tv_prox": (t4 - t3) * g.nz / nzs, "tv_inner": rep.inner_iters},
             "sample": f"oracle P and P^T on {views} of {g.n_proj} views at full resolution ({g.nx}x{g.ny}x{g.nz}, "
-                      f"{g.nu}x{g.nv}) scaled x{g.n_proj / views:.0f}, plus one oracle TV-prox call on a "
-                      f"{nzs}-slice slab scaled x{g.nz / nzs:.0f}; sum = one finest-level FBS iteration"}
+                      f"{g.nu}x{g.nv}) scaled x{g.n_proj / views:.4g}, plus one oracle TV-prox call on a "
+                      f"{nzs}-slice slab scaled x{g.nz / nzs:.4g}; sum = one finest-level FBS iteration"}
 
 
 def cpu_baseline(cfg, y, budget: str = "default"):
