@@ -269,8 +269,10 @@ def run_ours(args):
 
     k, cfg = workload(args.workload)
     g = cfg.geom
-    cfg.seed = rank_seed(cfg.seed, rank)
-    y_host = I.make_projections(cfg)
+    sharded = bool(args.sharded)
+    if not sharded:
+        cfg.seed = rank_seed(cfg.seed, rank)        # replicas: every rank its own noise realisation
+    y_host = I.make_projections(cfg)                # sharded: ONE problem, the same data on every rank
     n_levels = len(cfg.fbs.iters_per_level)
     fbs = cfg.fbs
     stream = torch.cuda.Stream()
@@ -307,8 +309,20 @@ def run_ours(args):
             ceilings[key] = max(cbct.gather_ceiling(cal, variant, reuse, iters, stream=stream)[0] for _ in range(3))
         del cal
 
+        # --sharded (NEXT-4): the ranks reconstruct ONE problem, the projectors sharded by output ownership
+        # (cbct_fbs_reconstruct_sharded; strong scaling).  At one GPU the communicator is trivial.
+        comm = None
+        if sharded:
+            comm = (cbct.torch_distributed_comm() if world > 1 else
+                    cbct.Comm(0, 1, lambda t, root: None, lambda t: None))
+
+        def run_fbs(setup, **kw):
+            if comm is not None:
+                return h.fbs_reconstruct_sharded(comm, y, f, setup, stream=stream, **kw)
+            return h.fbs_reconstruct(y, f, setup, stream=stream, **kw)
+
         def step_device():
-            return h.fbs_reconstruct(y, f, one, use_initial=True, objective=False, stream=stream)
+            return run_fbs(one, use_initial=True, objective=False)
 
         for _ in range(args.warmup):
             step_device()
@@ -332,7 +346,7 @@ def run_ours(args):
         with ClockSampler(local) as clk:
             torch.cuda.profiler.start()        # cudaProfilerStart: `ncu --profile-from-start off` sees only the timed region
             ev0.record(stream)
-            r = h.fbs_reconstruct(y, f, k_steps, use_initial=True, objective=False, stream=stream)
+            r = run_fbs(k_steps, use_initial=True, objective=False)
             ev1.record(stream)
             barrier()
             torch.cuda.profiler.stop()
@@ -344,12 +358,22 @@ def run_ours(args):
         # ---- e2e: the same step through the HOST entry point, copies inside the timed region -
         y_pin = torch.from_numpy(y_host).pin_memory()
         f_pin = f.cpu().pin_memory()
+        def step_e2e():
+            if comm is None:
+                h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
+            else:           # no host entry point of the sharded call: the same copies, issued here
+                y.copy_(y_pin, non_blocking=True)
+                f.copy_(f_pin, non_blocking=True)
+                run_fbs(one, use_initial=True, objective=False)
+                f_pin.copy_(f, non_blocking=True)
+                stream.synchronize()
+
         for _ in range(max(1, min(args.warmup, 2))):
-            h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
+            step_e2e()
         barrier()
         ev0.record(stream)
         for _ in range(args.steps):
-            h.fbs_reconstruct_host(y_pin, f_pin, one, use_initial=True, stream=stream)
+            step_e2e()
         ev1.record(stream)
         barrier()
         ms_e2e = max_over_ranks(ev0.elapsed_time(ev1), world)
@@ -368,7 +392,7 @@ def run_ours(args):
         if not args.no_recon:
             f.zero_()
             barrier()
-            rr = h.fbs_reconstruct(y, f, fbs, objective=False, stream=stream)
+            rr = run_fbs(fbs, objective=False)
             e_rec, c_rec = h.quality_metrics(f, torch.from_numpy(I.paint(cfg.ellipsoids, g)).cuda(), stream=stream)
             t0 = time.perf_counter()
             vol_host = np.zeros(g.vol_shape, dtype=np.float32)
@@ -497,12 +521,13 @@ def run_ours(args):
     roof["back_path"] = back_path
 
     base = cpu_baseline(cfg, y_host)
+    jobs = 1 if sharded else world              # sharded: all ranks worked on the same K steps
     line = {
-        "metric": METRIC, "value": aggregate_value(K, world, ms_total), "unit": UNIT, "n_gpus": world, "steps": K,
+        "metric": METRIC, "value": aggregate_value(K, jobs, ms_total), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms_total / K,
         "separate_calls_ms_per_step": {"mean": float(np.mean(per_step)), "median": float(np.median(per_step)),
                                        "best": float(np.min(per_step))},
-        "higher_is_better": True, "scaling": "weak",
+        "higher_is_better": True, "scaling": "strong" if sharded else "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"config{k} ({cfg.name}): {g.nx}x{g.ny}x{g.nz} fp32 voxels at {g.hx} mm, {g.n_proj} views "
                                f"of {g.nu}x{g.nv} at {g.du} mm, one finest-level FBS iteration per step after "
@@ -511,9 +536,10 @@ def run_ours(args):
                    "iters_per_level": list(fbs.iters_per_level),
                    "l2": "working set (5 volumes + 2 projection stacks = %.0f MiB) exceeds the 126 MB L2; no flush"
                          % ((5 * nvox + 2 * nray) * 4 / 2 ** 20),
-                   "parallelism": "independent problem per GPU" if world > 1 else "single GPU"},
+                   "parallelism": ("projectors sharded by output ownership over %d GPUs (cbct_fbs_reconstruct_sharded)" % world
+                                   if sharded else "independent problem per GPU" if world > 1 else "single GPU")},
         "clocks": clocks,
-        "e2e": {"value": aggregate_value(K, world, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 4 * (nray + nvox),
+        "e2e": {"value": aggregate_value(K, jobs, ms_e2e), "unit": UNIT, "h2d_bytes_per_step": 4 * (nray + nvox),
                 "d2h_bytes_per_step": 4 * nvox, "ms_per_step": ms_e2e / K},
         "gpu_launches": int(launches),
         "roofline": roof,
@@ -666,6 +692,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--sharded", action="store_true",
+                    help="N ranks reconstruct ONE problem, projectors sharded by output ownership (strong scaling); "
+                         "default under torchrun: N independent problems (weak scaling)")
     ap.add_argument("--no-recon", action="store_true", help="skip the whole-reconstruction timing")
     ap.add_argument("--no-extra", action="store_true", help="skip the TV-weight scan / field-of-view error beside the headline")
     ap.add_argument("--sweep", action="store_true", help="config 5: operator microbenchmarks instead of the FBS step")

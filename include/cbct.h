@@ -236,6 +236,37 @@ cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_pro
                                       float *h_vol_inout, const cbct_fbs_params *params,
                                       cbct_fbs_report *report, void *cuda_stream);
 
+/* NEXT-4 -- the reconstruction sharded over `world` GPUs by OUTPUT OWNERSHIP (one process and one handle per GPU, every
+ * rank calling with the same arguments).  Every rank holds the whole volume and the whole data; per iteration
+ *   - rank r projects ITS base views (cbct_shard_range over cbct_shard_units' n_base_views; with quarter-turn symmetry a
+ *     base view stands for its four quarter-turn partners) and the residual chunks are broadcast from their owners;
+ *   - the blocks' partial sums of T^2 are added across ranks (every slot is written by exactly one rank, the others hold
+ *     0, so the addition is exact) and summed in the single-GPU order;
+ *   - rank r evaluates g = f - tau c_norm P^T T on ITS z-units (n_z_units of z_unit_slices slices of the lower half volume,
+ *     with their mirror images; of the whole volume without mirror symmetry) and the slabs are broadcast from their owners;
+ *   - the TV step, the grid transfers and the step bound run replicated: deterministic kernels on identical inputs.
+ * Every residual value and every voxel of g is computed by exactly one rank with the arithmetic of the single-GPU launch, so
+ * the result on every rank is BIT FOR BIT cbct_fbs_reconstruct's.  The two collectives are the caller's (NCCL through
+ * torch.distributed in the Python binding): callbacks on caller-owned DEVICE memory of the handle, to be ordered on
+ * `cuda_stream` (enqueue on it, or synchronise it before and after); they return 0 on success.
+ * Only CBCT_BACKPROJECTOR_EXACT.  Not exercised on more than one GPU in this repository's CI (one-GPU boxes): covered by a
+ * two-rank emulation on one GPU against the single-GPU result and by CPU tests of the partition. */
+typedef struct cbct_comm {
+    int rank, world;
+    void *ctx;
+    int (*broadcast)(void *ctx, void *d_buf, unsigned long long bytes, int root, void *cuda_stream);    /* in place */
+    int (*allreduce_sum_f64)(void *ctx, double *d_buf, unsigned long long n, void *cuda_stream);        /* in place */
+} cbct_comm;
+
+/* Balanced contiguous split of n_units over `world` ranks: [*lo, *hi) for `rank` (the first n_units % world ranks take one
+ * unit more).  Pure host arithmetic: needs no device. */
+cbct_status cbct_shard_range(int n_units, int world, int rank, int *lo, int *hi);
+/* The units a level's projectors are sharded in (any pointer may be NULL). */
+cbct_status cbct_shard_units(const cbct_geometry *g, int level, int *n_base_views, int *n_z_units, int *z_unit_slices);
+cbct_status cbct_fbs_reconstruct_sharded(const cbct_geometry *g, const cbct_comm *comm, const float *d_proj_y,
+                                         float *d_vol_inout, const cbct_fbs_params *params, cbct_fbs_report *report,
+                                         void *cuda_stream);
+
 /* Kernel launches issued by this handle since create (for the bench's gpu_launches). */
 unsigned long long cbct_launch_count(const cbct_geometry *g);
 

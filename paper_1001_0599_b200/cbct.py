@@ -32,7 +32,8 @@ EXPORTS = [
     "cbct_forward_project", "cbct_back_project", "cbct_back_project_eq6", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
     "cbct_quality_metrics",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
-    "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_launch_count",
+    "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_fbs_reconstruct_sharded", "cbct_shard_range",
+    "cbct_shard_units", "cbct_launch_count",
     "cbct_set_stage_timing", "cbct_get_stage_ms", "cbct_gather_ceiling", "cbct_last_error", "cbct_version",
 ]
 
@@ -74,6 +75,15 @@ class _FbsReport(C.Structure):
     _fields_ = [("n_iters_total", C.c_int), ("objective", C.POINTER(C.c_double)),
                 ("step_abs", C.POINTER(C.c_double)), ("iters_done", C.POINTER(C.c_int)), ("inner_total", C.c_int), ("trials_total", C.c_int),
                 ("ms_total", C.c_float)]
+
+
+_BCAST_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_int, C.c_void_p)
+_ALLRED_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_ulonglong, C.c_void_p)
+
+
+class _Comm(C.Structure):
+    _fields_ = [("rank", C.c_int), ("world", C.c_int), ("ctx", C.c_void_p), ("broadcast", _BCAST_FN),
+                ("allreduce_sum_f64", _ALLRED_FN)]
 
 
 @dataclass
@@ -132,6 +142,9 @@ def load_library():
     lib.cbct_prolong_volume.argtypes = [vp, ip, vp, vp, vp]
     lib.cbct_fbs_reconstruct.argtypes = [vp, vp, vp, C.POINTER(_FbsParams), C.POINTER(_FbsReport), vp]
     lib.cbct_fbs_reconstruct_host.argtypes = [vp, vp, vp, C.POINTER(_FbsParams), C.POINTER(_FbsReport), vp]
+    lib.cbct_fbs_reconstruct_sharded.argtypes = [vp, C.POINTER(_Comm), vp, vp, C.POINTER(_FbsParams), C.POINTER(_FbsReport), vp]
+    lib.cbct_shard_range.argtypes = [ip, ip, ip, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    lib.cbct_shard_units.argtypes = [vp, ip, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     lib.cbct_launch_count.argtypes = [vp]
     lib.cbct_launch_count.restype = C.c_ulonglong
     lib.cbct_set_stage_timing.argtypes = [vp, ip]
@@ -364,6 +377,23 @@ class Geometry:
                                                         C.byref(r), _stream_ptr(stream)))
         return self._fbs_report(r, keep)
 
+    def fbs_reconstruct_sharded(self, comm: "Comm", proj_y, vol_inout, fbs, use_initial: bool = False,
+                                objective: bool = True, stream=None) -> FbsReport:
+        """cbct_fbs_reconstruct_sharded: this rank's part of a reconstruction sharded over comm.world GPUs."""
+        p, r, keep = self._fbs_args(fbs, use_initial, objective)
+        _check(load_library().cbct_fbs_reconstruct_sharded(self._h, C.byref(comm.struct), _dev(proj_y, self._nray(0), "proj_y"),
+                                                           _dev(vol_inout, self._nvox(0), "vol_inout"), C.byref(p),
+                                                           C.byref(r), _stream_ptr(stream)))
+        if comm.error is not None:
+            raise comm.error
+        return self._fbs_report(r, keep)
+
+    def shard_units(self, level: int = 0):
+        """(base views, z-units, slices per z-unit) the level's projectors are sharded in."""
+        a, b, c = C.c_int(0), C.c_int(0), C.c_int(0)
+        _check(load_library().cbct_shard_units(self._h, level, C.byref(a), C.byref(b), C.byref(c)))
+        return a.value, b.value, c.value
+
     # profiling --------------------------------------------------------------
     def set_stage_timing(self, enable: bool):
         _check(load_library().cbct_set_stage_timing(self._h, int(bool(enable))))
@@ -376,6 +406,74 @@ class Geometry:
         calls = (C.c_ulonglong * len(self.STAGES))()
         _check(load_library().cbct_get_stage_ms(self._h, ms, calls))
         return {k: (float(m), int(c)) for k, m, c in zip(self.STAGES, ms, calls)}
+
+
+def shard_range(n_units: int, world: int, rank: int):
+    """cbct_shard_range: the contiguous share [lo, hi) of `rank` (pure host arithmetic, no device needed)."""
+    lo, hi = C.c_int(0), C.c_int(0)
+    _check(load_library().cbct_shard_range(n_units, world, rank, C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+class _DevBytes:
+    """A window of device memory as a __cuda_array_interface__ object (zero copy into a torch tensor)."""
+
+    def __init__(self, ptr: int, n: int, typestr: str):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": typestr, "data": (ptr, False), "version": 2}
+
+
+def device_window(ptr: int, n: int, typestr: str = "|u1"):
+    import torch
+    return torch.as_tensor(_DevBytes(ptr, n, typestr), device="cuda")
+
+
+class Comm:
+    """cbct_comm: the two collectives of cbct_fbs_reconstruct_sharded as Python callables on torch tensors that alias the
+    handle's device memory.  `broadcast(tensor_u8, root)` and `allreduce_sum(tensor_f64)` work in place and must be ordered
+    on the torch stream current when they are called (the binding makes the library's stream current around each call)."""
+
+    def __init__(self, rank: int, world: int, broadcast, allreduce_sum):
+        import torch
+        self.error = None
+
+        def on_stream(stream_ptr):
+            return torch.cuda.stream(torch.cuda.ExternalStream(stream_ptr or 0))
+
+        def bcast(_ctx, ptr, nbytes, root, stream_ptr):
+            try:
+                with on_stream(stream_ptr):
+                    broadcast(device_window(ptr, nbytes), root)
+                return 0
+            except Exception as e:      # nothing may propagate through the C frames
+                self.error = e
+                return 1
+
+        def allred(_ctx, ptr, n, stream_ptr):
+            try:
+                with on_stream(stream_ptr):
+                    allreduce_sum(device_window(ptr, n, "<f8"))
+                return 0
+            except Exception as e:
+                self.error = e
+                return 1
+
+        self._keep = (_BCAST_FN(bcast), _ALLRED_FN(allred))
+        self.struct = _Comm(rank, world, None, self._keep[0], self._keep[1])
+        self.rank, self.world = rank, world
+
+
+def torch_distributed_comm(group=None) -> Comm:
+    """The communicator over a torch.distributed process group (backend nccl: one process per GPU)."""
+    import torch.distributed as dist
+    ranks = dist.get_process_group_ranks(group) if group is not None else list(range(dist.get_world_size()))
+
+    def broadcast(t, root):
+        dist.broadcast(t, src=ranks[root], group=group)
+
+    def allreduce_sum(t):
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+
+    return Comm(dist.get_rank(group), dist.get_world_size(group), broadcast, allreduce_sum)
 
 
 def gather_ceiling(buf, variant: int, reuse: int = 1, iters: int = 64, stream=None):

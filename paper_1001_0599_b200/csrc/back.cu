@@ -138,7 +138,7 @@ __device__ __forceinline__ void gather_column(float (&acc)[KT][R * M], const flo
 template <int R, int M, int KT>
 __global__ void __launch_bounds__(32 * BK_BX, 3)
 back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
-            const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
+            const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out, int z_off)
 {
     const int lane = threadIdx.x;
     const int i = blockIdx.x * BK_BX + threadIdx.y;
@@ -150,7 +150,7 @@ back_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__r
     float zl[KT];                                    // lower z-plane of the voxel relative to the source plane (index units)
 #pragma unroll
     for (int t = 0; t < KT; ++t) {
-        kv[t] = blockIdx.z * (32 * KT) + lane + 32 * t;
+        kv[t] = (blockIdx.z + z_off) * (32 * KT) + lane + 32 * t;       // z_off: first z-unit of a sharded launch
         zl[t] = (float)(min(kv[t], nzh - 1) - P.cz) - P.sz;      // a ragged tail recomputes the last voxel, not stored
     }
     // the R quarter-turn images of the voxel: (i,j), (n-1-j, i), (n-1-i, n-1-j), (j, n-1-i)
@@ -231,7 +231,7 @@ constexpr int BK_MAXC = 5, BK_LIST = 32 * BK_MAXC;      // list entries per warp
 template <int R, int M, int KT>
 __global__ void __launch_bounds__(32 * BK_BX, 3)
 back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
-                 const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out)
+                 const float *__restrict__ TL, const float *__restrict__ f, float coef, float *__restrict__ out, int z_off)
 {
     __shared__ float4 s_list[BK_BX][2][BK_LIST];
     constexpr int LCAP = BK_LIST / R;                 // per image: (32 / R) base views x BK_MAXC
@@ -246,7 +246,7 @@ back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC
     float zl[KT];
 #pragma unroll
     for (int t = 0; t < KT; ++t) {
-        kv[t] = blockIdx.z * (32 * KT) + lane + 32 * t;
+        kv[t] = (blockIdx.z + z_off) * (32 * KT) + lane + 32 * t;       // z_off: first z-unit of a sharded launch
         zl[t] = (float)(min(kv[t], nzh - 1) - P.cz) - P.sz;
     }
     int vi[R], vj[R];
@@ -352,26 +352,38 @@ back_list_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC
 
 template <int R, int M, int KT>
 static void launch_back_kernel(const LevelParams &P, const Level &L, const float *src, const float *d_f, float coef,
-                               float *d_out, cudaStream_t st)
+                               float *d_out, cudaStream_t st, const Shard *sh)
 {
     const int nzh = P.nz / M, ni = R == 4 ? P.nx / 2 : P.nx, nj = R == 4 ? P.ny / 2 : P.ny;
     const int kchunk = 32 * KT;
     dim3 b(32, BK_BX), gr((ni + BK_BX - 1) / BK_BX, nj, (nzh + kchunk - 1) / kchunk);
-    if (L.back_maxc <= BK_MAXC) back_list_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
-    else back_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out);
+    int z_off = 0;
+    if (sh) { z_off = sh->zu_lo; gr.z = sh->zu_hi - sh->zu_lo; if (gr.z == 0) return; }
+    if (L.back_maxc <= BK_MAXC) back_list_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out, z_off);
+    else back_kernel<R, M, KT><<<gr, b, 0, st>>>(P, L.d_rayu, L.d_view, src, d_f, coef, d_out, z_off);
 }
+
+// voxels per thread along z: two at 80 registers measured best at 256^3 (1 and 4 voxels, 64 / 100+ registers: 3-50 % slower)
+static int back_kt(const LevelParams &P) { return P.nz / P.nmir >= 64 ? 2 : 1; }
 
 template <int R, int M>
 static void launch_back_rm(const LevelParams &P, const Level &L, const float *src, const float *d_f, float coef,
-                           float *d_out, cudaStream_t st)
+                           float *d_out, cudaStream_t st, const Shard *sh)
 {
-    // two voxels per thread at 80 registers measured best at 256^3 (1 and 4 voxels, 64 / 100+ registers: 3-50 % slower)
-    if (P.nz / M >= 64) launch_back_kernel<R, M, 2>(P, L, src, d_f, coef, d_out, st);
-    else launch_back_kernel<R, M, 1>(P, L, src, d_f, coef, d_out, st);
+    if (back_kt(P) == 2) launch_back_kernel<R, M, 2>(P, L, src, d_f, coef, d_out, st, sh);
+    else launch_back_kernel<R, M, 1>(P, L, src, d_f, coef, d_out, st, sh);
+}
+
+// The z-unit of a sharded back-projection: the slices one block of the level's kernel covers along z.
+int back_zunit(const Level &L) { return L.bt.ok ? 32 : 32 * back_kt(L.p); }
+int back_nzunits(const Level &L)
+{
+    const int nzh = L.p.nz / L.p.nmir, u = back_zunit(L);
+    return (nzh + u - 1) / u;
 }
 
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
-                        const float *d_f, float coef, float *d_out, cudaStream_t st)
+                        const float *d_f, float coef, float *d_out, cudaStream_t st, const Shard *sh)
 {
     const LevelParams &P = L.p;
     const float *src = d_in;
@@ -386,11 +398,12 @@ cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_i
         src = L.d_T;
     }
     StageTimer t(g, st, ST_BACK);
-    if (L.bt.ok) return launch_back_tma(g, L, d_f, coef, d_out, st);      // src is L.d_T on this path (below)
-    if (P.nsym == 4 && P.nmir == 2) launch_back_rm<4, 2>(P, L, src, d_f, coef, d_out, st);
-    else if (P.nsym == 4) launch_back_rm<4, 1>(P, L, src, d_f, coef, d_out, st);
-    else if (P.nmir == 2) launch_back_rm<1, 2>(P, L, src, d_f, coef, d_out, st);
-    else launch_back_rm<1, 1>(P, L, src, d_f, coef, d_out, st);
+    if (sh && (sh->zu_lo < 0 || sh->zu_hi > back_nzunits(L) || sh->zu_lo > sh->zu_hi)) return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_back: bad shard");
+    if (L.bt.ok) return launch_back_tma(g, L, d_f, coef, d_out, st, sh);      // src is L.d_T on this path (below)
+    if (P.nsym == 4 && P.nmir == 2) launch_back_rm<4, 2>(P, L, src, d_f, coef, d_out, st, sh);
+    else if (P.nsym == 4) launch_back_rm<4, 1>(P, L, src, d_f, coef, d_out, st, sh);
+    else if (P.nmir == 2) launch_back_rm<1, 2>(P, L, src, d_f, coef, d_out, st, sh);
+    else launch_back_rm<1, 1>(P, L, src, d_f, coef, d_out, st, sh);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }

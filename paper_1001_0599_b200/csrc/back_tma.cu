@@ -161,7 +161,7 @@ template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
 __global__ void __launch_bounds__((BI * BJ / CPW + 1) * 32, MINB)
 back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const BtParams Q,
                 const RayU *__restrict__ rayu, const ViewC *__restrict__ views, const float *__restrict__ f, float coef,
-                float *__restrict__ out, unsigned int *__restrict__ errflag)
+                float *__restrict__ out, unsigned int *__restrict__ errflag, int kb_top)
 {
     constexpr int NIJ = BI * BJ, NW = NIJ / CPW;      // voxel columns of the brick, consumer warps
     constexpr int SPR = 4 / CPW;                      // stages per list round: 32 lanes = SPR stages x CPW columns x 8 candidates
@@ -169,7 +169,7 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
     extern __shared__ __align__(1024) char smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // the slices nearest to the central plane first: the truncated bottom bricks are the cheap ones and fill the tail
-    const int i0 = blockIdx.x * BI, j0 = blockIdx.y * BJ, k0 = (gridDim.z - 1 - blockIdx.z) * 32;
+    const int i0 = blockIdx.x * BI, j0 = blockIdx.y * BJ, k0 = (kb_top - 1 - blockIdx.z) * 32;     // kb_top: one past the last 32-slice unit of this launch
     const int ni = P.nx / 2, nj = P.ny / 2, n1 = P.nx - 1;
     const int n_stages = 4 * P.nbase;
 
@@ -429,7 +429,8 @@ EncodeTiledFn encode_tiled_fn()
 }
 
 template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
-cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out, unsigned int *errflag, cudaStream_t st)
+cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out, unsigned int *errflag, cudaStream_t st,
+                      const Shard *sh)
 {
     const LevelParams &P = L.p;
     const BtPlan &B = L.bt;
@@ -442,7 +443,9 @@ cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out
     }
     const int ni = P.nx / 2, nj = P.ny / 2;
     dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 31) / 32), b((BI * BJ / CPW + 1) * 32);
-    kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag);
+    int kb_top = gr.z;
+    if (sh) { kb_top = sh->zu_hi; gr.z = sh->zu_hi - sh->zu_lo; if (gr.z == 0) return CBCT_OK; }
+    kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag, kb_top);
     return CBCT_OK;
 }
 
@@ -550,14 +553,15 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     return CBCT_OK;
 }
 
-cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st)
+cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st,
+                            const Shard *sh)
 {
     const BtPlan &B = L.bt;
     cbct_status s = CBCT_ERR_INVALID_ARG;
 #define BT_CASE(NS, TPV)                                                                                         \
     if (B.NSLOT == NS && B.TP == TPV)                                                                            \
-        s = B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2>(L, d_f, coef, d_out, g->d_errflag, st)                   \
-                        : bt_launch<4, 4, 1, NS, TPV, 1>(L, d_f, coef, d_out, g->d_errflag, st);
+        s = B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2>(L, d_f, coef, d_out, g->d_errflag, st, sh)               \
+                        : bt_launch<4, 4, 1, NS, TPV, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh);
     BT_CASE(2, 1) BT_CASE(3, 1) BT_CASE(4, 1) BT_CASE(2, 2) BT_CASE(3, 2) BT_CASE(4, 2)
 #undef BT_CASE
     if (s != CBCT_OK) return s == CBCT_ERR_INVALID_ARG ? cbct_fail(s, "launch_back_tma: no kernel for this plan") : s;

@@ -187,21 +187,34 @@ static inline const Level *get_level(const cbct_geometry *g, int level)
     return &g->levels[level];
 }
 
+// A rank's share of the two projectors in a sharded reconstruction (fbs.cu): base views [base_lo, base_hi) of the forward
+// projector, z-units [zu_lo, zu_hi) of the back-projector (back_zunit() slices of the lower half volume each -- of the whole
+// volume without mirror symmetry -- with their mirror images).  NULL = everything, with the fused reduction.
+struct Shard {
+    int base_lo, base_hi, zu_lo, zu_hi;
+};
+int back_zunit(const Level &L);
+int back_nzunits(const Level &L);
+
 // internal launchers (asynchronous on `st`)
 // forward.cu : mode 0: out = P vol (plain layout).
 //              mode 1: out = L * (P vol - y) in the d_T layout, *d_sum_sq = sum (P vol - y)^2.
 //              mode 2: out = L * (P vol) in the d_T layout.
 //              mode 3: *d_sum_sq = number of (ray, voxel) pairs, no volume read
 //              mode 4: out = P vol - y (plain layout), *d_sum_sq = sum (P vol - y)^2
+//              With a shard (modes 1, 2): only its base views; mode 1 then leaves the blocks' partial sums of (P vol - y)^2
+//              in g->d_partials row 0 at their index in the full launch (no sum is formed).
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
-                           float *d_out, int mode, double *d_sum_sq, cudaStream_t st);
+                           float *d_out, int mode, double *d_sum_sq, cudaStream_t st, const Shard *sh = nullptr);
 // back.cu : scaled != 0: d_in already holds L*T in the d_T layout; else plain layout, unscaled.
 //           out = f - coef * P^T in (f may be NULL: out = P^T in)
+//           With a shard: only the voxels of its z-units are written.
 cbct_status launch_back(const cbct_geometry *g, const Level &L, const float *d_in, int scaled,
-                        const float *d_f, float coef, float *d_out, cudaStream_t st);
+                        const float *d_f, float coef, float *d_out, cudaStream_t st, const Shard *sh = nullptr);
 // back_tma.cu : plan of the TMA back-projector for a level (create time; needs L.d_T), and its launch (input = L.d_T)
 cbct_status bt_plan_level(const cbct_geometry *g, Level &L);
-cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st);
+cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float *d_f, float coef, float *d_out, cudaStream_t st,
+                            const Shard *sh = nullptr);
 // back_eq6.cu : out = f - coef * b6(T) with T in the plain [view][row][column] layout (f may be NULL: out = b6(T))
 cbct_status launch_back_eq6(const cbct_geometry *g, const Level &L, const float *d_T, const float *d_f, float coef,
                             float *d_out, cudaStream_t st);

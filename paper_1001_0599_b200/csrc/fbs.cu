@@ -9,6 +9,7 @@
 // Every stage is a kernel of this library; the host only sequences launches.
 #include <math.h>
 #include "cbct_internal.cuh"
+#include "reduce.cuh"
 
 namespace {
 
@@ -69,9 +70,75 @@ cbct_status check_params(const cbct_geometry *g, const cbct_fbs_params *p)
     return CBCT_OK;
 }
 
-// The whole reconstruction on device buffers (level-0 sized d_y, d_vol).
+// ---- NEXT-4: the two projectors sharded by output ownership ------------------------------------
+// Every rank holds the whole volume and the whole data.  A rank computes the residual of ITS base views (with their
+// quarter-turn partners) and g = f - tau c_norm P^T T on ITS z-units (with their mirror images); the residual chunks and
+// the slabs of g are then broadcast from their owners, and the blocks' partial sums of T^2 are added across ranks (each
+// slot is written by one rank, the others hold 0: exact) and summed in the single-GPU order.  Every element is computed
+// by exactly one rank with the arithmetic of the single-GPU launch, so the volume is bit for bit the single-GPU one; the TV
+// step, the transfers and the step bound run replicated (deterministic: every rank gets the same bits).
+void shard_range(int n, int world, int rank, int *lo, int *hi)
+{
+    const int q = n / world, r = n % world;             // the first r ranks take one unit more
+    *lo = rank * q + (rank < r ? rank : r);
+    *hi = *lo + q + (rank < r ? 1 : 0);
+}
+
+#define CBCT_COMM(expr)                                                                                  \
+    do {                                                                                                 \
+        if ((expr) != 0) return cbct_fail(CBCT_ERR_CUDA, "communicator callback failed: %s", #expr);     \
+    } while (0)
+
+// T = L inv_dd (P f - y) on every rank, and sum T^2 / (L inv_dd)^2 in *d_sum_sq
+cbct_status sharded_forward(const cbct_geometry *g, const Level &L, const cbct_comm *cm, const float *f, const float *y,
+                            double *d_sum_sq, cudaStream_t st)
+{
+    const LevelParams &P = L.p;
+    cbct_status s;
+    Shard sh = {0, 0, 0, 0};
+    shard_range(P.nbase, cm->world, cm->rank, &sh.base_lo, &sh.base_hi);
+    const size_t nblk = (size_t)((P.nu + 7) / 8) * P.nbase * ((P.nv / P.nmir + 31) / 32);      // forward.cu's full grid
+    if (nblk > (size_t)g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
+    CBCT_CUDA(cudaMemsetAsync(g->d_partials, 0, nblk * sizeof(double), st));
+    if ((s = launch_forward(g, L, f, y, L.d_T, 1, nullptr, st, &sh)) != CBCT_OK) return s;
+    const size_t per_base = (size_t)P.nu * P.nv * P.nsym * sizeof(float);                       // one base view of the stack
+    for (int r = 0; r < cm->world; ++r) {
+        int lo, hi;
+        shard_range(P.nbase, cm->world, r, &lo, &hi);
+        if (hi > lo) CBCT_COMM(cm->broadcast(cm->ctx, (char *)L.d_T + (size_t)lo * per_base, (unsigned long long)(hi - lo) * per_base, r, st));
+    }
+    CBCT_COMM(cm->allreduce_sum_f64(cm->ctx, g->d_partials, (unsigned long long)nblk, st));
+    finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
+    CBCT_LAUNCH_CHECK(g);
+    return CBCT_OK;
+}
+
+// d_g = f - coef P^T T on every rank
+cbct_status sharded_back(const cbct_geometry *g, const Level &L, const cbct_comm *cm, const float *f, float coef, float *d_g,
+                         cudaStream_t st)
+{
+    const LevelParams &P = L.p;
+    cbct_status s;
+    const int nzu = back_nzunits(L), unit = back_zunit(L), nzh = P.nz / P.nmir;
+    Shard sh = {0, 0, 0, 0};
+    shard_range(nzu, cm->world, cm->rank, &sh.zu_lo, &sh.zu_hi);
+    if ((s = launch_back(g, L, L.d_T, 1, f, coef, d_g, st, &sh)) != CBCT_OK) return s;
+    const size_t slice = (size_t)P.nx * P.ny * sizeof(float);
+    for (int r = 0; r < cm->world; ++r) {
+        int lo, hi;
+        shard_range(nzu, cm->world, r, &lo, &hi);
+        const int k_lo = lo * unit, k_hi = hi * unit < nzh ? hi * unit : nzh;
+        if (k_hi <= k_lo) continue;
+        CBCT_COMM(cm->broadcast(cm->ctx, (char *)d_g + (size_t)k_lo * slice, (unsigned long long)(k_hi - k_lo) * slice, r, st));
+        if (P.nmir == 2)        // the mirror images of those slices
+            CBCT_COMM(cm->broadcast(cm->ctx, (char *)d_g + (size_t)(P.nz - k_hi) * slice, (unsigned long long)(k_hi - k_lo) * slice, r, st));
+    }
+    return CBCT_OK;
+}
+
+// The whole reconstruction on device buffers (level-0 sized d_y, d_vol).  cm == NULL: one GPU.
 cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, const cbct_fbs_params *p,
-                       cbct_fbs_report *rep, cudaStream_t st)
+                       cbct_fbs_report *rep, cudaStream_t st, const cbct_comm *cm = nullptr)
 {
     cbct_status s;
     const int nl = p->n_levels;
@@ -129,7 +196,9 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
         for (int it = 0; it < n_it; ++it, ++done) {
             if (p->conv_tol > 0.0)      // keep the volume that enters the iteration for the convergence test
                 CBCT_CUDA(cudaMemcpyAsync(L.d_prev, f, L.nvox * sizeof(float), cudaMemcpyDeviceToDevice, st));
-            if (!fwd_queued) {
+            if (cm) {
+                if ((s = sharded_forward(g, L, cm, f, y, obj_slot(done) + 1, st)) != CBCT_OK) return s;
+            } else if (!fwd_queued) {
                 if ((s = launch_forward(g, L, f, y, L.d_T, eq6 ? 4 : 1, obj_slot(done) + 1, st)) != CBCT_OK) return s;
             }
             fwd_queued = false;
@@ -137,7 +206,8 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
                 if ((s = launch_tv_energy(g, L, f, p->tv.eps_delta, obj_slot(done), st)) != CBCT_OK) return s;
             }
             {
-                if (eq6) s = launch_back_eq6(g, L, L.d_T, f, (float)(tau * c_norm), L.d_g, st);
+                if (cm) s = sharded_back(g, L, cm, f, (float)(tau * c_norm), L.d_g, st);
+                else if (eq6) s = launch_back_eq6(g, L, L.d_T, f, (float)(tau * c_norm), L.d_g, st);
                 else s = launch_back(g, L, L.d_T, 1, f, (float)(tau * c_norm), L.d_g, st);
                 if (s != CBCT_OK) return s;
             }
@@ -146,7 +216,7 @@ cbct_status fbs_device(const cbct_geometry *g, const float *d_y, float *d_vol, c
                 ForwardAhead fa = {g, &L, f, y, eq6 ? 4 : 1, obj_slot(done + 1) + 1, st};
                 TvAhead ah = {forward_ahead, &fa, false};
                 // (host-sequenced Armijo loop only: the cooperative kernel has no host wait to hide)
-                const bool look_ahead = g->host_armijo && !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
+                const bool look_ahead = !cm && g->host_armijo && !want_obj && p->conv_tol == 0.0 && it + 1 < n_it;
                 if ((s = run_tv_prox(g, L, L.d_g, f, w, p->nonneg, p->tv, &tr, false, st, look_ahead ? &ah : nullptr)) != CBCT_OK) return s;
                 fwd_queued = look_ahead && ah.valid;
                 inner_total += tr.inner_iters;
@@ -207,6 +277,38 @@ extern "C" cbct_status cbct_fbs_reconstruct(const cbct_geometry *g, const float 
     if (s != CBCT_OK) return s;
     if (!d_proj_y || !d_vol_inout) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct: NULL buffer");
     return fbs_device(g, d_proj_y, d_vol_inout, params, report, (cudaStream_t)cuda_stream);
+}
+
+extern "C" cbct_status cbct_shard_range(int n_units, int world, int rank, int *lo, int *hi)
+{
+    if (n_units < 0 || world < 1 || rank < 0 || rank >= world || !lo || !hi)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_shard_range: bad argument");
+    shard_range(n_units, world, rank, lo, hi);
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_shard_units(const cbct_geometry *g, int level, int *n_base_views, int *n_z_units, int *z_unit_slices)
+{
+    const Level *L = get_level(g, level);
+    if (!L) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_shard_units: bad handle or level");
+    if (n_base_views) *n_base_views = L->p.nbase;
+    if (n_z_units) *n_z_units = back_nzunits(*L);
+    if (z_unit_slices) *z_unit_slices = back_zunit(*L);
+    return CBCT_OK;
+}
+
+extern "C" cbct_status cbct_fbs_reconstruct_sharded(const cbct_geometry *g, const cbct_comm *comm, const float *d_proj_y,
+                                                    float *d_vol_inout, const cbct_fbs_params *params,
+                                                    cbct_fbs_report *report, void *cuda_stream)
+{
+    cbct_status s = check_params(g, params);
+    if (s != CBCT_OK) return s;
+    if (!d_proj_y || !d_vol_inout) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct_sharded: NULL buffer");
+    if (!comm || comm->world < 1 || comm->rank < 0 || comm->rank >= comm->world || !comm->broadcast || !comm->allreduce_sum_f64)
+        return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_fbs_reconstruct_sharded: bad communicator");
+    if (params->backprojector != CBCT_BACKPROJECTOR_EXACT)
+        return cbct_fail(CBCT_ERR_UNSUPPORTED, "cbct_fbs_reconstruct_sharded: only the exact-transpose back-projector is sharded");
+    return fbs_device(g, d_proj_y, d_vol_inout, params, report, (cudaStream_t)cuda_stream, comm);
 }
 
 extern "C" cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_proj_y,

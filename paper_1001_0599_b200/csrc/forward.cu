@@ -105,7 +105,7 @@ template <int R, int M, int MODE>
 __global__ void __launch_bounds__(FWD_BV *FWD_BU, FWD_MINB)
 forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
-               unsigned int *__restrict__ counter, double *__restrict__ sum_out)
+               unsigned int *__restrict__ counter, double *__restrict__ sum_out, int a_off)
 {
     typedef typename StageCell<M>::type cell;
     const cell *__restrict__ stage = reinterpret_cast<const cell *>(stage_v);
@@ -114,7 +114,7 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
     // staged copy for every view, which stays in L2 (with the view slowest, every view re-reads the whole copy)
     const int iv = blockIdx.z * FWD_BV + threadIdx.x;
     const int iu = blockIdx.x * FWD_BU + threadIdx.y;
-    const int a = blockIdx.y;                  // base view
+    const int a = blockIdx.y + a_off;          // base view (a_off: first base view of a sharded launch)
     const int nvh = M == 2 ? P.nv / 2 : P.nv;  // rows this grid walks; the others are their mirrors
     double sq = 0.0;
     if (iu < P.nu && iv < nvh) {
@@ -243,7 +243,8 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
     if (MODE == 1 || MODE == 4) {        // E2 numerator: sum of squared residuals, second stage fused (reduce.cuh)
         double s[1];
         s[0] = block_sum(sq, slot);
-        publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
+        if (counter) publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
+        else publish_only<1>(s, 1, partials, stride, ((unsigned)blockIdx.z * P.nbase + a) * gridDim.x + blockIdx.x);   // sharded launch
     }
 }
 
@@ -290,20 +291,23 @@ count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double 
 
 template <int R, int M>
 static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode,
-                                const void *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq)
+                                const void *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq,
+                                int a_off, bool fused_sum)
 {
-    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
-    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr);
+    unsigned int *ctr = fused_sum ? g->d_counter : nullptr;
+    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
+    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
     else if (mode == 4) forward_kernel<R, M, 4><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
-                                                                 g->d_counter, d_sum_sq);
+                                                                 ctr, d_sum_sq, a_off);
     else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
-                                                   g->d_counter, d_sum_sq);
+                                                   ctr, d_sum_sq, a_off);
 }
 
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
-                           float *d_out, int mode, double *d_sum_sq, cudaStream_t st)
+                           float *d_out, int mode, double *d_sum_sq, cudaStream_t st, const Shard *sh)
 {
     const LevelParams &P = L.p;
+    if (sh && mode != 1 && mode != 2) return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_forward: a sharded launch writes the residual stack");
     dim3 b(FWD_BX, FWD_BY);
     if (mode == 3) {
         dim3 gr((P.nu + FWD_BX - 1) / FWD_BX, (P.nv + FWD_BY - 1) / FWD_BY, P.np);
@@ -330,15 +334,23 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     }
     b = dim3(FWD_BV, FWD_BU);
     dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, P.nbase, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
-    const size_t nblk = (size_t)gr.x * gr.y * gr.z;
+    const size_t nblk = (size_t)gr.x * gr.y * gr.z;             // of the full launch: the numbering of the partial sums
     if ((mode == 1 || mode == 4) && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
+    int a_off = 0;
+    if (sh) {
+        if (sh->base_lo < 0 || sh->base_hi > P.nbase || sh->base_lo > sh->base_hi) return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_forward: bad shard");
+        a_off = sh->base_lo;
+        gr.y = sh->base_hi - sh->base_lo;
+        if (gr.y == 0) return CBCT_OK;
+    }
     {
         StageTimer t(g, st, ST_FORWARD);
-        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
-        else if (P.nsym == 4) launch_forward_mode<4, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
-        else if (P.nmir == 2) launch_forward_mode<1, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
-        else launch_forward_mode<1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq);
+        const bool fused = sh == nullptr;
+        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nsym == 4) launch_forward_mode<4, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nmir == 2) launch_forward_mode<1, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else launch_forward_mode<1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
         CBCT_LAUNCH_CHECK(g);
     }
     return CBCT_OK;

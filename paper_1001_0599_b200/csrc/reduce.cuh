@@ -108,3 +108,17 @@ __device__ __forceinline__ void publish_and_finalize(const double (&vals)[ROWS],
     }
     if (tid == 0) *counter = 0u;
 }
+
+// Sharded launches (fbs.cu, cbct_fbs_reconstruct_sharded): a block only publishes its partial sums at its index in the
+// FULL launch's numbering; the sums are added by finalize_sums_kernel once every rank's partials are in -- in the same
+// order as publish_and_finalize's last block (thread t adds elements t, t + 256, ...: both run 256 threads).
+template <int ROWS>
+__device__ __forceinline__ void publish_only(const double (&vals)[ROWS], int rows, double *partials, int stride, unsigned int blk)
+{
+    const int tid = (threadIdx.z * blockDim.y + threadIdx.y) * blockDim.x + threadIdx.x;
+    if (tid == 0) {
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r)
+            if (r < rows) partials[(size_t)r * stride + blk] = vals[r];
+    }
+}
