@@ -8,6 +8,7 @@
 // value (BC_REFLECT) (L161).  div is the exact negative transpose (backward differences,
 // p_{-1} = 0).  Per-voxel terms are fp32, sums are fp64 in a fixed order (reduce.cuh).
 #include <math.h>
+#include <stdlib.h>
 #include <cooperative_groups.h>
 #include "cbct_internal.cuh"
 #include "reduce.cuh"
@@ -235,23 +236,6 @@ __device__ __forceinline__ void tv_grad_tile(const TvDims &D, const TvTile &T, c
     }
 }
 
-template <bool FIRST>
-__global__ void __launch_bounds__(32 * TV_WPB)
-tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ g, float beta, float delta2,
-               float *__restrict__ d_out, int zc, double *__restrict__ partials, int stride,
-               unsigned int *__restrict__ counter, double *__restrict__ out)
-{
-    __shared__ double slot[32];
-    const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
-    double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
-    tv_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
-    double s[3];
-    s[0] = block_sum(e_tv, slot);
-    s[1] = block_sum(e_q, slot);
-    s[2] = block_sum(e_d, slot);
-    publish_and_finalize<3>(s, 3, partials, stride, counter, out, slot);
-}
-
 // Energy pass at u = f - lam*dir (TRIAL) or u = f:  out[0] = sum |grad u|_delta and, when rows == 2,
 // out[1] = sum (u-g)^2.  Same warp tiles and march; nothing but u(i+1) is exchanged between voxels.
 template <bool TRIAL>
@@ -320,7 +304,338 @@ __device__ __forceinline__ void tv_energy_tile(const TvDims &D, const TvTile &T,
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The 16-byte form of the warp tiles (volumes with nx % 4 == 0, nx >= 128 and 16-byte aligned rows): a lane owns FOUR
+// consecutive voxels of a row, so a warp tile is 128 (x) x TQ_R (y) voxels and every access is a 16-byte load or store of
+// a whole 128-byte line per quarter warp.  Same stencil, same boundary rules and the same per-voxel fp32 expressions as the
+// tiles above; what changes is the bookkeeping per voxel: one shuffle pair per FOUR voxels for u(i+1) and p_x(i-1), a
+// quarter of the load / store instructions, and the row j0-1 that supplies p_y(.,j0-1) is a register row like the others.
+// Loads run one to two slices ahead WITHOUT extra buffers: a row of slice k is dead once its own row and the row below it
+// are done, and is refilled with the same row of slice k+2 on the spot (the march is unrolled by two, the two register
+// sets swapping roles), so every load has a whole slice of arithmetic to land.
+// ---------------------------------------------------------------------------------------------------------------------
+#ifndef TQ_ROWS
+#define TQ_ROWS 4
+#endif
+constexpr int TQ_R = TQ_ROWS; // rows per warp tile
+#ifndef TQ_VOX
+#define TQ_VOX 4
+#endif
+constexpr int TQ_V = TQ_VOX;  // consecutive voxels per lane (4: 16-byte accesses, 2: 8-byte)
+constexpr int TQ_W = 32 * TQ_V;   // voxels per warp tile row
+
+struct F4 { float v[TQ_V]; };
+// The refills are volatile asm with a memory clobber: the compiler otherwise sinks them to the end of the slice (their
+// targets are dead registers either way), right in front of their first use, and the march stalls on every load.
+__device__ __forceinline__ F4 ldg4(const float *__restrict__ p)
+{
+    F4 r;
+    if constexpr (TQ_V == 4)
+        asm volatile("ld.volatile.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[TQ_V - 1]) : "l"(p) : "memory");
+    else
+        asm volatile("ld.volatile.global.v2.f32 {%0, %1}, [%2];" : "=f"(r.v[0]), "=f"(r.v[1]) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ float ldg1(const float *__restrict__ p)
+{
+    float r;
+    asm volatile("ld.volatile.global.f32 %0, [%1];" : "=f"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st4(float *__restrict__ p, const F4 &a)
+{
+    if constexpr (TQ_V == 4)
+        asm volatile("st.volatile.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]), "f"(a.v[2]), "f"(a.v[TQ_V - 1]) : "memory");
+    else
+        asm volatile("st.volatile.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]) : "memory");
+}
+
+struct TqTile {
+    int lane, k0, k1, ks;
+    bool hy, hx, xedge;        // row j0-1 / column i0-1 exists; the lane's last voxel is the last of its row
+    float xm, bz;
+    unsigned ro[TQ_R + 2];     // element offsets inside a slice of rows j0-1 .. j0+TQ_R (clamped), at the lane's first voxel
+    bool rv[TQ_R];             // voxels (i..i+3, j0+r) exist
+    float ym[TQ_R + 1];        // multiplier of the y-neighbour of rows j0-1 .. j0+TQ_R-1
+    unsigned lco;              // lanes <= TQ_R: voxel (i0-1, j0+lane)        (p_x of the column left of the tile)
+    float lym;
+    unsigned rco;              // lanes <= TQ_R: voxel (i0+128, j0-1+lane)    (u(i+1) of lane 31)
+    size_t plane;
+};
+
+// `ntz` = number of z-chunks: chunk bz holds slices [bz nz / ntz, (bz+1) nz / ntz) -- balanced, so that the host can fit the
+// tile count to the blocks resident at once (tv_tiling)
+__device__ __forceinline__ TqTile tq_tile(const TvDims &D, int ntz, int bx, int by, int bz)
+{
+    TqTile T;
+    T.lane = threadIdx.x;
+    const int i0 = bx * TQ_W, i = i0 + TQ_V * T.lane;
+    const int j0 = (by * TV_WPB + threadIdx.y) * TQ_R;
+    T.k0 = (int)(((long long)bz * D.nz) / ntz);
+    T.k1 = (int)(((long long)(bz + 1) * D.nz) / ntz);
+    T.ks = T.k0 > 0 ? T.k0 - 1 : 0;
+    T.hy = j0 > 0;
+    T.hx = i0 > 0;
+    const float bxy = D.zero_xy ? 0.0f : 1.0f;
+    T.bz = D.zero_z ? 0.0f : 1.0f;
+    T.xedge = i + TQ_V >= D.nx;
+    T.xm = T.xedge ? bxy : 1.0f;
+    const int ic = min(i, D.nx - TQ_V);
+#pragma unroll
+    for (int q = 0; q <= TQ_R + 1; ++q) T.ro[q] = (unsigned)(min(max(j0 - 1 + q, 0), D.ny - 1) * D.nx + ic);
+#pragma unroll
+    for (int r = 0; r < TQ_R; ++r) T.rv[r] = i < D.nx && j0 + r < D.ny;
+#pragma unroll
+    for (int q = 0; q <= TQ_R; ++q) T.ym[q] = (j0 + q < D.ny) ? 1.0f : bxy;        // row j0-1+q, neighbour j0+q
+    const int lj = j0 + min(T.lane, TQ_R);
+    T.lco = (unsigned)(min(lj, D.ny - 1) * D.nx + max(i0 - 1, 0));
+    T.lym = (lj + 1 < D.ny) ? 1.0f : bxy;
+    const int rj = min(max(j0 - 1 + min(T.lane, TQ_R), 0), D.ny - 1);
+    T.rco = (unsigned)(rj * D.nx + min(i0 + TQ_W, D.nx - 1));
+    T.plane = (size_t)D.nx * D.ny;
+    return T;
+}
+
+// forward differences of the four voxels of a lane: c = u(i..i+3, j, k), yv = u(., j+1, k), zn = u(., ., k+1) (already the
+// boundary value at the top of the grid), xr = u(i+4, j, k)
+__device__ __forceinline__ void tq_gradient(const TvDims &D, const F4 &c, const F4 &yv, const F4 &zn, float xr, float xm, float ym,
+                                            float delta2, F4 &gx, F4 &gy, F4 &gz, F4 &inv, F4 &nrm)
+{
+#pragma unroll
+    for (int e = 0; e + 1 < TQ_V; ++e) gx.v[e] = (c.v[e + 1] - c.v[e]) * D.ihx;
+    gx.v[TQ_V - 1] = fmaf(xr, xm, -c.v[TQ_V - 1]) * D.ihx;
+#pragma unroll
+    for (int e = 0; e < TQ_V; ++e) {
+        gy.v[e] = fmaf(yv.v[e], ym, -c.v[e]) * D.ihy;
+        gz.v[e] = (zn.v[e] - c.v[e]) * D.ihz;
+        nrm.v[e] = grad_norm(gx.v[e], gy.v[e], gz.v[e], delta2, inv.v[e]);
+    }
+}
+
+template <bool FIRST>
+__device__ __forceinline__ void tq_grad_tile(const TvDims &D, const TqTile &T, const float *__restrict__ f,
+                                             const float *__restrict__ g, float beta, float delta2,
+                                             float *__restrict__ d_out, double &e_tv, double &e_q, double &e_d)
+{
+    constexpr int R = TQ_R;
+    const size_t pl = T.plane;
+    const int ztopk = D.nz - 1, kend = min(T.k1, ztopk);
+    F4 A[R + 2], B[R + 2], G[R], pzp[R];
+    float lA, lB, rA, rB;
+    {
+        const float *p0 = f + (size_t)T.ks * pl, *p1 = f + (size_t)min(T.ks + 1, ztopk) * pl;
+#pragma unroll
+        for (int q = 0; q <= R + 1; ++q) { A[q] = ldg4(p0 + T.ro[q]); B[q] = ldg4(p1 + T.ro[q]); }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (!FIRST) G[r] = ldg4(g + (size_t)T.ks * pl + T.ro[r + 1]);
+#pragma unroll
+            for (int e = 0; e < TQ_V; ++e) { pzp[r].v[e] = 0.0f; if (FIRST) G[r].v[e] = 0.0f; }
+        }
+        lA = ldg1(p0 + T.lco); lB = ldg1(p1 + T.lco);
+        rA = ldg1(p0 + T.rco); rB = ldg1(p1 + T.rco);
+    }
+
+    auto step = [&](int k, F4 (&c)[R + 2], F4 (&n)[R + 2], float &lc, float &ln, float &rc) {
+        // refills: slice k+2, held at the last slice this tile reads (a re-read of a line just loaded, never used)
+        const float *p2 = f + (size_t)min(k + 2, kend) * pl;
+        const float *pg = g + (size_t)min(k + 1, T.k1 - 1) * pl;
+        float *pd = d_out + (size_t)k * pl;
+        const bool ztop = k + 1 >= D.nz, emit = k >= T.k0;
+        if (ztop) {                                      // the top slice of the grid: u(.,.,k+1) is the boundary value
+#pragma unroll
+            for (int q = 0; q <= R; ++q)
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) n[q].v[e] = T.bz * c[q].v[e];
+            ln = T.bz * lc;
+        }
+        float hpx = 0.0f;
+        if (T.hx) {                                      // warp-uniform: column i0-1, p_x only, its rows in lanes 0..R-1
+            float xn = 0.0f;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float v = __shfl_sync(0xffffffffu, c[r + 1].v[0], 0);
+                if (T.lane == r) xn = v;
+            }
+            const float yn = __shfl_down_sync(0xffffffffu, lc, 1);
+            const float gx = (xn - lc) * D.ihx, gy = fmaf(yn, T.lym, -lc) * D.ihy, gz = (ln - lc) * D.ihz;
+            float inv;
+            grad_norm(gx, gy, gz, delta2, inv);
+            hpx = gx * inv;
+            lc = ldg1(p2 + T.lco);
+        }
+        F4 pyp;
+#pragma unroll
+        for (int e = 0; e < TQ_V; ++e) pyp.v[e] = 0.0f;
+        float s_tv = 0.0f, s_q = 0.0f, s_d = 0.0f;
+#pragma unroll
+        for (int q = 0; q <= R; ++q) {                   // rows j0-1 (p_y only) .. j0+R-1
+            if (q == 0 && !T.hy) { c[0] = ldg4(p2 + T.ro[0]); continue; }
+            F4 gx, gy, gz, inv, nrm;
+            float xr = __shfl_down_sync(0xffffffffu, c[q].v[0], 1);
+            const float ed = __shfl_sync(0xffffffffu, rc, q);
+            if (T.lane == 31) xr = ed;
+            if (T.xedge) xr = c[q].v[TQ_V - 1];
+            tq_gradient(D, c[q], c[q + 1], n[q], xr, T.xm, T.ym[q], delta2, gx, gy, gz, inv, nrm);
+            if (q == 0) {
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) pyp.v[e] = gy.v[e] * inv.v[e];
+            } else {
+                const int r = q - 1;
+                F4 px, dd;
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) px.v[e] = gx.v[e] * inv.v[e];
+                float left = __shfl_up_sync(0xffffffffu, px.v[TQ_V - 1], 1);
+                const float edge = __shfl_sync(0xffffffffu, hpx, r);
+                if (T.lane == 0) left = edge;
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) {
+                    const float py = gy.v[e] * inv.v[e], pz = gz.v[e] * inv.v[e];
+                    const float div = (px.v[e] - (e == 0 ? left : px.v[e > 0 ? e - 1 : 0])) * D.ihx + (py - pyp.v[e]) * D.ihy +
+                                      (pz - pzp[r].v[e]) * D.ihz;
+                    const float res = FIRST ? 0.0f : c[q].v[e] - G[r].v[e];
+                    dd.v[e] = FIRST ? -div : fmaf(beta, res, -div);
+                    pyp.v[e] = py; pzp[r].v[e] = pz;
+                    if (emit && T.rv[r]) {
+                        s_tv += nrm.v[e];
+                        if (!FIRST) s_q = fmaf(res, res, s_q);
+                        s_d = fmaf(dd.v[e], dd.v[e], s_d);
+                    }
+                }
+                if (emit && T.rv[r]) st4(pd + T.ro[q], dd);
+                if (!FIRST) G[r] = ldg4(pg + T.ro[q]);
+            }
+            c[q] = ldg4(p2 + T.ro[q]);                   // this row of slice k is done with: refill it two slices ahead
+        }
+        c[R + 1] = ldg4(p2 + T.ro[R + 1]);
+        rc = ldg1(p2 + T.rco);
+        e_tv += (double)s_tv; e_d += (double)s_d;
+        if (!FIRST) e_q += (double)s_q;
+    };
+
+    for (int k = T.ks; k < T.k1; k += 2) {
+        step(k, A, B, lA, lB, rA);
+        if (k + 1 >= T.k1) break;
+        step(k + 1, B, A, lB, lA, rB);
+    }
+}
+
+// Energy pass on the 16-byte tiles: rows j0 .. j0+R-1 and the value-only row j0+R.  TRIAL: u = f - lam dir, combined one slice
+// after its two loads were issued (the raw f sits in the register row that will hold u, the raw dir in `rawd`).
 template <bool TRIAL>
+__device__ __forceinline__ void tq_energy_tile(const TvDims &D, const TqTile &T, const float *__restrict__ f,
+                                               const float *__restrict__ dir, const float *__restrict__ g, float lam,
+                                               float delta2, float *__restrict__ cand, int cand_clip, double &e_tv, double &e_q)
+{
+    constexpr int R = TQ_R;
+    const bool hasg = g != nullptr;
+    const size_t pl = T.plane;
+    const int ztopk = D.nz - 1, kend = min(T.k1, ztopk);
+    F4 A[R + 1], B[R + 1], rawd[R + 1], G[R];
+    float rA, rB, rD = 0.0f;
+    const unsigned *ro = T.ro + 1;                                        // rows j0 .. j0+R
+    const unsigned rco = __shfl_down_sync(0xffffffffu, T.rco, 1);         // lanes <= R: voxel (i0+128, j0+lane)
+    {
+        const size_t o0 = (size_t)T.k0 * pl, o1 = (size_t)min(T.k0 + 1, ztopk) * pl;
+#pragma unroll
+        for (int q = 0; q <= R; ++q) {
+            A[q] = ldg4(f + o0 + ro[q]); B[q] = ldg4(f + o1 + ro[q]);
+            if (TRIAL) {
+                const F4 d0 = ldg4(dir + o0 + ro[q]);
+                rawd[q] = ldg4(dir + o1 + ro[q]);
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) A[q].v[e] = fmaf(-lam, d0.v[e], A[q].v[e]);
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            if (hasg) G[r] = ldg4(g + o0 + ro[r]);
+            else {
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) G[r].v[e] = 0.0f;
+            }
+        }
+        rA = ldg1(f + o0 + rco); rB = ldg1(f + o1 + rco);
+        if (TRIAL) { rA = fmaf(-lam, ldg1(dir + o0 + rco), rA); rD = ldg1(dir + o1 + rco); }
+    }
+
+    auto step = [&](int k, F4 (&c)[R + 1], F4 (&n)[R + 1], float &rc, float &rn) {
+        const size_t o2 = (size_t)min(k + 2, kend) * pl, og = (size_t)min(k + 1, T.k1 - 1) * pl, ok = (size_t)k * pl;
+        const bool ztop = k + 1 >= D.nz;
+        if (TRIAL) {                                      // slice k+1: combine what the last step loaded
+#pragma unroll
+            for (int q = 0; q <= R; ++q)
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) n[q].v[e] = fmaf(-lam, rawd[q].v[e], n[q].v[e]);
+            rn = fmaf(-lam, rD, rn);
+        }
+        if (ztop) {
+#pragma unroll
+            for (int q = 0; q < R; ++q)
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) n[q].v[e] = T.bz * c[q].v[e];
+        }
+        float s_tv = 0.0f, s_q = 0.0f;
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            F4 gx, gy, gz, inv, nrm;
+            float xr = __shfl_down_sync(0xffffffffu, c[q].v[0], 1);
+            const float ed = __shfl_sync(0xffffffffu, rc, q);
+            if (T.lane == 31) xr = ed;
+            if (T.xedge) xr = c[q].v[TQ_V - 1];
+            tq_gradient(D, c[q], c[q + 1], n[q], xr, T.xm, T.ym[q + 1], delta2, gx, gy, gz, inv, nrm);
+            if (T.rv[q]) {
+                F4 o;
+#pragma unroll
+                for (int e = 0; e < TQ_V; ++e) {
+                    const float res = c[q].v[e] - G[q].v[e];
+                    s_tv += nrm.v[e]; s_q = fmaf(res, res, s_q);
+                    o.v[e] = (cand_clip && c[q].v[e] < 0.0f) ? 0.0f : c[q].v[e];
+                }
+                if (TRIAL && cand) st4(cand + ok + ro[q], o);
+            }
+            if (hasg) G[q] = ldg4(g + og + ro[q]);
+            c[q] = ldg4(f + o2 + ro[q]);
+            if (TRIAL) rawd[q] = ldg4(dir + o2 + ro[q]);
+        }
+        c[R] = ldg4(f + o2 + ro[R]);
+        if (TRIAL) rawd[R] = ldg4(dir + o2 + ro[R]);
+        rc = ldg1(f + o2 + rco);
+        if (TRIAL) rD = ldg1(dir + o2 + rco);
+        e_tv += (double)s_tv; e_q += (double)s_q;
+    };
+
+    for (int k = T.k0; k < T.k1; k += 2) {
+        step(k, A, B, rA, rB);
+        if (k + 1 >= T.k1) break;
+        step(k + 1, B, A, rB, rA);
+    }
+}
+
+// The passes as kernels of their own (the host-sequenced loop, cbct_tv_energy): one block per tile.  VEC: the 16-byte tiles.
+template <bool FIRST, bool VEC>
+__global__ void __launch_bounds__(32 * TV_WPB)
+tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ g, float beta, float delta2,
+               float *__restrict__ d_out, int zc, double *__restrict__ partials, int stride,
+               unsigned int *__restrict__ counter, double *__restrict__ out)
+{
+    __shared__ double slot[32];
+    double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
+    if (VEC) {
+        const TqTile T = tq_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+        tq_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
+    } else {
+        const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+        tv_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
+    }
+    double s[3];
+    s[0] = block_sum(e_tv, slot);
+    s[1] = block_sum(e_q, slot);
+    s[2] = block_sum(e_d, slot);
+    publish_and_finalize<3>(s, 3, partials, stride, counter, out, slot);
+}
+
+template <bool TRIAL, bool VEC>
 __global__ void __launch_bounds__(32 * TV_WPB)
 tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__restrict__ dir,
                  const float *__restrict__ g, float lam, float delta2, int zc, int rows,
@@ -328,9 +643,14 @@ tv_energy_kernel(const TvDims D, const float *__restrict__ f, const float *__res
                  double *__restrict__ out, float *__restrict__ cand, int cand_clip)
 {
     __shared__ double slot[32];
-    const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
     double e_tv = 0.0, e_q = 0.0;
-    tv_energy_tile<TRIAL>(D, T, f, dir, g, lam, delta2, cand, cand_clip, e_tv, e_q);
+    if (VEC) {
+        const TqTile T = tq_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+        tq_energy_tile<TRIAL>(D, T, f, dir, g, lam, delta2, cand, cand_clip, e_tv, e_q);
+    } else {
+        const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
+        tv_energy_tile<TRIAL>(D, T, f, dir, g, lam, delta2, cand, cand_clip, e_tv, e_q);
+    }
     double s[2];
     s[0] = block_sum(e_tv, slot);
     s[1] = g != nullptr ? block_sum(e_q, slot) : 0.0;
@@ -393,7 +713,11 @@ struct TvCoop {
     double *report;         // [0] inner, [1] trials, [2] E_first, [3] E_last of this call; [4], [5] += inner, trials
 };
 
-__global__ void __launch_bounds__(32 * TV_WPB, 4)
+#ifndef TVC_MINB
+#define TVC_MINB 4
+#endif
+template <bool VEC>
+__global__ void __launch_bounds__(32 * TV_WPB, VEC ? TVC_MINB : 4)
 tv_prox_coop_kernel(const TvCoop p)
 {
     cg::grid_group grid = cg::this_grid();
@@ -469,9 +793,16 @@ tv_prox_coop_kernel(const TvCoop p)
         double tot[3];
         for (int t = next_tile(); t < ntiles; t = next_tile()) {
             double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-            const TvTile T = tv_tile(p.D, p.zc, t % p.ntx, (t / p.ntx) % p.nty, t / (p.ntx * p.nty));
-            if (cur == p.g) tv_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
-            else tv_grad_tile<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+            const int tx = t % p.ntx, ty = (t / p.ntx) % p.nty, tz = t / (p.ntx * p.nty);
+            if (VEC) {
+                const TqTile T = tq_tile(p.D, p.zc, tx, ty, tz);
+                if (cur == p.g) tq_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+                else tq_grad_tile<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+            } else {
+                const TvTile T = tv_tile(p.D, p.zc, tx, ty, tz);
+                if (cur == p.g) tv_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+                else tv_grad_tile<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+            }
             publish(t, a0, a1, a2, 3);
         }
         grid_sums(3, tot);
@@ -483,8 +814,14 @@ tv_prox_coop_kernel(const TvCoop p)
         for (int bt = 0; bt <= p.max_bt; ++bt) {
             for (int t = next_tile(); t < ntiles; t = next_tile()) {
                 double a0 = 0.0, a1 = 0.0;
-                const TvTile T = tv_tile(p.D, p.zc, t % p.ntx, (t / p.ntx) % p.nty, t / (p.ntx * p.nty));
-                tv_energy_tile<true>(p.D, T, cur, p.d, p.g, (float)lam, p.delta2, cand, p.nonneg, a0, a1);
+                const int tx = t % p.ntx, ty = (t / p.ntx) % p.nty, tz = t / (p.ntx * p.nty);
+                if (VEC) {
+                    const TqTile T = tq_tile(p.D, p.zc, tx, ty, tz);
+                    tq_energy_tile<true>(p.D, T, cur, p.d, p.g, (float)lam, p.delta2, cand, p.nonneg, a0, a1);
+                } else {
+                    const TvTile T = tv_tile(p.D, p.zc, tx, ty, tz);
+                    tv_energy_tile<true>(p.D, T, cur, p.d, p.g, (float)lam, p.delta2, cand, p.nonneg, a0, a1);
+                }
                 publish(t, a0, a1, 0.0, 2);
             }
             double tr[3];
@@ -514,18 +851,61 @@ tv_prox_coop_kernel(const TvCoop p)
     }
 }
 
-// z-slices per block: long marches amortise the halo slice and the block reduction; short ones
-// keep at least ~8 blocks per SM in flight on small volumes.
-static int tv_zchunk(const cbct_geometry *g, const TvDims &D)
+// The 16-byte tiles need whole 16-byte groups per row and aligned rows; below 128 voxels per row they would idle lanes.
+static bool tv_vec_ok(const TvDims &D, const void *a, const void *b = nullptr, const void *c = nullptr, const void *d = nullptr)
 {
+    if (getenv("CBCT_TV_NOVEC")) return false;
+    if (D.nx % TQ_V != 0 || D.nx < TQ_W) return false;
+    const void *p[4] = {a, b, c, d};
+    for (int i = 0; i < 4; ++i)
+        if (p[i] && (uintptr_t)p[i] % (4 * TQ_V) != 0) return false;
+    return true;
+}
+
+// blocks of the cooperative kernel resident per SM (the register cap of its launch bounds decides)
+static int tv_coop_occupancy(bool vec)
+{
+    static int occs[2] = {0, 0};
+    int &occ = occs[vec ? 1 : 0];
+    if (occ == 0) {
+        cudaError_t e = vec ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel<true>, 32 * TV_WPB, 0)
+                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel<false>, 32 * TV_WPB, 0);
+        if (e != cudaSuccess) { cudaGetLastError(); occ = 0; return 0; }
+    }
+    return occ;
+}
+
+// The z-extent of a tile (the `zc` argument of the tile functions), the same for the cooperative kernel and for the passes as
+// kernels of their own, so that both add the same per-tile partial sums.
+//  * 32-voxel tiles: zc slices per tile; long marches amortise the halo slice and the block reduction, short ones keep every
+//    SM supplied on small volumes (at least ~8 tiles per SM).
+//  * 128-voxel tiles: the NUMBER of balanced z-chunks, fitted to the blocks resident at once: with chunks of about 16 slices
+//    the tiles need m rounds of the persistent grid, and the chunk count is the largest that still fits m rounds -- at 256^3:
+//    592 blocks, 32 tiles per chunk -> 18 chunks of 14-15 slices, one round (16 chunks of 16 would leave 80 blocks idle,
+//    19 would need a second round for 16 tiles).
+static int tv_zchunk(const cbct_geometry *g, const TvDims &D, bool vec)
+{
+    if (const char *e = getenv("CBCT_TV_ZC")) return atoi(e);
+    if (vec) {
+        const long bxy = (long)((D.nx + TQ_W - 1) / TQ_W) * ((D.ny + TQ_R * TV_WPB - 1) / (TQ_R * TV_WPB));
+        const long slots = (long)g->sm_count * (tv_coop_occupancy(true) > 0 ? tv_coop_occupancy(true) : 1);
+        const long base = (D.nz + 15) / 16;
+        const long m = (bxy * base + slots - 1) / slots;
+        long ntz = m * slots / bxy;
+        const long cap = D.nz >= 8 ? D.nz / 4 : 1;
+        if (ntz > cap) ntz = cap;
+        if (ntz < 1) ntz = 1;
+        return (int)ntz;
+    }
     const int bxy = ((D.nx + 31) / 32) * ((D.ny + TV_R * TV_WPB - 1) / (TV_R * TV_WPB));
     int zc = 32;
     while (zc > 4 && (long)bxy * ((D.nz + zc - 1) / zc) < 8L * g->sm_count) zc >>= 1;
     return zc;
 }
 
-static dim3 tv_grid(const TvDims &D, int zc)
+static dim3 tv_grid(const TvDims &D, int zc, bool vec)
 {
+    if (vec) return dim3((D.nx + TQ_W - 1) / TQ_W, (D.ny + TQ_R * TV_WPB - 1) / (TQ_R * TV_WPB), zc);
     return dim3((D.nx + 31) / 32, (D.ny + TV_R * TV_WPB - 1) / (TV_R * TV_WPB), (D.nz + zc - 1) / zc);
 }
 
@@ -548,13 +928,18 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
                              double *d_out, cudaStream_t st)
 {
     TvDims D = tv_dims(L);
-    const int zc = tv_zchunk(g, D);
-    dim3 gr = tv_grid(D, zc), b(32, TV_WPB);
+    const bool vec = tv_vec_ok(D, d_f);
+    const int zc = tv_zchunk(g, D, vec);
+    dim3 gr = tv_grid(D, zc, vec), b(32, TV_WPB);
     if ((size_t)gr.x * gr.y * gr.z > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     StageTimer t(g, st, ST_REDUCE);
-    tv_energy_kernel<false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, 0.0f, (float)(delta * delta), zc, 1,
-                                              g->d_partials, g->partials_stride, g->d_counter, d_out, nullptr, 0);
+    if (vec)
+        tv_energy_kernel<false, true><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, 0.0f, (float)(delta * delta), zc, 1,
+                                                        g->d_partials, g->partials_stride, g->d_counter, d_out, nullptr, 0);
+    else
+        tv_energy_kernel<false, false><<<gr, b, 0, st>>>(D, d_f, nullptr, nullptr, 0.0f, (float)(delta * delta), zc, 1,
+                                                         g->d_partials, g->partials_stride, g->d_counter, d_out, nullptr, 0);
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
@@ -564,15 +949,13 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
 static cbct_status launch_tv_prox_coop(const cbct_geometry *g, const Level &L, const float *d_g, float *d_f, double w,
                                        int nonneg, const cbct_tv_params &tp, cudaStream_t st)
 {
-    static int occ = 0;
-    if (occ == 0) {
-        CBCT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel, 32 * TV_WPB, 0));
-        if (occ < 1) return cbct_fail(CBCT_ERR_CUDA, "the cooperative TV-prox kernel does not fit an SM");
-    }
     TvCoop p;
     p.D = tv_dims(L);
-    p.zc = tv_zchunk(g, p.D);
-    const dim3 tg = tv_grid(p.D, p.zc);
+    const bool vec = tv_vec_ok(p.D, d_g, d_f, L.d_f2, L.d_d);
+    const int occ = tv_coop_occupancy(vec);
+    if (occ < 1) return cbct_fail(CBCT_ERR_CUDA, "the cooperative TV-prox kernel does not fit an SM");
+    p.zc = tv_zchunk(g, p.D, vec);
+    const dim3 tg = tv_grid(p.D, p.zc, vec);
     p.ntx = tg.x; p.nty = tg.y; p.ntz = tg.z;
     p.g = d_g; p.f = d_f; p.f2 = L.d_f2; p.d = L.d_d;
     p.beta = 1.0 / w; p.armijo_c = tp.armijo_c; p.alpha = tp.shrink_alpha; p.rel_tol = tp.rel_tol; p.n = (double)L.nvox;
@@ -588,7 +971,8 @@ static cbct_status launch_tv_prox_coop(const cbct_geometry *g, const Level &L, c
     if (ntiles > g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     void *args[] = {&p};
     StageTimer t(g, st, ST_TV_GRAD);
-    CBCT_CUDA(cudaLaunchCooperativeKernel((const void *)tv_prox_coop_kernel, dim3((unsigned)blocks), dim3(32, TV_WPB), args, 0, st));
+    const void *kern = vec ? (const void *)tv_prox_coop_kernel<true> : (const void *)tv_prox_coop_kernel<false>;
+    CBCT_CUDA(cudaLaunchCooperativeKernel(kern, dim3((unsigned)blocks), dim3(32, TV_WPB), args, 0, st));
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
@@ -625,8 +1009,9 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         return CBCT_OK;
     }
     TvDims D = tv_dims(L);
-    const int zc = tv_zchunk(g, D);
-    dim3 gr = tv_grid(D, zc), b(32, TV_WPB);
+    const bool vec = tv_vec_ok(D, d_g, d_f, L.d_f2, L.d_d);
+    const int zc = tv_zchunk(g, D, vec);
+    dim3 gr = tv_grid(D, zc, vec), b(32, TV_WPB);
     const int S = g->partials_stride;
     if ((size_t)gr.x * gr.y * gr.z > (size_t)S) return cbct_fail(CBCT_ERR_INVALID_ARG, "volume too large for the reduction buffer");
     const double beta = 1.0 / w, N = (double)n;
@@ -641,8 +1026,10 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     for (int it = 0; it < tp.max_inner; ++it) {
         {
             StageTimer t(g, st, ST_TV_GRAD);
-            if (cur == d_g) tv_grad_kernel<true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
-            else tv_grad_kernel<false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            if (cur == d_g && vec) tv_grad_kernel<true, true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            else if (cur == d_g) tv_grad_kernel<true, false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            else if (vec) tv_grad_kernel<false, true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            else tv_grad_kernel<false, false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
             CBCT_LAUNCH_CHECK(g);
         }
         double lam = 1.0 / beta, Enew = E0, Dm = 0.0;
@@ -652,8 +1039,12 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
             {
                 StageTimer t(g, st, ST_TV_TRIAL);
                 // the trial also leaves its (truncated) volume in d_f unless d_f is what it reads
-                tv_energy_kernel<true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, (float)lam, delta2, zc, 2, g->d_partials, S,
-                                                         g->d_counter, ds + 4, cur != d_f ? d_f : nullptr, nonneg);
+                if (vec)
+                    tv_energy_kernel<true, true><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, (float)lam, delta2, zc, 2, g->d_partials, S,
+                                                                   g->d_counter, ds + 4, cur != d_f ? d_f : nullptr, nonneg);
+                else
+                    tv_energy_kernel<true, false><<<gr, b, 0, st>>>(D, cur, L.d_d, d_g, (float)lam, delta2, zc, 2, g->d_partials, S,
+                                                                    g->d_counter, ds + 4, cur != d_f ? d_f : nullptr, nonneg);
                 CBCT_LAUNCH_CHECK(g);
             }
             CBCT_CUDA(cudaMemcpyAsync(hs, ds, 6 * sizeof(double), cudaMemcpyDeviceToHost, st));
