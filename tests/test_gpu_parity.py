@@ -176,10 +176,15 @@ def test_edge_cases_missing_rays_and_unseen_voxels(torch, cbct, orc):
 
 @pytest.mark.parametrize("host_armijo", [False, True])
 @pytest.mark.parametrize("bc", [(I.BC_ZERO, I.BC_REFLECT), (I.BC_REFLECT, I.BC_REFLECT), (I.BC_ZERO, I.BC_ZERO)])
-def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc, host_armijo):
+@pytest.mark.parametrize("shape", [(37, 45, 19), (132, 21, 11), (256, 16, 5)])
+def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc, host_armijo, shape):
     """Both control paths of the Armijo loop: the cooperative kernel that decides on the device (default) and the
-    host-sequenced loop (CBCT_KERNEL_HOST_ARMIJO)."""
-    g = I.Geometry(nx=37, ny=45, nz=19, hx=1.7, hy=1.3, hz=2.9, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
+    host-sequenced loop (CBCT_KERNEL_HOST_ARMIJO).  Shapes: the 32-voxel warp tiles (nx = 37: ragged in x, y and z), and
+    the 16-byte tiles of tv.cu (nx % 4 == 0, nx >= 128): 132 x 21 x 11 has a second tile column with ONE valid lane (so the
+    p_x column left of a tile and the right-neighbour column are both exercised), ragged rows and two z-chunks;
+    256 x 16 x 5 fills both tile columns exactly."""
+    nx, ny, nz = shape
+    g = I.Geometry(nx=nx, ny=ny, nz=nz, hx=1.7, hy=1.3, hz=2.9, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
                    n_proj=1, bc_xy=bc[0], bc_z=bc[1])
     rng = np.random.default_rng(41)
     base = I.paint([I.Ellipsoid((2.0, -3.0, 1.0), (20.0, 18.0, 16.0), 0.3, 0.02),
@@ -207,9 +212,34 @@ def test_tv_energy_and_prox_match_oracle(torch, cbct, orc, bc, host_armijo):
     assert rep.e_last < rep.e_first
 
 
+def test_tv_prox_unaligned_volumes_take_the_scalar_tiles(torch, cbct, orc):
+    """nx = 128 qualifies for the 16-byte tiles, buffers 4 bytes off a 16-byte boundary do not: same result either way."""
+    g = I.Geometry(nx=128, ny=9, nz=6, hx=1.0, hy=1.5, hz=2.0, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
+                   n_proj=1, bc_xy=I.BC_ZERO, bc_z=I.BC_REFLECT)
+    rng = np.random.default_rng(43)
+    gg = (0.01 + 0.003 * rng.standard_normal(g.vol_shape)).astype(np.float32)
+    setup = I.FbsSetup(eps_delta=1e-5, max_inner=3, rel_tol=0.0)
+    want, wrep = orc.tv_prox(g, gg, 2e-3, setup)
+    n = gg.size
+    with cbct.geometry_create(g) as h:
+        outs = []
+        for off in (0, 1):
+            src = torch.zeros(n + 4, device="cuda", dtype=torch.float32)
+            dst = torch.zeros(n + 4, device="cuda", dtype=torch.float32)
+            gv, fv = src[off:off + n].view(g.vol_shape), dst[off:off + n].view(g.vol_shape)
+            gv.copy_(dev(torch, gg))
+            rep = h.tv_prox(gv, fv, 2e-3, setup)
+            assert (rep.inner_iters, rep.trials) == (wrep.inner_iters, wrep.trials)
+            assert h.tv_energy(gv, setup.eps_delta) == pytest.approx(orc.tv_energy(g, gg, setup.eps_delta), rel=1e-6)
+            outs.append(fv.cpu().numpy().copy())
+    assert rel_l2(outs[0], want) <= 1e-5 and rel_l2(outs[1], want) <= 1e-5
+    assert rel_l2(outs[0], outs[1]) <= 1e-6
+
+
 @pytest.mark.parametrize("host_armijo", [False, True])
-def test_tv_prox_degenerate_cases(torch, cbct, host_armijo):
-    g = I.Geometry(nx=16, ny=12, nz=6, hx=1.0, hy=1.0, hz=1.0, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
+@pytest.mark.parametrize("nx", [16, 128])
+def test_tv_prox_degenerate_cases(torch, cbct, host_armijo, nx):
+    g = I.Geometry(nx=nx, ny=12, nz=6, hx=1.0, hy=1.0, hz=1.0, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
                    n_proj=1, bc_xy=I.BC_REFLECT, bc_z=I.BC_REFLECT)
     setup = I.FbsSetup()
     with cbct.geometry_create(g, host_armijo=host_armijo) as h:
