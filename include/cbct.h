@@ -76,6 +76,9 @@ typedef struct {
 #define CBCT_KERNEL_HOST_ARMIJO 2 /* cbct_tv_prox sequenced by the host (one stream synchronisation per Armijo trial) instead
                                      of the single cooperative kernel that takes every accept / shrink / stop decision on
                                      the device; same passes, same decisions.  For A/B measurements and tests. */
+#define CBCT_KERNEL_TV_SCALAR_TILES 4 /* the TV passes always on the 32-voxel warp tiles (one voxel per lane), never on the
+                                         16-byte tiles that volumes with nx % 4 == 0, nx >= 128 and 16-byte aligned buffers
+                                         otherwise take; same stencil, for A/B measurements and tests. */
 
 /* Validates the description, uploads per-view tables and allocates all scratch for
  * `max_levels` levels.  *out is NULL on failure. */

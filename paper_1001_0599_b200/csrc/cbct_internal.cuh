@@ -126,6 +126,7 @@ struct cbct_geometry {
     int sm_count = 148;
     int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
     int host_armijo = 0;            // bit 1: the host-sequenced Armijo loop instead of the cooperative TV-prox kernel
+    int tv_scalar_tiles = 0;        // bit 2: the TV passes on the 32-voxel warp tiles only
     unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always
 };
 

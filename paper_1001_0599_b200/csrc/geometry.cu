@@ -149,6 +149,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     g->allow_symmetry = desc->no_symmetry ? 0 : 1;
     g->disable_tma = (desc->kernel_flags & CBCT_KERNEL_NO_TMA) ? 1 : 0;
     g->host_armijo = (desc->kernel_flags & CBCT_KERNEL_HOST_ARMIJO) ? 1 : 0;
+    g->tv_scalar_tiles = (desc->kernel_flags & CBCT_KERNEL_TV_SCALAR_TILES) ? 1 : 0;
     {   // the cooperative TV-prox kernel needs cooperative launches (every sm_100 device has them; checked all the same)
         int coop = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) g->host_armijo = 1;

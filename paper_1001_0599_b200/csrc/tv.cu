@@ -8,7 +8,6 @@
 // value (BC_REFLECT) (L161).  div is the exact negative transpose (backward differences,
 // p_{-1} = 0).  Per-voxel terms are fp32, sums are fp64 in a fixed order (reduce.cuh).
 #include <math.h>
-#include <stdlib.h>
 #include <cooperative_groups.h>
 #include "cbct_internal.cuh"
 #include "reduce.cuh"
@@ -314,40 +313,28 @@ __device__ __forceinline__ void tv_energy_tile(const TvDims &D, const TvTile &T,
 // are done, and is refilled with the same row of slice k+2 on the spot (the march is unrolled by two, the two register
 // sets swapping roles), so every load has a whole slice of arithmetic to land.
 // ---------------------------------------------------------------------------------------------------------------------
-#ifndef TQ_ROWS
-#define TQ_ROWS 4
-#endif
-constexpr int TQ_R = TQ_ROWS; // rows per warp tile
-#ifndef TQ_VOX
-#define TQ_VOX 4
-#endif
-constexpr int TQ_V = TQ_VOX;  // consecutive voxels per lane (4: 16-byte accesses, 2: 8-byte)
+constexpr int TQ_R = 4;       // rows per warp tile
+constexpr int TQ_V = 4;       // consecutive voxels per lane: 16-byte accesses (2, with 8-byte accesses, measured 25-30 % slower)
 constexpr int TQ_W = 32 * TQ_V;   // voxels per warp tile row
 
 struct F4 { float v[TQ_V]; };
-// The refills are volatile asm with a memory clobber: the compiler otherwise sinks them to the end of the slice (their
-// targets are dead registers either way), right in front of their first use, and the march stalls on every load.
+// Streaming loads: read-only path, no L1 line allocated -- the gradient pass's rings leave the SM ~20 KB of L1, and every
+// line a streaming load allocates there is one fewer load in flight.
 __device__ __forceinline__ F4 ldg4(const float *__restrict__ p)
 {
     F4 r;
-    if constexpr (TQ_V == 4)
-        asm volatile("ld.volatile.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[TQ_V - 1]) : "l"(p) : "memory");
-    else
-        asm volatile("ld.volatile.global.v2.f32 {%0, %1}, [%2];" : "=f"(r.v[0]), "=f"(r.v[1]) : "l"(p) : "memory");
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "l"(p) : "memory");
     return r;
 }
 __device__ __forceinline__ float ldg1(const float *__restrict__ p)
 {
     float r;
-    asm volatile("ld.volatile.global.f32 %0, [%1];" : "=f"(r) : "l"(p) : "memory");
+    asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(r) : "l"(p) : "memory");
     return r;
 }
 __device__ __forceinline__ void st4(float *__restrict__ p, const F4 &a)
 {
-    if constexpr (TQ_V == 4)
-        asm volatile("st.volatile.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]), "f"(a.v[2]), "f"(a.v[TQ_V - 1]) : "memory");
-    else
-        asm volatile("st.volatile.global.v2.f32 [%0], {%1, %2};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]) : "memory");
+    asm volatile("st.global.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a.v[0]), "f"(a.v[1]), "f"(a.v[2]), "f"(a.v[3]) : "memory");
 }
 
 struct TqTile {
@@ -412,112 +399,151 @@ __device__ __forceinline__ void tq_gradient(const TvDims &D, const F4 &c, const 
     }
 }
 
-template <bool FIRST>
-__device__ __forceinline__ void tq_grad_tile(const TvDims &D, const TqTile &T, const float *__restrict__ f,
-                                             const float *__restrict__ g, float beta, float delta2,
-                                             float *__restrict__ d_out, double &e_tv, double &e_q, double &e_d)
+// The gradient pass with its loads staged through shared memory by cp.async (sm_80+ LDGSTS; 16 bytes per lane, L1 bypassed):
+// every warp owns a ring of three slices x (R+2) rows of u and two slices x R rows of g, 13 KB, filled two slices ahead of
+// the arithmetic by the lanes that will read it (no block barrier: a lane reads back its own 16 bytes; the one cross-lane read
+// -- lane 0's first voxel for the column left of the tile -- follows a __syncwarp).  The slices in flight cost no registers,
+// so the pass keeps 16 warps per SM where the register-staged form above spilled under the 128-register cap of the
+// cooperative kernel.  Same arithmetic, same order of operations per voxel, same sums.
+constexpr int TQ_RING = 3;
+constexpr int TQ_SMEM_PER_WARP = (TQ_RING * (TQ_R + 2) + 2 * TQ_R) * 32 * 16;      // bytes
+constexpr int TQ_SMEM_PER_BLOCK = TQ_SMEM_PER_WARP * TV_WPB;
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const float *src)
 {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ F4 lds4(uint32_t a)
+{
+    F4 r;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(r.v[0]), "=f"(r.v[1]), "=f"(r.v[2]), "=f"(r.v[3]) : "r"(a) : "memory");
+    return r;
+}
+__device__ __forceinline__ float lds1(uint32_t a)
+{
+    float r;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(r) : "r"(a) : "memory");
+    return r;
+}
+
+// this warp's ring in the block's dynamic shared memory (TQ_SMEM_PER_BLOCK bytes)
+extern __shared__ __align__(16) unsigned char tq_dyn_smem[];
+__device__ __forceinline__ uint32_t tq_ring_base()
+{
+    return (uint32_t)__cvta_generic_to_shared(tq_dyn_smem) + threadIdx.y * TQ_SMEM_PER_WARP;
+}
+
+template <bool FIRST>
+__device__ __forceinline__ void tq_grad_tile_async(const TvDims &D, const TqTile &T, const float *__restrict__ f,
+                                                   const float *__restrict__ g, float beta, float delta2,
+                                                   float *__restrict__ d_out, uint32_t ring, double &e_tv, double &e_q, double &e_d)
+{
+    static_assert(TQ_V == 4, "cp.async stages 16 bytes per lane");
     constexpr int R = TQ_R;
     const size_t pl = T.plane;
     const int ztopk = D.nz - 1, kend = min(T.k1, ztopk);
-    F4 A[R + 2], B[R + 2], G[R], pzp[R];
-    float lA, lB, rA, rB;
-    {
-        const float *p0 = f + (size_t)T.ks * pl, *p1 = f + (size_t)min(T.ks + 1, ztopk) * pl;
+    // ring addresses of this lane: slice s, row q -> ring + ((s % 3) * (R+2) + q) * 512 + lane * 16; g: gring + ((s & 1) * R + r) * 512
+    const uint32_t fr = ring + T.lane * 16, gr = ring + TQ_RING * (R + 2) * 512 + T.lane * 16;
+    auto issue_f = [&](int slice, int slot) {
+        const float *ps = f + (size_t)slice * pl;
 #pragma unroll
-        for (int q = 0; q <= R + 1; ++q) { A[q] = ldg4(p0 + T.ro[q]); B[q] = ldg4(p1 + T.ro[q]); }
+        for (int q = 0; q <= R + 1; ++q) cp_async16(fr + (slot * (R + 2) + q) * 512, ps + T.ro[q]);
+    };
+    auto issue_g = [&](int slice, int slot) {
+        if (FIRST) return;
+        const float *ps = g + (size_t)slice * pl;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            if (!FIRST) G[r] = ldg4(g + (size_t)T.ks * pl + T.ro[r + 1]);
+        for (int r = 0; r < R; ++r) cp_async16(gr + (slot * R + r) * 512, ps + T.ro[r + 1]);
+    };
+    F4 pzp[R];
 #pragma unroll
-            for (int e = 0; e < TQ_V; ++e) { pzp[r].v[e] = 0.0f; if (FIRST) G[r].v[e] = 0.0f; }
-        }
-        lA = ldg1(p0 + T.lco); lB = ldg1(p1 + T.lco);
-        rA = ldg1(p0 + T.rco); rB = ldg1(p1 + T.rco);
-    }
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int e = 0; e < TQ_V; ++e) pzp[r].v[e] = 0.0f;
+    int s0 = T.ks % TQ_RING;                              // ring slot of slice k
+    issue_f(T.ks, s0); issue_g(T.ks, T.ks & 1); cp_async_commit();
+    issue_f(min(T.ks + 1, ztopk), (s0 + 1) % TQ_RING); cp_async_commit();
+    float lc = ldg1(f + (size_t)T.ks * pl + T.lco), ln = ldg1(f + (size_t)min(T.ks + 1, ztopk) * pl + T.lco);
+    float rc = ldg1(f + (size_t)T.ks * pl + T.rco), rn = ldg1(f + (size_t)min(T.ks + 1, ztopk) * pl + T.rco);
 
-    auto step = [&](int k, F4 (&c)[R + 2], F4 (&n)[R + 2], float &lc, float &ln, float &rc) {
-        // refills: slice k+2, held at the last slice this tile reads (a re-read of a line just loaded, never used)
-        const float *p2 = f + (size_t)min(k + 2, kend) * pl;
-        const float *pg = g + (size_t)min(k + 1, T.k1 - 1) * pl;
+    for (int k = T.ks; k < T.k1; ++k) {
+        const int s1 = s0 + 1 == TQ_RING ? 0 : s0 + 1, s2 = s1 + 1 == TQ_RING ? 0 : s1 + 1;
+        issue_f(min(k + 2, kend), s2); issue_g(min(k + 1, T.k1 - 1), (k + 1) & 1); cp_async_commit();
+        const float l2 = ldg1(f + (size_t)min(k + 2, kend) * pl + T.lco), r2 = ldg1(f + (size_t)min(k + 2, kend) * pl + T.rco);
+        cp_async_wait<1>();                              // slices k, k+1 and g(k) have landed
+        __syncwarp();
         float *pd = d_out + (size_t)k * pl;
         const bool ztop = k + 1 >= D.nz, emit = k >= T.k0;
-        if (ztop) {                                      // the top slice of the grid: u(.,.,k+1) is the boundary value
-#pragma unroll
-            for (int q = 0; q <= R; ++q)
-#pragma unroll
-                for (int e = 0; e < TQ_V; ++e) n[q].v[e] = T.bz * c[q].v[e];
-            ln = T.bz * lc;
-        }
+        const uint32_t fc = fr + s0 * (R + 2) * 512, fn = fr + s1 * (R + 2) * 512, gc = gr + (k & 1) * R * 512;
+        if (ztop) ln = T.bz * lc;
         float hpx = 0.0f;
         if (T.hx) {                                      // warp-uniform: column i0-1, p_x only, its rows in lanes 0..R-1
-            float xn = 0.0f;
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float v = __shfl_sync(0xffffffffu, c[r + 1].v[0], 0);
-                if (T.lane == r) xn = v;
-            }
+            const float xn = lds1(fc - T.lane * 16 + (min(T.lane, R - 1) + 1) * 512);     // lane 0's first voxel of row j0+lane
             const float yn = __shfl_down_sync(0xffffffffu, lc, 1);
             const float gx = (xn - lc) * D.ihx, gy = fmaf(yn, T.lym, -lc) * D.ihy, gz = (ln - lc) * D.ihz;
             float inv;
             grad_norm(gx, gy, gz, delta2, inv);
             hpx = gx * inv;
-            lc = ldg1(p2 + T.lco);
         }
-        F4 pyp;
+        F4 pyp, cq = lds4(fc);
 #pragma unroll
         for (int e = 0; e < TQ_V; ++e) pyp.v[e] = 0.0f;
         float s_tv = 0.0f, s_q = 0.0f, s_d = 0.0f;
 #pragma unroll
         for (int q = 0; q <= R; ++q) {                   // rows j0-1 (p_y only) .. j0+R-1
-            if (q == 0 && !T.hy) { c[0] = ldg4(p2 + T.ro[0]); continue; }
-            F4 gx, gy, gz, inv, nrm;
-            float xr = __shfl_down_sync(0xffffffffu, c[q].v[0], 1);
-            const float ed = __shfl_sync(0xffffffffu, rc, q);
-            if (T.lane == 31) xr = ed;
-            if (T.xedge) xr = c[q].v[TQ_V - 1];
-            tq_gradient(D, c[q], c[q + 1], n[q], xr, T.xm, T.ym[q], delta2, gx, gy, gz, inv, nrm);
-            if (q == 0) {
+            const F4 cy = lds4(fc + (q + 1) * 512);
+            if (q > 0 || T.hy) {
+                F4 zn, gx, gy, gz, inv, nrm;
+                if (ztop) {
 #pragma unroll
-                for (int e = 0; e < TQ_V; ++e) pyp.v[e] = gy.v[e] * inv.v[e];
-            } else {
-                const int r = q - 1;
-                F4 px, dd;
-#pragma unroll
-                for (int e = 0; e < TQ_V; ++e) px.v[e] = gx.v[e] * inv.v[e];
-                float left = __shfl_up_sync(0xffffffffu, px.v[TQ_V - 1], 1);
-                const float edge = __shfl_sync(0xffffffffu, hpx, r);
-                if (T.lane == 0) left = edge;
-#pragma unroll
-                for (int e = 0; e < TQ_V; ++e) {
-                    const float py = gy.v[e] * inv.v[e], pz = gz.v[e] * inv.v[e];
-                    const float div = (px.v[e] - (e == 0 ? left : px.v[e > 0 ? e - 1 : 0])) * D.ihx + (py - pyp.v[e]) * D.ihy +
-                                      (pz - pzp[r].v[e]) * D.ihz;
-                    const float res = FIRST ? 0.0f : c[q].v[e] - G[r].v[e];
-                    dd.v[e] = FIRST ? -div : fmaf(beta, res, -div);
-                    pyp.v[e] = py; pzp[r].v[e] = pz;
-                    if (emit && T.rv[r]) {
-                        s_tv += nrm.v[e];
-                        if (!FIRST) s_q = fmaf(res, res, s_q);
-                        s_d = fmaf(dd.v[e], dd.v[e], s_d);
-                    }
+                    for (int e = 0; e < TQ_V; ++e) zn.v[e] = T.bz * cq.v[e];
+                } else {
+                    zn = lds4(fn + q * 512);
                 }
-                if (emit && T.rv[r]) st4(pd + T.ro[q], dd);
-                if (!FIRST) G[r] = ldg4(pg + T.ro[q]);
+                float xr = __shfl_down_sync(0xffffffffu, cq.v[0], 1);
+                const float ed = __shfl_sync(0xffffffffu, rc, q);
+                if (T.lane == 31) xr = ed;
+                if (T.xedge) xr = cq.v[TQ_V - 1];
+                tq_gradient(D, cq, cy, zn, xr, T.xm, T.ym[q], delta2, gx, gy, gz, inv, nrm);
+                if (q == 0) {
+#pragma unroll
+                    for (int e = 0; e < TQ_V; ++e) pyp.v[e] = gy.v[e] * inv.v[e];
+                } else {
+                    const int r = q - 1;
+                    F4 px, dd, G;
+                    if (!FIRST) G = lds4(gc + r * 512);
+#pragma unroll
+                    for (int e = 0; e < TQ_V; ++e) px.v[e] = gx.v[e] * inv.v[e];
+                    float left = __shfl_up_sync(0xffffffffu, px.v[TQ_V - 1], 1);
+                    const float edge = __shfl_sync(0xffffffffu, hpx, r);
+                    if (T.lane == 0) left = edge;
+#pragma unroll
+                    for (int e = 0; e < TQ_V; ++e) {
+                        const float py = gy.v[e] * inv.v[e], pz = gz.v[e] * inv.v[e];
+                        const float div = (px.v[e] - (e == 0 ? left : px.v[e > 0 ? e - 1 : 0])) * D.ihx + (py - pyp.v[e]) * D.ihy +
+                                          (pz - pzp[r].v[e]) * D.ihz;
+                        const float res = FIRST ? 0.0f : cq.v[e] - G.v[e];
+                        dd.v[e] = FIRST ? -div : fmaf(beta, res, -div);
+                        pyp.v[e] = py; pzp[r].v[e] = pz;
+                        if (emit && T.rv[r]) {
+                            s_tv += nrm.v[e];
+                            if (!FIRST) s_q = fmaf(res, res, s_q);
+                            s_d = fmaf(dd.v[e], dd.v[e], s_d);
+                        }
+                    }
+                    if (emit && T.rv[r]) st4(pd + T.ro[q], dd);
+                }
             }
-            c[q] = ldg4(p2 + T.ro[q]);                   // this row of slice k is done with: refill it two slices ahead
+            cq = cy;
         }
-        c[R + 1] = ldg4(p2 + T.ro[R + 1]);
-        rc = ldg1(p2 + T.rco);
         e_tv += (double)s_tv; e_d += (double)s_d;
         if (!FIRST) e_q += (double)s_q;
-    };
-
-    for (int k = T.ks; k < T.k1; k += 2) {
-        step(k, A, B, lA, lB, rA);
-        if (k + 1 >= T.k1) break;
-        step(k + 1, B, A, lB, lA, rB);
+        lc = ln; ln = l2; rc = rn; rn = r2;
+        s0 = s1;
     }
+    cp_async_wait<0>();
 }
 
 // Energy pass on the 16-byte tiles: rows j0 .. j0+R-1 and the value-only row j0+R.  TRIAL: u = f - lam dir, combined one slice
@@ -623,7 +649,7 @@ tv_grad_kernel(const TvDims D, const float *__restrict__ f, const float *__restr
     double e_tv = 0.0, e_q = 0.0, e_d = 0.0;
     if (VEC) {
         const TqTile T = tq_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
-        tq_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
+        tq_grad_tile_async<FIRST>(D, T, f, g, beta, delta2, d_out, tq_ring_base(), e_tv, e_q, e_d);
     } else {
         const TvTile T = tv_tile(D, zc, blockIdx.x, blockIdx.y, blockIdx.z);
         tv_grad_tile<FIRST>(D, T, f, g, beta, delta2, d_out, e_tv, e_q, e_d);
@@ -699,6 +725,14 @@ __global__ void tv_update_kernel<float4>(size_t n, const float4 *f, const float4
 // volume doubling as the result when the accepted step is the last.  Sums depend on the grid size only (fixed for a
 // device), never on timing: bitwise reproducible.
 // ---------------------------------------------------------------------------------------------------------------------
+// a 16-byte load that does not allocate an L1 line (plain ld: the target may be written by the same thread afterwards)
+__device__ __forceinline__ float4 ld_stream4(const float4 *p)
+{
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
 struct TvCoop {
     TvDims D;
     const float *g;
@@ -713,11 +747,8 @@ struct TvCoop {
     double *report;         // [0] inner, [1] trials, [2] E_first, [3] E_last of this call; [4], [5] += inner, trials
 };
 
-#ifndef TVC_MINB
-#define TVC_MINB 4
-#endif
 template <bool VEC>
-__global__ void __launch_bounds__(32 * TV_WPB, VEC ? TVC_MINB : 4)
+__global__ void __launch_bounds__(32 * TV_WPB, 4)
 tv_prox_coop_kernel(const TvCoop p)
 {
     cg::grid_group grid = cg::this_grid();
@@ -765,9 +796,9 @@ tv_prox_coop_kernel(const TvCoop p)
         const bool vec = p.nvox % 4 == 0 && ((uintptr_t)src % 16 == 0) && ((uintptr_t)out % 16 == 0) && (!dir || (uintptr_t)dir % 16 == 0);
         if (vec) {
             for (size_t o = i0; o < p.nvox / 4; o += step) {
-                float4 v = reinterpret_cast<const float4 *>(src)[o];
+                float4 v = ld_stream4(reinterpret_cast<const float4 *>(src) + o);
                 if (dir) {
-                    const float4 w = reinterpret_cast<const float4 *>(dir)[o];
+                    const float4 w = ld_stream4(reinterpret_cast<const float4 *>(dir) + o);
                     v.x = fmaf(-lam, w.x, v.x); v.y = fmaf(-lam, w.y, v.y); v.z = fmaf(-lam, w.z, v.z); v.w = fmaf(-lam, w.w, v.w);
                 }
                 if (clip) {
@@ -796,8 +827,8 @@ tv_prox_coop_kernel(const TvCoop p)
             const int tx = t % p.ntx, ty = (t / p.ntx) % p.nty, tz = t / (p.ntx * p.nty);
             if (VEC) {
                 const TqTile T = tq_tile(p.D, p.zc, tx, ty, tz);
-                if (cur == p.g) tq_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
-                else tq_grad_tile<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
+                if (cur == p.g) tq_grad_tile_async<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, tq_ring_base(), a0, a1, a2);
+                else tq_grad_tile_async<false>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, tq_ring_base(), a0, a1, a2);
             } else {
                 const TvTile T = tv_tile(p.D, p.zc, tx, ty, tz);
                 if (cur == p.g) tv_grad_tile<true>(p.D, T, cur, p.g, (float)p.beta, p.delta2, p.d, a0, a1, a2);
@@ -852,9 +883,10 @@ tv_prox_coop_kernel(const TvCoop p)
 }
 
 // The 16-byte tiles need whole 16-byte groups per row and aligned rows; below 128 voxels per row they would idle lanes.
-static bool tv_vec_ok(const TvDims &D, const void *a, const void *b = nullptr, const void *c = nullptr, const void *d = nullptr)
+static bool tv_vec_ok(const cbct_geometry *g, const TvDims &D, const void *a, const void *b = nullptr, const void *c = nullptr,
+                      const void *d = nullptr)
 {
-    if (getenv("CBCT_TV_NOVEC")) return false;
+    if (g->tv_scalar_tiles) return false;
     if (D.nx % TQ_V != 0 || D.nx < TQ_W) return false;
     const void *p[4] = {a, b, c, d};
     for (int i = 0; i < 4; ++i)
@@ -863,12 +895,20 @@ static bool tv_vec_ok(const TvDims &D, const void *a, const void *b = nullptr, c
 }
 
 // blocks of the cooperative kernel resident per SM (the register cap of its launch bounds decides)
+// dynamic shared memory of the kernels that run the 16-byte gradient tiles (the cp.async rings); set once per kernel
+static int tv_vec_smem() { return TQ_SMEM_PER_BLOCK; }
+template <typename K> static bool tv_allow_smem(K kern)
+{
+    return tv_vec_smem() <= 48 * 1024 || cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, tv_vec_smem()) == cudaSuccess;
+}
+
 static int tv_coop_occupancy(bool vec)
 {
     static int occs[2] = {0, 0};
     int &occ = occs[vec ? 1 : 0];
     if (occ == 0) {
-        cudaError_t e = vec ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel<true>, 32 * TV_WPB, 0)
+        if (vec && !tv_allow_smem(tv_prox_coop_kernel<true>)) { cudaGetLastError(); return 0; }
+        cudaError_t e = vec ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel<true>, 32 * TV_WPB, tv_vec_smem())
                             : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tv_prox_coop_kernel<false>, 32 * TV_WPB, 0);
         if (e != cudaSuccess) { cudaGetLastError(); occ = 0; return 0; }
     }
@@ -885,7 +925,6 @@ static int tv_coop_occupancy(bool vec)
 //    19 would need a second round for 16 tiles).
 static int tv_zchunk(const cbct_geometry *g, const TvDims &D, bool vec)
 {
-    if (const char *e = getenv("CBCT_TV_ZC")) return atoi(e);
     if (vec) {
         const long bxy = (long)((D.nx + TQ_W - 1) / TQ_W) * ((D.ny + TQ_R * TV_WPB - 1) / (TQ_R * TV_WPB));
         const long slots = (long)g->sm_count * (tv_coop_occupancy(true) > 0 ? tv_coop_occupancy(true) : 1);
@@ -928,7 +967,7 @@ cbct_status launch_tv_energy(const cbct_geometry *g, const Level &L, const float
                              double *d_out, cudaStream_t st)
 {
     TvDims D = tv_dims(L);
-    const bool vec = tv_vec_ok(D, d_f);
+    const bool vec = tv_vec_ok(g, D, d_f);
     const int zc = tv_zchunk(g, D, vec);
     dim3 gr = tv_grid(D, zc, vec), b(32, TV_WPB);
     if ((size_t)gr.x * gr.y * gr.z > (size_t)g->partials_stride)
@@ -951,7 +990,7 @@ static cbct_status launch_tv_prox_coop(const cbct_geometry *g, const Level &L, c
 {
     TvCoop p;
     p.D = tv_dims(L);
-    const bool vec = tv_vec_ok(p.D, d_g, d_f, L.d_f2, L.d_d);
+    const bool vec = tv_vec_ok(g, p.D, d_g, d_f, L.d_f2, L.d_d);
     const int occ = tv_coop_occupancy(vec);
     if (occ < 1) return cbct_fail(CBCT_ERR_CUDA, "the cooperative TV-prox kernel does not fit an SM");
     p.zc = tv_zchunk(g, p.D, vec);
@@ -972,7 +1011,7 @@ static cbct_status launch_tv_prox_coop(const cbct_geometry *g, const Level &L, c
     void *args[] = {&p};
     StageTimer t(g, st, ST_TV_GRAD);
     const void *kern = vec ? (const void *)tv_prox_coop_kernel<true> : (const void *)tv_prox_coop_kernel<false>;
-    CBCT_CUDA(cudaLaunchCooperativeKernel(kern, dim3((unsigned)blocks), dim3(32, TV_WPB), args, 0, st));
+    CBCT_CUDA(cudaLaunchCooperativeKernel(kern, dim3((unsigned)blocks), dim3(32, TV_WPB), args, vec ? tv_vec_smem() : 0, st));
     CBCT_LAUNCH_CHECK(g);
     return CBCT_OK;
 }
@@ -1009,7 +1048,7 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
         return CBCT_OK;
     }
     TvDims D = tv_dims(L);
-    const bool vec = tv_vec_ok(D, d_g, d_f, L.d_f2, L.d_d);
+    const bool vec = tv_vec_ok(g, D, d_g, d_f, L.d_f2, L.d_d);
     const int zc = tv_zchunk(g, D, vec);
     dim3 gr = tv_grid(D, zc, vec), b(32, TV_WPB);
     const int S = g->partials_stride;
@@ -1026,9 +1065,11 @@ cbct_status run_tv_prox(const cbct_geometry *g, const Level &L, const float *d_g
     for (int it = 0; it < tp.max_inner; ++it) {
         {
             StageTimer t(g, st, ST_TV_GRAD);
-            if (cur == d_g && vec) tv_grad_kernel<true, true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            if (vec && !(tv_allow_smem(tv_grad_kernel<true, true>) && tv_allow_smem(tv_grad_kernel<false, true>)))
+                return cbct_fail(CBCT_ERR_CUDA, "the gradient pass's shared-memory rings do not fit");
+            if (cur == d_g && vec) tv_grad_kernel<true, true><<<gr, b, tv_vec_smem(), st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
             else if (cur == d_g) tv_grad_kernel<true, false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
-            else if (vec) tv_grad_kernel<false, true><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
+            else if (vec) tv_grad_kernel<false, true><<<gr, b, tv_vec_smem(), st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
             else tv_grad_kernel<false, false><<<gr, b, 0, st>>>(D, cur, d_g, (float)beta, delta2, L.d_d, zc, g->d_partials, S, g->d_counter, ds);
             CBCT_LAUNCH_CHECK(g);
         }

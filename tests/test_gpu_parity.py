@@ -236,6 +236,26 @@ def test_tv_prox_unaligned_volumes_take_the_scalar_tiles(torch, cbct, orc):
     assert rel_l2(outs[0], outs[1]) <= 1e-6
 
 
+def test_tv_tile_families_agree(torch, cbct):
+    """CBCT_KERNEL_TV_SCALAR_TILES keeps a 16-byte-eligible volume on the 32-voxel tiles: both families give the same
+    descent (identical counts, volumes to fp32 rounding of the fp64 sums' inputs) -- zero-BC in-plane, several tile columns
+    and rows, more z-chunks than one."""
+    g = I.Geometry(nx=260, ny=37, nz=23, hx=0.9, hy=1.1, hz=1.7, nu=8, nv=8, du=2.0, dv=2.0, sad=400.0, sdd=650.0,
+                   n_proj=1, bc_xy=I.BC_ZERO, bc_z=I.BC_REFLECT)
+    rng = np.random.default_rng(44)
+    gg = dev(torch, 0.01 + 0.003 * rng.standard_normal(g.vol_shape))
+    setup = I.FbsSetup(eps_delta=1e-5, max_inner=5, rel_tol=0.0)
+    outs, reps = [], []
+    for scalar in (False, True):
+        with cbct.geometry_create(g, tv_scalar_tiles=scalar) as h:
+            f = torch.empty_like(gg)
+            reps.append(h.tv_prox(gg, f, 3e-3, setup, nonneg=True))
+            outs.append(f.cpu().numpy())
+    assert (reps[0].inner_iters, reps[0].trials) == (reps[1].inner_iters, reps[1].trials) and reps[0].trials > reps[0].inner_iters
+    assert reps[0].e_last == pytest.approx(reps[1].e_last, rel=1e-9)
+    assert rel_l2(outs[0], outs[1]) <= 1e-6
+
+
 @pytest.mark.parametrize("host_armijo", [False, True])
 @pytest.mark.parametrize("nx", [16, 128])
 def test_tv_prox_degenerate_cases(torch, cbct, host_armijo, nx):
