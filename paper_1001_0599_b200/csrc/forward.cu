@@ -85,6 +85,45 @@ __global__ void stage_volume_packed_kernel(const float *__restrict__ in, float2 
     }
 }
 
+// The same copy with 16-byte accesses on both sides (nx % 4 == 0, nzP even): a block takes one j, 64 voxels in i and 32
+// cells in kk; a half warp reads a 256-byte row of the volume with one float4 per lane, and writes 32 consecutive cells of a
+// staged column (256 bytes) with one float4 = two cells per lane.  Ten times fewer instructions per cell than the kernel
+// above, which was issue bound (0.054 ms at 256^3, 36 M warp instructions).
+constexpr int STG_I = 64, STG_K = 32;
+__global__ void __launch_bounds__(256)
+stage_volume_packed_vec_kernel(const float *__restrict__ in, float4 *__restrict__ stage2, int nx, int ny, int nz,
+                               int istride, int jstride)
+{
+    __shared__ float lo[STG_K][STG_I + 1], hi[STG_K][STG_I + 1];
+    const int j = blockIdx.z, i0 = blockIdx.x * STG_I, kk0 = blockIdx.y * STG_K;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    {
+        const int c = lane & 15, i = i0 + 4 * c;
+#pragma unroll
+        for (int pass = 0; pass < 2; ++pass) {
+            const int r = pass * 16 + warp * 2 + (lane >> 4);
+            const int k = kk0 + r - PAD_Z, km = nz - 1 - k;
+            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+            if (i < nx && k >= 0 && k < nz) {                    // km is in range exactly when k is
+                a = __ldg(reinterpret_cast<const float4 *>(in + ((size_t)k * ny + j) * nx + i));
+                b = __ldg(reinterpret_cast<const float4 *>(in + ((size_t)km * ny + j) * nx + i));
+            }
+            lo[r][4 * c + 0] = a.x; lo[r][4 * c + 1] = a.y; lo[r][4 * c + 2] = a.z; lo[r][4 * c + 3] = a.w;
+            hi[r][4 * c + 0] = b.x; hi[r][4 * c + 1] = b.y; hi[r][4 * c + 2] = b.z; hi[r][4 * c + 3] = b.w;
+        }
+    }
+    __syncthreads();
+    const int kl = 2 * (lane & 15), kk = kk0 + kl;               // this lane's two cells
+#pragma unroll
+    for (int pass = 0; pass < 4; ++pass) {
+        const int il = pass * 16 + warp * 2 + (lane >> 4), ii = i0 + il;
+        if (ii < nx && kk < jstride) {                          // jstride = nzP is even: kk + 1 < nzP too
+            const size_t cell = (size_t)(ii + PAD_M) * istride + (size_t)(j + PAD_M) * jstride + kk;
+            stage2[cell >> 1] = make_float4(lo[kl][il], hi[kl][il], lo[kl + 1][il], hi[kl + 1][il]);
+        }
+    }
+}
+
 constexpr int FWD_BV = 32, FWD_BU = 8;      // block: 32 detector rows (lanes) x 8 detector columns
 #ifndef FWD_MINB
 #define FWD_MINB 2
@@ -323,9 +362,15 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         StageTimer t(g, st, ST_TRANSPOSE);
         dim3 tb(32, 8);
         if (P.nmir == 2) {
-            dim3 tg((P.nx + 31) / 32, (P.nzP + 31) / 32, P.ny);
-            stage_volume_packed_kernel<<<tg, tb, 0, st>>>(d_vol, reinterpret_cast<float2 *>(L.d_stage), P.nx, P.ny, P.nz,
-                                                         P.istride, P.jstride);
+            if (P.nx % 4 == 0 && P.nzP % 2 == 0 && (uintptr_t)d_vol % 16 == 0) {
+                dim3 tg((P.nx + STG_I - 1) / STG_I, (P.nzP + STG_K - 1) / STG_K, P.ny);
+                stage_volume_packed_vec_kernel<<<tg, 256, 0, st>>>(d_vol, reinterpret_cast<float4 *>(L.d_stage), P.nx, P.ny, P.nz,
+                                                                    P.istride, P.jstride);
+            } else {
+                dim3 tg((P.nx + 31) / 32, (P.nzP + 31) / 32, P.ny);
+                stage_volume_packed_kernel<<<tg, tb, 0, st>>>(d_vol, reinterpret_cast<float2 *>(L.d_stage), P.nx, P.ny, P.nz,
+                                                             P.istride, P.jstride);
+            }
         } else {
             dim3 tg((P.nx + 31) / 32, (P.nz + 31) / 32, P.ny);
             stage_volume_kernel<<<tg, tb, 0, st>>>(d_vol, L.d_stage, P.nx, P.ny, P.nz, P.istride, P.jstride);
