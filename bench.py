@@ -504,6 +504,10 @@ def run_ours(args):
                 "frac": bpv * nvox / t / 1e9 / hbm_peak, "bytes_per_voxel": bpv, "peak_source": peak_src}
     if coop_prox:
         per["tv_prox"] = per["tv_grad"]
+    if per["transpose"]["ms_per_launch"]:       # the staging copy: reads the volume, writes the padded z-fastest copy
+        t = per["transpose"]["ms_per_launch"] / 1e3
+        kern["transpose"] = {"bound": "hbm", "achieved": 8.0 * nvox / t / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": 8.0 * nvox / t / 1e9 / hbm_peak, "bytes_per_voxel": 8.0, "peak_source": peak_src}
     for name in kern:
         if name in counters:                    # the tracked capture is of this workload and of these kernel sources
             kern[name]["ncu"] = counters[name]

@@ -375,7 +375,7 @@ static void launch_back_rm(const LevelParams &P, const Level &L, const float *sr
 }
 
 // The z-unit of a sharded back-projection: the slices one block of the level's kernel covers along z.
-int back_zunit(const Level &L) { return L.bt.ok ? 32 : 32 * back_kt(L.p); }
+int back_zunit(const Level &L) { return L.bt.ok ? 32 * L.bt.ZV : 32 * back_kt(L.p); }
 int back_nzunits(const Level &L)
 {
     const int nzh = L.p.nz / L.p.nmir, u = back_zunit(L);

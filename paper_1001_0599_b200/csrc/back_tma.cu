@@ -110,54 +110,74 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
 // its two z-planes are crossed in a known order -- plane zlo + oA first, oA = 1 when q > 0 -- and rows with v > 0 clip to
 // weight 0 by the same expressions.  A lane whose rows all lie below the detector (the
 // truncated bottom of the volume) does nothing.
-template <int SG, int NSLOT, int TP>
-__device__ __forceinline__ void bt_visit(float (&acc)[8], const BtConsts &C, float zlo, float zhi, const float4 e0, const float4 e1,
+template <int SG, int NSLOT, int TP, int ZV>
+__device__ __forceinline__ void bt_visit(float (&acc)[ZV][8], const BtConsts &C, const float (&zlo)[ZV], const float4 e0, const float4 e1,
                                          int r0A)
 {
-    const int r = __float2int_ru(fmaf(zlo, e1.y, C.c0v_m));
-    if (r + NSLOT <= 0) return;
-    const int rr = r - r0A;
-    CBCT_DEV_ASSERT(rr >= 0 && rr + NSLOT - 1 <= C.rr_max);
-    const float e = e0.z;
-    const float zA = zlo + e1.w, zB = zhi - e1.w;
-    const uint32_t colA = (uint32_t)__float_as_int(e1.z);
-    // byte offset of row rr in its column: rr / 2 entries into the plane of its parity, the odd plane shifted by one entry
-    uint32_t off, d1;
-    if (TP == 2) {
-        const int p = rr & 1;
-        off = rr * 8 + p * C.plane_step8;              // (rr >> 1) * 16 + p * (plane_bytes + 16)
-        d1 = p ? C.step_odd : C.step_even;             // to row rr + 1: the other plane
-    } else {
-        off = rr << 4;
-        d1 = 16;
+    int r[ZV];
+    bool any = false;
+#pragma unroll
+    for (int v = 0; v < ZV; ++v) {
+        r[v] = __float2int_ru(fmaf(zlo[v], e1.y, C.c0v_m));
+        any = any || r[v] + NSLOT > 0;
     }
-    const uint32_t aA = colA + off, aB = colA + C.KB - off;
-    const float rf = (float)r;
+    if (!any) return;                   // every row of this lane's voxels lies below the detector (zero-filled rows otherwise)
+    const float e = e0.z;
+    const uint32_t colA = (uint32_t)__float_as_int(e1.z);
+    float w[ZV][NSLOT];
+    uint32_t aA[ZV], aB[ZV], d1[ZV];
+#pragma unroll
+    for (int v = 0; v < ZV; ++v) {
+        const int rr = r[v] - r0A;
+        CBCT_DEV_ASSERT(rr >= 0 && rr + NSLOT - 1 <= C.rr_max);
+        const float zA = zlo[v] + e1.w, zB = zlo[v] + 1.0f - e1.w;
+        // byte offset of row rr in its column: rr / 2 entries into the plane of its parity, the odd plane shifted by one entry
+        uint32_t off;
+        if (TP == 2) {
+            const int p = rr & 1;
+            off = rr * 8 + p * C.plane_step8;              // (rr >> 1) * 16 + p * (plane_bytes + 16)
+            d1[v] = p ? C.step_odd : C.step_even;          // to row rr + 1: the other plane
+        } else {
+            off = rr << 4;
+            d1[v] = 16;
+        }
+        aA[v] = colA + off; aB[v] = colA + C.KB - off;
+        const float rf = (float)r[v];
+#pragma unroll
+        for (int s = 0; s < NSLOT; ++s) {
+            // v from one rounding of r dv + v0 (it cancels to a fraction of a pixel at the centre of the detector, and the
+            // crossing parameter amplifies its relative error by the source distance in slabs); v != 0: even row count, centred
+            const float inv = rcp_approx(fmaf(rf + (float)s, C.dv, C.v0) * e0.w);
+            const float qa = fmaf(zA, inv, -e), qb = fmaf(zB, inv, -e);
+            w[v][s] = fmaxf(fminf(qb, e0.y) - fmaxf(qa, e0.x), 0.0f);
+        }
+    }
 #pragma unroll
     for (int s = 0; s < NSLOT; ++s) {
-        // v from one rounding of r dv + v0 (it cancels to a fraction of a pixel at the centre of the detector, and the
-        // crossing parameter amplifies its relative error by the source distance in slabs); v != 0: even row count, centred
-        const float inv = rcp_approx(fmaf(rf + (float)s, C.dv, C.v0) * e0.w);
-        const float qa = fmaf(zA, inv, -e), qb = fmaf(zB, inv, -e);
-        const float w = fmaxf(fminf(qb, e0.y) - fmaxf(qa, e0.x), 0.0f);
-        const uint32_t os = TP == 2 ? (s & 1) * d1 + (s >> 1) * 16 : 16 * s;
-        if (s < NSLOT - 1 || w > 0.0f) {
-            const float4 tA = lds128(aA + os);
-            const float4 tB = lds128(aB - os);
-            acc[(SG + 0) % 4] = fmaf(w, tA.x, acc[(SG + 0) % 4]);
-            acc[(SG + 1) % 4] = fmaf(w, tA.y, acc[(SG + 1) % 4]);
-            acc[(SG + 2) % 4] = fmaf(w, tA.z, acc[(SG + 2) % 4]);
-            acc[(SG + 3) % 4] = fmaf(w, tA.w, acc[(SG + 3) % 4]);
-            acc[4 + (SG + 0) % 4] = fmaf(w, tB.x, acc[4 + (SG + 0) % 4]);
-            acc[4 + (SG + 1) % 4] = fmaf(w, tB.y, acc[4 + (SG + 1) % 4]);
-            acc[4 + (SG + 2) % 4] = fmaf(w, tB.z, acc[4 + (SG + 2) % 4]);
-            acc[4 + (SG + 3) % 4] = fmaf(w, tB.w, acc[4 + (SG + 3) % 4]);
+#pragma unroll
+        for (int v = 0; v < ZV; ++v) {
+            const uint32_t os = TP == 2 ? (s & 1) * d1[v] + (s >> 1) * 16 : 16 * s;
+            if (s < NSLOT - 1 || w[v][s] > 0.0f) {
+                const float4 tA = lds128(aA[v] + os);
+                const float4 tB = lds128(aB[v] - os);
+                const float ww = w[v][s];
+                acc[v][(SG + 0) % 4] = fmaf(ww, tA.x, acc[v][(SG + 0) % 4]);
+                acc[v][(SG + 1) % 4] = fmaf(ww, tA.y, acc[v][(SG + 1) % 4]);
+                acc[v][(SG + 2) % 4] = fmaf(ww, tA.z, acc[v][(SG + 2) % 4]);
+                acc[v][(SG + 3) % 4] = fmaf(ww, tA.w, acc[v][(SG + 3) % 4]);
+                acc[v][4 + (SG + 0) % 4] = fmaf(ww, tB.x, acc[v][4 + (SG + 0) % 4]);
+                acc[v][4 + (SG + 1) % 4] = fmaf(ww, tB.y, acc[v][4 + (SG + 1) % 4]);
+                acc[v][4 + (SG + 2) % 4] = fmaf(ww, tB.z, acc[v][4 + (SG + 2) % 4]);
+                acc[v][4 + (SG + 3) % 4] = fmaf(ww, tB.w, acc[v][4 + (SG + 3) % 4]);
+            }
         }
     }
 }
 
 // R == 4, M == 2 only (square centred in-plane grid with quarter-turn views, volume and detector centred in z / v).
-template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
+// ZV = voxels per lane along z: a block owns 32 ZV slices of the lower half volume (lane l: slices k0 + l, k0 + 32 + l).  With
+// ZV = 2 the in-plane lists, the stage headers and the 4 n_base barrier handshakes of a block serve twice the voxels.
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV>
 __global__ void __launch_bounds__((BI * BJ / CPW + 1) * 32, MINB)
 back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const BtParams Q,
                 const RayU *__restrict__ rayu, const ViewC *__restrict__ views, const float *__restrict__ f, float coef,
@@ -169,7 +189,8 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
     extern __shared__ __align__(1024) char smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // the slices nearest to the central plane first: the truncated bottom bricks are the cheap ones and fill the tail
-    const int i0 = blockIdx.x * BI, j0 = blockIdx.y * BJ, k0 = (kb_top - 1 - blockIdx.z) * 32;     // kb_top: one past the last 32-slice unit of this launch
+    constexpr int ZPB = 32 * ZV;                       // slices per block
+    const int i0 = blockIdx.x * BI, j0 = blockIdx.y * BJ, k0 = (kb_top - 1 - blockIdx.z) * ZPB;     // kb_top: one past the last z-unit of this launch
     const int ni = P.nx / 2, nj = P.ny / 2, n1 = P.nx - 1;
     const int n_stages = 4 * P.nbase;
 
@@ -189,11 +210,13 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
     C.step_even = Q.plane_bytes + 16; C.step_odd = 16 - (Q.plane_bytes + 16);
     C.KB = Q.half_bytes + (TP == 2 ? Q.plane_bytes : 0) + (Q.XB - 1) * 16;
 
-    float acc[CPW][8];
+    float acc[CPW][ZV][8];
 #pragma unroll
     for (int cp = 0; cp < CPW; ++cp)
 #pragma unroll
-        for (int q = 0; q < 8; ++q) acc[cp][q] = 0.0f;
+        for (int v = 0; v < ZV; ++v)
+#pragma unroll
+            for (int q = 0; q < 8; ++q) acc[cp][v][q] = 0.0f;
 
     // ---------------- every stage's detector rectangle, by all warps, before the ring starts ----------------
     // header = (skip, first detector column, first row of the A window, columns)
@@ -222,7 +245,7 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
         }
         // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
         // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
-        const int klast = min(k0 + 31, Q.nzh - 1);
+        const int klast = min(k0 + ZPB - 1, Q.nzh - 1);
         const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
         const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
         const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
@@ -274,11 +297,11 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
     } else {
         // ---------------- consumers ----------------
         float4 *__restrict__ l0 = reinterpret_cast<float4 *>(smem + Q.list_off) + warp * 64, *__restrict__ l1 = l0 + 32;
-        const int kv = k0 + lane;
-        const float zlo = (float)(min(kv, Q.nzh - 1) - P.cz) - P.sz;
+        float zlo[ZV];
+#pragma unroll
+        for (int v = 0; v < ZV; ++v) zlo[v] = (float)(min(k0 + 32 * v + lane, Q.nzh - 1) - P.cz) - P.sz;
         uint32_t tile0 = smem_u32(smem);
         asm volatile("" : "+r"(tile0));                 // keep the window address in a register
-        const float zhi = zlo + 1.0f;
         // this lane's candidate in a list round: unit u = lane / 8 -> (stage of the round, column of the warp), candidate lane % 8
         const int u = lane >> 3, cnd = lane & 7;
         const int my_cp = u % CPW, my_t = u / CPW;
@@ -338,10 +361,10 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                             const int n_u = __popc(hit & (0xffu << (8 * uu)));
                             for (int n = 0; n < n_u; ++n) {
                                 const float4 E0 = l0[uu * 8 + n], E1 = l1[uu * 8 + n];
-                                if (sg == 0) bt_visit<0, NSLOT, TP>(acc[cp], C, zlo, zhi, E0, E1, hdr.z);
-                                else if (sg == 1) bt_visit<1, NSLOT, TP>(acc[cp], C, zlo, zhi, E0, E1, hdr.z);
-                                else if (sg == 2) bt_visit<2, NSLOT, TP>(acc[cp], C, zlo, zhi, E0, E1, hdr.z);
-                                else bt_visit<3, NSLOT, TP>(acc[cp], C, zlo, zhi, E0, E1, hdr.z);
+                                if (sg == 0) bt_visit<0, NSLOT, TP, ZV>(acc[cp], C, zlo, E0, E1, hdr.z);
+                                else if (sg == 1) bt_visit<1, NSLOT, TP, ZV>(acc[cp], C, zlo, E0, E1, hdr.z);
+                                else if (sg == 2) bt_visit<2, NSLOT, TP, ZV>(acc[cp], C, zlo, E0, E1, hdr.z);
+                                else bt_visit<3, NSLOT, TP, ZV>(acc[cp], C, zlo, E0, E1, hdr.z);
                             }
                         }
                     }
@@ -354,7 +377,7 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
 
     // ---------------- results: through shared memory into x-fastest order, then g = f - coef b (A4) ----------------
     __syncthreads();        // every tile has been consumed; the ring is free
-    float *s_out = reinterpret_cast<float *>(smem);      // [image 8][k 32][rows of the image's footprint][its columns]
+    float *s_out = reinterpret_cast<float *>(smem);      // [image 8][k ZPB][rows of the image's footprint][its columns]
     if (warp < NW) {
 #pragma unroll
         for (int cp = 0; cp < CPW; ++cp) {
@@ -365,16 +388,17 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                 const int wr = (r & 1) ? BJ : BI;                                  // footprint width of image r
                 const int xl = r == 0 ? ii : r == 1 ? BJ - 1 - jj : r == 2 ? BI - 1 - ii : jj;
                 const int yl = r == 0 ? jj : r == 1 ? ii : r == 2 ? BJ - 1 - jj : BI - 1 - ii;
-                s_out[(img * 32 + lane) * NIJ + yl * wr + xl] = acc[cp][img];
+#pragma unroll
+                for (int v = 0; v < ZV; ++v) s_out[(img * ZPB + 32 * v + lane) * NIJ + yl * wr + xl] = acc[cp][v][img];
             }
         }
     }
     __syncthreads();
     const bool full_brick = i0 + BI <= ni && j0 + BJ <= nj;
     if (Q.vec4 && full_brick) {
-        constexpr int NV4 = 8 * 32 * NIJ / 4;
+        constexpr int NV4 = 8 * ZPB * NIJ / 4;
         for (int e4 = threadIdx.x; e4 < NV4; e4 += blockDim.x) {
-            const int e = e4 * 4, img = e / (32 * NIJ), k = (e / NIJ) % 32, w = e % NIJ;
+            const int e = e4 * 4, img = e / (ZPB * NIJ), k = (e / NIJ) % ZPB, w = e % NIJ;
             const int r = img & 3, wr = (r & 1) ? BJ : BI, yl = w / wr, xl = w % wr;
             const int kk = k0 + k;
             if (kk >= Q.nzh) continue;
@@ -390,9 +414,9 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
             *reinterpret_cast<float4 *>(out + o) = v;
         }
     } else {
-        constexpr int NE = 8 * 32 * NIJ;
+        constexpr int NE = 8 * ZPB * NIJ;
         for (int e = threadIdx.x; e < NE; e += blockDim.x) {
-            const int img = e / (32 * NIJ), k = (e / NIJ) % 32, w = e % NIJ;
+            const int img = e / (ZPB * NIJ), k = (e / NIJ) % ZPB, w = e % NIJ;
             const int r = img & 3, wr = (r & 1) ? BJ : BI, yl = w / wr, xl = w % wr;
             // back to the brick's own column (ii, jj): is it inside the quadrant?
             const int ii = r == 0 ? xl : r == 1 ? yl : r == 2 ? BI - 1 - xl : BI - 1 - yl;
@@ -428,13 +452,13 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB>
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV>
 cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out, unsigned int *errflag, cudaStream_t st,
                       const Shard *sh)
 {
     const LevelParams &P = L.p;
     const BtPlan &B = L.bt;
-    auto kern = back_tma_kernel<BI, BJ, CPW, NSLOT, TP, MINB>;
+    auto kern = back_tma_kernel<BI, BJ, CPW, NSLOT, TP, MINB, ZV>;
     static bool attr_set = false;       // per instantiation; the value only grows
     static int attr_bytes = 0;
     if (!attr_set || B.q.total > attr_bytes) {
@@ -442,7 +466,7 @@ cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out
         attr_set = true; attr_bytes = B.q.total;
     }
     const int ni = P.nx / 2, nj = P.ny / 2;
-    dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 31) / 32), b((BI * BJ / CPW + 1) * 32);
+    dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 32 * ZV - 1) / (32 * ZV)), b((BI * BJ / CPW + 1) * 32);
     int kb_top = gr.z;
     if (sh) { kb_top = sh->zu_hi; gr.z = sh->zu_hi - sh->zu_lo; if (gr.z == 0) return CBCT_OK; }
     kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag, kb_top);
@@ -475,7 +499,7 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     const double c0v_m = -(-0.5 * (P.nv - 1) * L.dv + d.det_off_v) / L.dv - 2.0e-3;
     // the first-quadrant bricks under every view = their four images under the base views
     double len_max = 0.0;
-    int span_max = 0, ncols_max = 0;
+    int span_max[2] = {0, 0}, ncols_max = 0;            // row span of a block of 32 / 64 slices
     for (int a = 0; a < P.np; ++a) {
         const double c = cos(g->angles[a]), s = sin(g->angles[a]);
         const double dn = 1.01 * 0.5 * (fabs(c) * L.hx + fabs(s) * L.hy), du = 1.003 * 0.5 * (fabs(s) * L.hx + fabs(c) * L.hy);
@@ -498,43 +522,54 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
                 // rows of one voxel (lowest slice, nearest depth of the brick) and of the brick's lowest 32 slices
                 const double len = K * ((double)nzh / (rn_lo - dn) - (double)(nzh - 1) / (rn_lo + dn)) + 5.0e-3;
                 if (len > len_max) len_max = len;
-                const int klast = nzh < 32 ? nzh - 1 : 31;
                 const double rfirst = ceil(-(double)nzh * K / (rn_lo - dn) + c0v_m) - 1.0;
-                const double rlast = ceil(-(double)(nzh - klast) * K / (rn_hi + dn) + c0v_m);
-                if ((int)(rlast - rfirst) > span_max) span_max = (int)(rlast - rfirst);
+                for (int zv = 1; zv <= 2; ++zv) {
+                    const int klast = nzh < 32 * zv ? nzh - 1 : 32 * zv - 1;
+                    const double rlast = ceil(-(double)(nzh - klast) * K / (rn_hi + dn) + c0v_m);
+                    if ((int)(rlast - rfirst) > span_max[zv - 1]) span_max[zv - 1] = (int)(rlast - rfirst);
+                }
             }
     }
     const int nslot = (int)floor(len_max) + 1;
     if (nslot > 4) return CBCT_OK;
     const int NSLOT = nslot <= 2 ? 2 : nslot;
     const int TP = (K / d.sad >= 1.5 && P.nv % 2 == 0) ? 2 : 1;
-    // window: rows rfirst .. rlast + NSLOT, one row of alignment, the odd plane's shift, and a row of margin at each end
-    const int rows = span_max + NSLOT + 1 + 1 + (TP == 2 ? 3 : 1) + 2;
-    const int XB = ((rows + TP - 1) / TP + 7) / 8 * 8;
-    if (2 * XB > 256) return CBCT_OK;
     const int ncols = ncols_max + 1;
     if (ncols >= (1 << BT_NMAPS)) return CBCT_OK;
-
+    // Voxels per lane along z.  Two (blocks of 64 slices: the lists, headers and handshakes of a block serve twice the voxels, but
+    // 96 registers and a doubled tile window: one block per SM) measured 0.888 ms against 0.831 ms at config 3, parity green:
+    // the 17 resident warps hide less latency than the halved overhead saves.  One is the default; -DBT_ZV_MAX=2 builds the other.
+#ifndef BT_ZV_MAX
+#define BT_ZV_MAX 1
+#endif
     BtParams &q = B.q;
-    q.XB = XB; q.ncols = ncols; q.nzh = nzh;
-    q.plane_bytes = ncols * XB * 16;
-    q.half_bytes = TP * q.plane_bytes;
-    q.stage_bytes = 2 * q.half_bytes;
+    int ZV = 0, XB = 0;
+    for (int zv = (nzh >= 64 ? BT_ZV_MAX : 1); zv >= 1 && !ZV; --zv) {
+        // window: rows rfirst .. rlast + NSLOT, one row of alignment, the odd plane's shift, and a row of margin at each end
+        const int rows = span_max[zv - 1] + NSLOT + 1 + 1 + (TP == 2 ? 3 : 1) + 2;
+        XB = ((rows + TP - 1) / TP + 7) / 8 * 8;
+        if (2 * XB > 256) continue;
+        q.XB = XB; q.ncols = ncols; q.nzh = nzh;
+        q.plane_bytes = ncols * XB * 16;
+        q.half_bytes = TP * q.plane_bytes;
+        q.stage_bytes = 2 * q.half_bytes;
+        const int nw = BI * BJ;
+        int off = BT_NST * q.stage_bytes;
+        const int out_bytes = 8 * 32 * zv * BI * BJ * 4;
+        if (off < out_bytes) off = out_bytes;
+        q.list_off = off; off += nw * 64 * 16;
+        q.view_off = off; off += P.nbase * 16;
+        q.hdr_off = off; off += 4 * P.nbase * 16;
+        q.bar_off = off; off += 2 * BT_NST * 8;
+        q.total = off;
+        if (q.total <= 227 * 1024) ZV = zv;
+    }
+    if (!ZV) return CBCT_OK;
     q.ic_scale = (float)K;
     q.c0v_m = (float)c0v_m;
-    const int nw = BI * BJ;
-    int off = BT_NST * q.stage_bytes;
-    const int out_bytes = 8 * 32 * BI * BJ * 4;
-    if (off < out_bytes) off = out_bytes;
-    q.list_off = off; off += nw * 64 * 16;
-    q.view_off = off; off += P.nbase * 16;
-    q.hdr_off = off; off += 4 * P.nbase * 16;
-    q.bar_off = off; off += 2 * BT_NST * 8;
-    q.total = off;
     q.vec4 = (P.nx % 4 == 0 && BI % 4 == 0 && BJ % 4 == 0) ? 1 : 0;
-    if (q.total > 227 * 1024) return CBCT_OK;
-    B.BI = BI; B.BJ = BJ; B.CPW = 1; B.NSLOT = NSLOT; B.TP = TP;
-    B.minb = 2 * (q.total + 1024) <= 228 * 1024 ? 2 : 1;
+    B.BI = BI; B.BJ = BJ; B.CPW = 1; B.NSLOT = NSLOT; B.TP = TP; B.ZV = ZV;
+    B.minb = (ZV == 1 && 2 * (q.total + 1024) <= 228 * 1024) ? 2 : 1;
 
     // the residual stack as a 4-d tensor of 8-byte elements: (2 x entry index within a plane, plane, column, base view)
     const int tXP = P.nv / TP;
@@ -560,8 +595,9 @@ cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float 
     cbct_status s = CBCT_ERR_INVALID_ARG;
 #define BT_CASE(NS, TPV)                                                                                         \
     if (B.NSLOT == NS && B.TP == TPV)                                                                            \
-        s = B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2>(L, d_f, coef, d_out, g->d_errflag, st, sh)               \
-                        : bt_launch<4, 4, 1, NS, TPV, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh);
+        s = B.ZV == 2 ? bt_launch<4, 4, 1, NS, TPV, 1, 2>(L, d_f, coef, d_out, g->d_errflag, st, sh)              \
+          : B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh)            \
+                        : bt_launch<4, 4, 1, NS, TPV, 1, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh);
     BT_CASE(2, 1) BT_CASE(3, 1) BT_CASE(4, 1) BT_CASE(2, 2) BT_CASE(3, 2) BT_CASE(4, 2)
 #undef BT_CASE
     if (s != CBCT_OK) return s == CBCT_ERR_INVALID_ARG ? cbct_fail(s, "launch_back_tma: no kernel for this plan") : s;

@@ -76,7 +76,7 @@ struct BtParams {
 struct BtConsts { float c0v_m, dv, v0; int rr_max, plane_step8, step_even, step_odd, KB; };
 struct BtPlan {
     bool ok = false;
-    int BI = 0, BJ = 0, CPW = 0, NSLOT = 0, TP = 1, minb = 1;
+    int BI = 0, BJ = 0, CPW = 0, NSLOT = 0, TP = 1, minb = 1, ZV = 1;    // ZV: voxels per lane along z (blocks of 32 ZV slices)
     BtParams q;
     BtMaps maps;
 };

@@ -22,7 +22,8 @@ CSRC = os.path.join(HERE, "csrc")
 # kernel-name prefix -> bench.py's stage name
 STAGES = {"forward_kernel": "forward", "back_tma_kernel": "back", "back_list_kernel": "back", "back_kernel": "back",
           "tv_grad_kernel": "tv_grad", "tv_energy_kernel": "tv_trial", "tv_update_kernel": "tv_update",
-          "stage_volume_packed_kernel": "transpose", "stage_volume_kernel": "transpose", "tv_first_kernel": "tv_first"}
+          "stage_volume_packed_kernel": "transpose", "stage_volume_packed_vec_kernel": "transpose",
+          "stage_volume_kernel": "transpose", "tv_prox_coop_kernel": "tv_prox"}
 METRICS = {
     "gpu__time_duration.sum": "ncu_duration_us",
     "dram__bytes_read.sum": "dram_read_bytes",
