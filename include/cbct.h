@@ -76,6 +76,10 @@ typedef struct {
 #define CBCT_KERNEL_HOST_ARMIJO 2 /* cbct_tv_prox sequenced by the host (one stream synchronisation per Armijo trial) instead
                                      of the single cooperative kernel that takes every accept / shrink / stop decision on
                                      the device; same passes, same decisions.  For A/B measurements and tests. */
+#define CBCT_KERNEL_BACK_LISTS_ON_THE_FLY 8 /* the TMA back-projector works out the in-plane part of its (voxel column, detector
+                                              column) pairs at the start of every base view instead of reading the table
+                                              cbct_geometry_create builds once (512 bytes per first-quadrant voxel column and
+                                              base view); same bits either way.  For A/B measurements and tests. */
 #define CBCT_KERNEL_TV_SCALAR_TILES 4 /* the TV passes always on the 32-voxel warp tiles (one voxel per lane), never on the
                                          16-byte tiles that volumes with nx % 4 == 0, nx >= 128 and 16-byte aligned buffers
                                          otherwise take; same stencil, for A/B measurements and tests. */

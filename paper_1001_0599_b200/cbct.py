@@ -189,7 +189,7 @@ class Geometry:
     """
 
     def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False, host_armijo: bool = False,
-                 tv_scalar_tiles: bool = False):
+                 tv_scalar_tiles: bool = False, back_lists_on_the_fly: bool = False):
         lib = load_library()
         self._h = C.c_void_p()
         self.desc = desc
@@ -206,8 +206,9 @@ class Geometry:
         d.angles_rad = ang.ctypes.data_as(C.POINTER(C.c_double))
         d.bc_xy, d.bc_z, d.max_levels = desc.bc_xy, desc.bc_z, self.max_levels
         d.no_symmetry = int(bool(no_symmetry))
-        # CBCT_KERNEL_NO_TMA | CBCT_KERNEL_HOST_ARMIJO | CBCT_KERNEL_TV_SCALAR_TILES
-        d.kernel_flags = (1 if no_tma else 0) | (2 if host_armijo else 0) | (4 if tv_scalar_tiles else 0)
+        # CBCT_KERNEL_NO_TMA | CBCT_KERNEL_HOST_ARMIJO | CBCT_KERNEL_TV_SCALAR_TILES | CBCT_KERNEL_BACK_LISTS_ON_THE_FLY
+        d.kernel_flags = ((1 if no_tma else 0) | (2 if host_armijo else 0) | (4 if tv_scalar_tiles else 0) |
+                          (8 if back_lists_on_the_fly else 0))
         _check(lib.cbct_geometry_create(C.byref(d), C.byref(self._h)))
 
     def close(self):
@@ -491,8 +492,8 @@ def gather_ceiling(buf, variant: int, reuse: int = 1, iters: int = 64, stream=No
 
 
 def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False,
-                    host_armijo: bool = False, tv_scalar_tiles: bool = False) -> Geometry:
-    return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo, tv_scalar_tiles)
+                    host_armijo: bool = False, tv_scalar_tiles: bool = False, back_lists_on_the_fly: bool = False) -> Geometry:
+    return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo, tv_scalar_tiles, back_lists_on_the_fly)
 
 
 def version() -> str:

@@ -110,6 +110,61 @@ __device__ __forceinline__ float4 lds128(uint32_t addr)
 // its two z-planes are crossed in a known order -- plane zlo + oA first, oA = 1 when q > 0 -- and rows with v > 0 clip to
 // weight 0 by the same expressions.  A lane whose rows all lie below the detector (the
 // truncated bottom of the volume) does nothing.
+// The in-plane part of (voxel column (vi0, vj0) of the first quadrant, base view, image sg, candidate detector column cnd of the
+// image's shadow): e0 = (s_lo, s_hi, e, q), e1 = (-, 1/c, -, oA) as bt_visit reads them, and the detector column iu.  One
+// definition for the list rounds of the kernel and for the table built once per geometry (bt_build_lists_kernel): the two
+// hold the same bits.
+__device__ __forceinline__ bool bt_list_entry(const LevelParams &P, const float4 vw, const RayU *__restrict__ rayu, int a, int vi0,
+                                              int vj0, int n1, int sg, int cnd, float4 &e0, float4 &e1, int &iu)
+{
+    int mi, mj, iu_lo, iu_hi;
+    float rn;
+    bt_image(sg, vi0, vj0, n1, mi, mj);
+    bt_shadow(P, vw, mi, mj, iu_lo, iu_hi, rn);
+    CBCT_DEV_ASSERT(iu_hi - iu_lo + 1 <= BT_MAXC);
+    if (cnd > iu_hi - iu_lo) return false;
+    iu = iu_lo + cnd;
+    const RayU r = load_rayu(rayu, a * P.nu + iu);
+    const float bx = (float)(mi - P.cx), by = (float)(mj - P.cy);
+    const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;
+    const float y0 = fmaf(d0, r.m, r.a0);
+    const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
+    const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
+    const float e = d0 - r.sd;
+    const float icA = rcp_approx(r.q * (e + s_lo)), icB = rcp_approx(r.q * (e + s_hi));
+    e0 = make_float4(s_lo, s_hi, e, r.q);
+    e1 = make_float4(0.0f, fmaxf(icA, icB) * P.inv_dv, 0.0f, r.q > 0.0f ? 1.0f : 0.0f);
+    return s_hi > s_lo;
+}
+
+// The list table: for every first-quadrant voxel column and base view, BT_TABH entries per image in candidate order
+// (32 float4 = 512 bytes: entry (sg, n) at float4 2 (4 sg + n) and the next), the count of an image in the .x of its first
+// entry's second half, the detector column in the .z.  One warp per (column, base view); *overflow counts images with more hits.
+constexpr int BT_TABH = 4;
+__global__ void bt_build_lists_kernel(const LevelParams P, const RayU *__restrict__ rayu, const ViewC *__restrict__ views,
+                                      float4 *__restrict__ table, unsigned int *__restrict__ overflow)
+{
+    const int lane = threadIdx.x & 31, w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int ni = P.nx / 2, nj = P.ny / 2;
+    if (w >= ni * nj * P.nbase) return;
+    const int a = w % P.nbase, colidx = w / P.nbase, vi0 = colidx % ni, vj0 = colidx / ni;
+    const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + a);
+    const int sg = lane >> 3, cnd = lane & 7;
+    float4 e0 = make_float4(0.f, 0.f, 0.f, 0.f), e1 = e0;
+    int iu = 0;
+    const bool ok = bt_list_entry(P, vw, rayu, a, vi0, vj0, P.nx - 1, sg, cnd, e0, e1, iu);
+    const unsigned hit = __ballot_sync(0xffffffffu, ok);
+    const unsigned grp = hit & (0xffu << (8 * sg));
+    const int rank = __popc(grp & ((1u << lane) - 1u)), cnt = __popc(grp);
+    if (cnt > BT_TABH && cnd == 0) atomicAdd(overflow, 1u);
+    if (ok && rank < BT_TABH) {
+        e1.z = __int_as_float(iu);
+        if (rank == 0) e1.x = __int_as_float(cnt);
+        float4 *t = table + (size_t)w * 32 + 2 * (BT_TABH * sg + rank);
+        t[0] = e0; t[1] = e1;
+    }
+}
+
 template <int SG, int NSLOT, int TP, int ZV>
 __device__ __forceinline__ void bt_visit(float (&acc)[ZV][8], const BtConsts &C, const float (&zlo)[ZV], const float4 e0, const float4 e1,
                                          int r0A)
@@ -174,14 +229,81 @@ __device__ __forceinline__ void bt_visit(float (&acc)[ZV][8], const BtConsts &C,
     }
 }
 
+// Detector rectangle of one stage (base view of vw, image sg) of the brick at (i0, j0), slices k0 .. k0 + 32 ZV - 1: header =
+// (skip, first detector column, first row of the A window, columns).  Warp-collective; one definition for the kernel and for
+// the table built once per geometry (bt_build_headers_kernel).  Bounds of create that do not hold are counted in *errflag.
+template <int BI, int BJ, int NSLOT, int TP, int ZV>
+__device__ __forceinline__ int4 bt_stage_header(const LevelParams &P, const BtParams &Q, const float4 vw, int i0, int j0, int k0, int sg,
+                                                int lane, unsigned int *errflag)
+{
+    constexpr int NIJ = BI * BJ;
+    const int ni = P.nx / 2, nj = P.ny / 2, n1 = P.nx - 1;
+    const int rr_max = TP * Q.XB - (TP == 2 ? 3 : 1);
+    int cmin = 1 << 30, cmax = -1;
+    float rn_lo = 3.0e38f, rn_hi = -3.0e38f;
+    for (int v = lane; v < NIJ; v += 32) {
+        const int i = i0 + v % BI, j = j0 + v / BI;
+        if (i < ni && j < nj) {
+            int mi, mj, lo, hi;
+            float rn;
+            bt_image(sg, i, j, n1, mi, mj);
+            bt_shadow(P, vw, mi, mj, lo, hi, rn);
+            if (lo <= hi) { cmin = min(cmin, lo); cmax = max(cmax, min(hi, lo + BT_MAXC - 1)); }
+            rn_lo = fminf(rn_lo, rn); rn_hi = fmaxf(rn_hi, rn);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        cmin = min(cmin, __shfl_xor_sync(0xffffffffu, cmin, o));
+        cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
+        rn_lo = fminf(rn_lo, __shfl_xor_sync(0xffffffffu, rn_lo, o));
+        rn_hi = fmaxf(rn_hi, __shfl_xor_sync(0xffffffffu, rn_hi, o));
+    }
+    // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
+    // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
+    const int klast = min(k0 + 32 * ZV - 1, Q.nzh - 1);
+    const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
+    const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
+    const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
+    const int rlast = __float2int_ru(fmaf(zl, ic_min, Q.c0v_m)) + NSLOT;
+    int ncols = cmax - cmin + 1;
+    const bool skip = ncols <= 0 || rlast < 0 || rmin > P.nv - 1;
+    const int x0 = TP == 2 ? (rmin >> 1) : rmin, r0A = TP * x0;
+    if (!skip && (ncols > Q.ncols || rlast - r0A > rr_max)) {   // the bounds of create do not hold: flag, stay in bounds
+        if (lane == 0) atomicAdd(errflag, 1u);
+        ncols = min(ncols, Q.ncols);
+    }
+    return make_int4(skip ? 1 : 0, cmin, r0A, ncols);
+}
+
+// The header table: [z-unit][brick row][brick column][stage], one warp per header.
+template <int BI, int BJ, int NSLOT, int TP, int ZV>
+__global__ void bt_build_headers_kernel(const LevelParams P, const BtParams Q, const ViewC *__restrict__ views, int gx, int gy, int gz,
+                                        int4 *__restrict__ table, unsigned int *__restrict__ errflag)
+{
+    const int lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int n_stages = 4 * P.nbase;
+    if (w >= (long long)gx * gy * gz * n_stages) return;
+    const int s = (int)(w % n_stages);
+    const long long b = w / n_stages;
+    const int bx = (int)(b % gx), by = (int)((b / gx) % gy), zu = (int)(b / ((long long)gx * gy));
+    const float4 vw = __ldg(reinterpret_cast<const float4 *>(views) + (s >> 2));
+    const int4 h = bt_stage_header<BI, BJ, NSLOT, TP, ZV>(P, Q, vw, bx * BI, by * BJ, zu * 32 * ZV, s & 3, lane, errflag);
+    if (lane == 0) table[w] = h;
+}
+
 // R == 4, M == 2 only (square centred in-plane grid with quarter-turn views, volume and detector centred in z / v).
 // ZV = voxels per lane along z: a block owns 32 ZV slices of the lower half volume (lane l: slices k0 + l, k0 + 32 + l).  With
 // ZV = 2 the in-plane lists, the stage headers and the 4 n_base barrier handshakes of a block serve twice the voxels.
-template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV>
+// LT: the in-plane lists come from the table bt_build_lists_kernel made at create (copied into the warp's list area by cp.async,
+// one base view ahead of the stages that read them) instead of being worked out by the lanes at the start of every base view.
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV, bool LT>
 __global__ void __launch_bounds__((BI * BJ / CPW + 1) * 32, MINB)
 back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const BtParams Q,
                 const RayU *__restrict__ rayu, const ViewC *__restrict__ views, const float *__restrict__ f, float coef,
-                float *__restrict__ out, unsigned int *__restrict__ errflag, int kb_top)
+                float *__restrict__ out, unsigned int *__restrict__ errflag, int kb_top, const float4 *__restrict__ lists,
+                const int4 *__restrict__ hdrs)
 {
     constexpr int NIJ = BI * BJ, NW = NIJ / CPW;      // voxel columns of the brick, consumer warps
     constexpr int SPR = 4 / CPW;                      // stages per list round: 32 lanes = SPR stages x CPW columns x 8 candidates
@@ -218,46 +340,15 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
 #pragma unroll
             for (int q = 0; q < 8; ++q) acc[cp][v][q] = 0.0f;
 
-    // ---------------- every stage's detector rectangle, by all warps, before the ring starts ----------------
-    // header = (skip, first detector column, first row of the A window, columns)
-    for (int s = warp; s < n_stages; s += NW + 1) {
-        const int a = s >> 2, sg = s & 3;
-        const float4 vw = s_view[a];
-        int cmin = 1 << 30, cmax = -1;
-        float rn_lo = 3.0e38f, rn_hi = -3.0e38f;
-        for (int v = lane; v < NIJ; v += 32) {
-            const int i = i0 + v % BI, j = j0 + v / BI;
-            if (i < ni && j < nj) {
-                int mi, mj, lo, hi;
-                float rn;
-                bt_image(sg, i, j, n1, mi, mj);
-                bt_shadow(P, vw, mi, mj, lo, hi, rn);
-                if (lo <= hi) { cmin = min(cmin, lo); cmax = max(cmax, min(hi, lo + BT_MAXC - 1)); }
-                rn_lo = fminf(rn_lo, rn); rn_hi = fmaxf(rn_hi, rn);
-            }
+    // ---------------- every stage's detector rectangle: from the table made at create, or by all warps, before the ring starts ----
+    if (LT && hdrs) {
+        const int4 *hb = hdrs + ((size_t)((kb_top - 1 - blockIdx.z) * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * n_stages;
+        for (int s = threadIdx.x; s < n_stages; s += blockDim.x) s_hdr[s] = __ldg(hb + s);
+    } else {
+        for (int s = warp; s < n_stages; s += NW + 1) {
+            const int4 h = bt_stage_header<BI, BJ, NSLOT, TP, ZV>(P, Q, s_view[s >> 2], i0, j0, k0, s & 3, lane, errflag);
+            if (lane == 0) s_hdr[s] = h;
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            cmin = min(cmin, __shfl_xor_sync(0xffffffffu, cmin, o));
-            cmax = max(cmax, __shfl_xor_sync(0xffffffffu, cmax, o));
-            rn_lo = fminf(rn_lo, __shfl_xor_sync(0xffffffffu, rn_lo, o));
-            rn_hi = fmaxf(rn_hi, __shfl_xor_sync(0xffffffffu, rn_hi, o));
-        }
-        // rows: v = z hz sdd / rn for a point at depth rn; the strip ends of a voxel lie within its half extent dn
-        // (vw.z, inflated) of its centre's depth.  First row of the lowest slice, last slot of the highest.
-        const int klast = min(k0 + ZPB - 1, Q.nzh - 1);
-        const float zf = (float)(k0 - P.cz) - P.sz, zl = (float)(klast - P.cz) - P.sz;
-        const float ic_max = Q.ic_scale / (rn_lo - vw.z) * 1.00001f, ic_min = Q.ic_scale / (rn_hi + vw.z) * 0.99999f;
-        const int rmin = __float2int_ru(fmaf(zf, ic_max, Q.c0v_m)) - 1;
-        const int rlast = __float2int_ru(fmaf(zl, ic_min, Q.c0v_m)) + NSLOT;
-        int ncols = cmax - cmin + 1;
-        const bool skip = ncols <= 0 || rlast < 0 || rmin > P.nv - 1;
-        const int x0 = TP == 2 ? (rmin >> 1) : rmin, r0A = TP * x0;
-        if (!skip && (ncols > Q.ncols || rlast - r0A > C.rr_max)) {   // the bounds of create do not hold: flag, stay in bounds
-            if (lane == 0) atomicAdd(errflag, 1u);
-            ncols = min(ncols, Q.ncols);
-        }
-        if (lane == 0) s_hdr[s] = make_int4(skip ? 1 : 0, cmin, r0A, ncols);
     }
     __syncthreads();
 
@@ -309,6 +400,45 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
         const int vi0 = i0 + col % BI, vj0 = j0 + col / BI;
         const bool col_ok = vi0 < ni && vj0 < nj;
         const unsigned lt_mask = (1u << lane) - 1u;
+        if constexpr (LT) {
+            static_assert(CPW == 1, "the list table holds one voxel column per warp");
+            // ---- lists from the table: 512 bytes per (column, base view), one 16-byte cp.async per lane, a base view ahead ----
+            const float4 *tab = lists + ((size_t)(vj0 * ni + vi0) * P.nbase) * 32 + lane;
+            const uint32_t lbuf = smem_u32(l0) + lane * 16;
+            if (col_ok) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(lbuf), "l"(tab) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            for (int a = 0; a < P.nbase; ++a) {
+                if (col_ok && a + 1 < P.nbase)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(lbuf + ((a + 1) & 1) * 512), "l"(tab + (size_t)(a + 1) * 32) : "memory");
+                asm volatile("cp.async.commit_group;" ::: "memory");
+                asm volatile("cp.async.wait_group 1;" ::: "memory");
+                __syncwarp();
+                const float4 *__restrict__ L = l0 + (a & 1) * 32;
+#pragma unroll
+                for (int sg = 0; sg < 4; ++sg) {
+                    const int s = 4 * a + sg, slot = s % BT_NST, use = s / BT_NST;
+                    mbar_wait(bar0 + 8 * slot, use & 1);
+                    const int4 hdr = s_hdr[s];
+                    if (!hdr.x && col_ok) {
+                        const int n_u = __float_as_int(L[2 * BT_TABH * sg + 1].x);
+                        const uint32_t col0 = tile0 + slot * Q.stage_bytes - hdr.y * (Q.XB * 16);
+                        for (int n = 0; n < n_u; ++n) {
+                            const float4 E0 = L[2 * (BT_TABH * sg + n)];
+                            float4 E1 = L[2 * (BT_TABH * sg + n) + 1];
+                            CBCT_DEV_ASSERT(__float_as_int(E1.z) - hdr.y >= 0 && __float_as_int(E1.z) - hdr.y < hdr.w);
+                            E1.z = __int_as_float((int)(col0 + __float_as_int(E1.z) * (Q.XB * 16)));
+                            if (sg == 0) bt_visit<0, NSLOT, TP, ZV>(acc[0], C, zlo, E0, E1, hdr.z);
+                            else if (sg == 1) bt_visit<1, NSLOT, TP, ZV>(acc[0], C, zlo, E0, E1, hdr.z);
+                            else if (sg == 2) bt_visit<2, NSLOT, TP, ZV>(acc[0], C, zlo, E0, E1, hdr.z);
+                            else bt_visit<3, NSLOT, TP, ZV>(acc[0], C, zlo, E0, E1, hdr.z);
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(bar0 + 8 * (BT_NST + slot));
+                }
+            }
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        } else {
         for (int a = 0; a < P.nbase; ++a) {
             const float4 vw = s_view[a];
 #pragma unroll
@@ -316,29 +446,15 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                 // ---- list round: every lane takes one (stage, column, candidate detector column) ----
                 bool ok = false;
                 float4 e0 = make_float4(0.f, 0.f, 0.f, 0.f), e1 = e0;
-                {
+                if (col_ok) {
                     const int sg = rd * SPR + my_t;
-                    int mi, mj, iu_lo, iu_hi;
-                    float rn;
-                    bt_image(sg, vi0, vj0, n1, mi, mj);
-                    bt_shadow(P, vw, mi, mj, iu_lo, iu_hi, rn);
-                    CBCT_DEV_ASSERT(!col_ok || iu_hi - iu_lo + 1 <= BT_MAXC);
-                    if (col_ok && cnd <= iu_hi - iu_lo) {
-                        const int iu = iu_lo + cnd;
-                        const RayU r = load_rayu(rayu, a * P.nu + iu);
-                        const float bx = (float)(mi - P.cx), by = (float)(mj - P.cy);
-                        const float d0 = r.drive ? by : bx, mn = r.drive ? bx : by;
-                        const float y0 = fmaf(d0, r.m, r.a0);
-                        const float t1 = (mn - y0) * r.inv_m, t2 = (mn + 1.0f - y0) * r.inv_m;
-                        const float s_lo = fmaxf(fminf(t1, t2), 0.0f), s_hi = fminf(fmaxf(t1, t2), 1.0f);
-                        ok = s_hi > s_lo;
-                        const float e = d0 - r.sd;
-                        const float icA = rcp_approx(r.q * (e + s_lo)), icB = rcp_approx(r.q * (e + s_hi));
-                        e0 = make_float4(s_lo, s_hi, e, r.q);
+                    int iu = 0;
+                    ok = bt_list_entry(P, vw, rayu, a, vi0, vj0, n1, sg, cnd, e0, e1, iu);
+                    if (ok) {
                         const int s_abs = 4 * a + sg, cidx = iu - s_hdr[s_abs].y;
                         CBCT_DEV_ASSERT(s_hdr[s_abs].x || (cidx >= 0 && cidx < s_hdr[s_abs].w));
                         const uint32_t col_addr = tile0 + (s_abs % BT_NST) * Q.stage_bytes + cidx * (Q.XB * 16);
-                        e1 = make_float4(0.0f, fmaxf(icA, icB) * P.inv_dv, __int_as_float((int)col_addr), r.q > 0.0f ? 1.0f : 0.0f);
+                        e1.z = __int_as_float((int)col_addr);
                     }
                 }
                 const unsigned hit = __ballot_sync(0xffffffffu, ok);
@@ -372,6 +488,7 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
                     if (lane == 0) mbar_arrive(bar0 + 8 * (BT_NST + slot));
                 }
             }
+        }
         }
     }
 
@@ -452,13 +569,13 @@ EncodeTiledFn encode_tiled_fn()
     return fn;
 }
 
-template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV>
+template <int BI, int BJ, int CPW, int NSLOT, int TP, int MINB, int ZV, bool LT>
 cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out, unsigned int *errflag, cudaStream_t st,
                       const Shard *sh)
 {
     const LevelParams &P = L.p;
     const BtPlan &B = L.bt;
-    auto kern = back_tma_kernel<BI, BJ, CPW, NSLOT, TP, MINB, ZV>;
+    auto kern = back_tma_kernel<BI, BJ, CPW, NSLOT, TP, MINB, ZV, LT>;
     static bool attr_set = false;       // per instantiation; the value only grows
     static int attr_bytes = 0;
     if (!attr_set || B.q.total > attr_bytes) {
@@ -469,7 +586,7 @@ cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out
     dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 32 * ZV - 1) / (32 * ZV)), b((BI * BJ / CPW + 1) * 32);
     int kb_top = gr.z;
     if (sh) { kb_top = sh->zu_hi; gr.z = sh->zu_hi - sh->zu_lo; if (gr.z == 0) return CBCT_OK; }
-    kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag, kb_top);
+    kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag, kb_top, B.d_lists, B.d_hdrs);
     return CBCT_OK;
 }
 
@@ -585,6 +702,43 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     }
     P.tP = TP; P.tXP = tXP;
     B.ok = true;
+
+    // The in-plane lists of every (first-quadrant voxel column, base view), once per geometry: 512 bytes each (84 MB at config
+    // 3's finest level).  Left out -- the kernel then works its lists out itself, as in the first half of round 2 -- when an
+    // image has more than BT_TABH hitting columns somewhere, when the table would pass 2 GB, or on request.
+    B.d_lists = nullptr;
+    const size_t n_lists = (size_t)ni * nj * P.nbase, bytes = n_lists * 512;
+    if (ZV == 1 && !g->back_lists_on_the_fly && bytes <= ((size_t)2 << 30)) {
+        float4 *tab = nullptr;
+        unsigned int *ovf = nullptr;
+        if (cudaMalloc((void **)&tab, bytes) != cudaSuccess || cudaMalloc((void **)&ovf, sizeof(unsigned int)) != cudaSuccess) {
+            cudaGetLastError(); cudaFree(tab); cudaFree(ovf);
+            return CBCT_OK;                                 // no room for the table: lists on the fly
+        }
+        unsigned int h_ovf = 1;
+        cudaMemset(tab, 0, bytes); cudaMemset(ovf, 0, sizeof(unsigned int));
+        const unsigned blocks = (unsigned)((n_lists + 7) / 8);
+        bt_build_lists_kernel<<<blocks, 256>>>(P, L.d_rayu, L.d_view, tab, ovf);
+        const cudaError_t e = cudaMemcpy(&h_ovf, ovf, sizeof(unsigned int), cudaMemcpyDeviceToHost);
+        cudaFree(ovf);
+        if (e != cudaSuccess) { cudaFree(tab); return cbct_fail(CBCT_ERR_CUDA, "bt_build_lists_kernel: %s", cudaGetErrorString(e)); }
+        if (h_ovf == 0) B.d_lists = tab; else cudaFree(tab);
+    }
+    // ... and the stage headers of every (brick, z-unit), 16 bytes per stage, with the lists
+    B.d_hdrs = nullptr;
+    if (B.d_lists) {
+        const int gx = (ni + BI - 1) / BI, gy = (nj + BJ - 1) / BJ, gz = (nzh + 31) / 32;
+        const size_t n_hdr = (size_t)gx * gy * gz * 4 * P.nbase;
+        int4 *tab = nullptr;
+        if (cudaMalloc((void **)&tab, n_hdr * sizeof(int4)) != cudaSuccess) { cudaGetLastError(); return CBCT_OK; }
+        const unsigned blocks = (unsigned)((n_hdr + 7) / 8);
+#define BT_HDR_CASE(NS, TPV) \
+        if (NSLOT == NS && TP == TPV) bt_build_headers_kernel<4, 4, NS, TPV, 1><<<blocks, 256>>>(P, q, L.d_view, gx, gy, gz, tab, g->d_errflag);
+        BT_HDR_CASE(2, 1) BT_HDR_CASE(3, 1) BT_HDR_CASE(4, 1) BT_HDR_CASE(2, 2) BT_HDR_CASE(3, 2) BT_HDR_CASE(4, 2)
+#undef BT_HDR_CASE
+        if (cudaDeviceSynchronize() != cudaSuccess) { cudaFree(tab); return cbct_fail(CBCT_ERR_CUDA, "bt_build_headers_kernel failed"); }
+        B.d_hdrs = tab;
+    }
     return CBCT_OK;
 }
 
@@ -594,10 +748,13 @@ cbct_status launch_back_tma(const cbct_geometry *g, const Level &L, const float 
     const BtPlan &B = L.bt;
     cbct_status s = CBCT_ERR_INVALID_ARG;
 #define BT_CASE(NS, TPV)                                                                                         \
-    if (B.NSLOT == NS && B.TP == TPV)                                                                            \
-        s = B.ZV == 2 ? bt_launch<4, 4, 1, NS, TPV, 1, 2>(L, d_f, coef, d_out, g->d_errflag, st, sh)              \
-          : B.minb == 2 ? bt_launch<4, 4, 1, NS, TPV, 2, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh)            \
-                        : bt_launch<4, 4, 1, NS, TPV, 1, 1>(L, d_f, coef, d_out, g->d_errflag, st, sh);
+    if (B.NSLOT == NS && B.TP == TPV) {                                                                          \
+        if (B.ZV == 2) s = bt_launch<4, 4, 1, NS, TPV, 1, 2, false>(L, d_f, coef, d_out, g->d_errflag, st, sh);   \
+        else if (B.d_lists && B.minb == 2) s = bt_launch<4, 4, 1, NS, TPV, 2, 1, true>(L, d_f, coef, d_out, g->d_errflag, st, sh); \
+        else if (B.d_lists) s = bt_launch<4, 4, 1, NS, TPV, 1, 1, true>(L, d_f, coef, d_out, g->d_errflag, st, sh); \
+        else if (B.minb == 2) s = bt_launch<4, 4, 1, NS, TPV, 2, 1, false>(L, d_f, coef, d_out, g->d_errflag, st, sh); \
+        else s = bt_launch<4, 4, 1, NS, TPV, 1, 1, false>(L, d_f, coef, d_out, g->d_errflag, st, sh);             \
+    }
     BT_CASE(2, 1) BT_CASE(3, 1) BT_CASE(4, 1) BT_CASE(2, 2) BT_CASE(3, 2) BT_CASE(4, 2)
 #undef BT_CASE
     if (s != CBCT_OK) return s == CBCT_ERR_INVALID_ARG ? cbct_fail(s, "launch_back_tma: no kernel for this plan") : s;

@@ -79,6 +79,8 @@ struct BtPlan {
     int BI = 0, BJ = 0, CPW = 0, NSLOT = 0, TP = 1, minb = 1, ZV = 1;    // ZV: voxels per lane along z (blocks of 32 ZV slices)
     BtParams q;
     BtMaps maps;
+    int4 *d_hdrs = nullptr;     // stage headers of every (z-unit, brick), 4 n_base int4 each (with d_lists)
+    float4 *d_lists = nullptr;  // in-plane lists of every (first-quadrant voxel column, base view), 32 float4 each; NULL: on the fly
 };
 
 struct Level {
@@ -127,6 +129,7 @@ struct cbct_geometry {
     int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
     int host_armijo = 0;            // bit 1: the host-sequenced Armijo loop instead of the cooperative TV-prox kernel
     int tv_scalar_tiles = 0;        // bit 2: the TV passes on the 32-voxel warp tiles only
+    int back_lists_on_the_fly = 0;  // bit 3: the TMA back-projector works its in-plane lists out itself (no table at create)
     unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always
 };
 

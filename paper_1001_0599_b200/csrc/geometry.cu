@@ -113,7 +113,7 @@ static void free_all(cbct_geometry *g)
 {
     if (!g) return;
     for (Level &L : g->levels) {
-        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_cs); cudaFree(L.d_stage); cudaFree(L.d_T);
+        cudaFree(L.d_rayu); cudaFree(L.d_view); cudaFree(L.d_cs); cudaFree(L.d_stage); cudaFree(L.d_T); cudaFree(L.bt.d_lists); cudaFree(L.bt.d_hdrs);
         cudaFree(L.d_g); cudaFree(L.d_d); cudaFree(L.d_f2); cudaFree(L.d_f); cudaFree(L.d_prev); cudaFree(L.d_y);
     }
     cudaFree(g->d_partials); cudaFree(g->d_scalars); cudaFree(g->d_objective); cudaFree(g->d_counter); cudaFree(g->d_errflag);
@@ -150,6 +150,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     g->disable_tma = (desc->kernel_flags & CBCT_KERNEL_NO_TMA) ? 1 : 0;
     g->host_armijo = (desc->kernel_flags & CBCT_KERNEL_HOST_ARMIJO) ? 1 : 0;
     g->tv_scalar_tiles = (desc->kernel_flags & CBCT_KERNEL_TV_SCALAR_TILES) ? 1 : 0;
+    g->back_lists_on_the_fly = (desc->kernel_flags & CBCT_KERNEL_BACK_LISTS_ON_THE_FLY) ? 1 : 0;
     {   // the cooperative TV-prox kernel needs cooperative launches (every sm_100 device has them; checked all the same)
         int coop = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) g->host_armijo = 1;
@@ -162,6 +163,8 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
 
     st = dev_alloc(g, &g->d_errflag, (size_t)1);
     if (st != CBCT_OK) { free_all(g); return st; }
+    // zeroed before the levels are planned: the tables bt_plan_level builds count violated tile bounds in it
+    if (cudaMemset(g->d_errflag, 0, sizeof(unsigned int)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset failed"); }
     g->levels.resize(desc->max_levels);
     for (int l = 0; l < desc->max_levels; ++l) {
         Level &L = g->levels[l];
@@ -264,7 +267,6 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     TRY(dev_alloc(g, &g->d_partials, (size_t)8 * g->partials_stride));
     TRY(dev_alloc(g, &g->d_scalars, (size_t)kScalars));
     TRY(dev_alloc(g, &g->d_counter, (size_t)4));        // [0] ticket of the fused reductions, [1..2] tile tickets of the cooperative TV-prox
-    if (cudaMemset(g->d_errflag, 0, sizeof(unsigned int)) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset failed"); }
     if (cudaMemset(g->d_counter, 0, 4 * sizeof(unsigned int)) != cudaSuccess || cudaMemset(g->d_scalars, 0, sizeof(double) * kScalars) != cudaSuccess) { free_all(g); return cbct_fail(CBCT_ERR_CUDA, "memset of the reduction scalars failed"); }
     g->objective_cap = 4096;
     TRY(dev_alloc(g, &g->d_objective, (size_t)2 * g->objective_cap));

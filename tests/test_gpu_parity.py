@@ -608,6 +608,14 @@ def test_back_projector_paths_agree(torch, cbct, orc):
             assert rel_l2(o, want) <= TOL_PROJ, (name, rel_l2(o, want))
             assert np.abs(o - want).max() <= 1e-4 * np.abs(want).max()
         assert rel_l2(outs[False], outs[True]) <= 1e-6
+        # the TMA kernel fed by the in-plane list and stage-header tables made at create (the default) and the same kernel
+        # working both out itself (CBCT_KERNEL_BACK_LISTS_ON_THE_FLY): one definition of every entry, so the same bits
+        with cbct.geometry_create(g, back_lists_on_the_fly=True) as h:
+            assert h.back_path(0) == "tma"
+            b = torch.empty(g.vol_shape, device="cuda", dtype=torch.float32)
+            h.back_project(dev(torch, q), b)
+            assert h.bound_violations() == 0
+            assert b.cpu().numpy().tobytes() == outs[False].tobytes(), name
 
 
 def test_fbs_device_and_host_armijo_agree_bitwise(torch, cbct, orc):
