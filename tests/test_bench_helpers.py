@@ -41,10 +41,13 @@ def test_ncu_counters_record_parses_a_raw_export(tmp_path):
     units = ["", "", "", "", "us", "Mbyte", "Mbyte", "%", "register/thread"]
     rows = [["0", "void <unnamed>::back_tma_kernel<4, 4, 1, 3, 2, 2>(BtMaps, LevelParams)", "(32, 32, 4)", "(544, 1, 1)", "889.1", "99.5", "44.3", "64.5", "56"],
             ["1", "void forward_kernel<4, 2, 1>(LevelParams, const void *)", "(64, 10, 6)", "(32, 8, 1)", "766.0", "99.3", "21.2", "68.2", "76"],
-            ["2", "void forward_kernel<4, 2, 1>(LevelParams, const void *)", "(64, 10, 6)", "(32, 8, 1)", "1.0", "1.0", "1.0", "1.0", "76"]]
+            ["2", "void forward_kernel<4, 2, 1>(LevelParams, const void *)", "(64, 10, 6)", "(32, 8, 1)", "1.0", "1.0", "1.0", "1.0", "76"],
+            ["3", "stage_volume_packed_vec_kernel(const float *, float4 *, int, int, int, int, int)", "(4, 5, 256)", "(256, 1, 1)", "23.3", "67.1", "24.6", "1.0", "28"],
+            ["4", "void tv_prox_coop_kernel<1>(TvCoop)", "(576, 1, 1)", "(32, 4, 1)", "111.0", "222.2", "85.5", "2.0", "128"]]
     raw.write_text("\n".join(",".join('"%s"' % c for c in r) for r in [hdr, units] + rows))
     k = ncu_counters.parse(str(raw))
-    assert set(k) == {"back", "forward"}
+    assert set(k) == {"back", "forward", "transpose", "tv_prox"}
+    assert k["transpose"]["registers"] == 28 and k["tv_prox"]["ncu_duration_us"] == 111.0
     assert k["back"]["dram_bytes_per_launch"] == 99.5e6 + 44.3e6 and k["back"]["registers"] == 56
     assert k["forward"]["ncu_duration_us"] == 766.0            # the FIRST launch of a kernel
     h = ncu_counters.kernel_sources_sha256()
@@ -55,6 +58,6 @@ def test_tracked_counters_record_is_well_formed():
     p = os.path.join(ROOT, "profiles", "r02_counters.json")
     rec = json.load(open(p))
     assert len(rec["kernel_sources_sha256"]) == 64 and rec["ncu_command"].startswith("ncu ")
-    assert {"forward", "back"} <= set(rec["kernels"])
+    assert {"forward", "back", "tv_prox", "transpose"} <= set(rec["kernels"])
     for k in rec["kernels"].values():
         assert k["dram_bytes_per_launch"] > 0
