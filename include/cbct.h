@@ -80,6 +80,9 @@ typedef struct {
                                               column) pairs at the start of every base view instead of reading the table
                                               cbct_geometry_create builds once (512 bytes per first-quadrant voxel column and
                                               base view); same bits either way.  For A/B measurements and tests. */
+#define CBCT_KERNEL_NO_REFLECTION 16 /* the forward projector walks one base view per thread group even where the view set is
+                                        also symmetric under theta -> -theta (then it walks view pairs: 16 rays per weight
+                                        instead of 8).  For A/B measurements and tests. */
 #define CBCT_KERNEL_TV_SCALAR_TILES 4 /* the TV passes always on the 32-voxel warp tiles (one voxel per lane), never on the
                                          16-byte tiles that volumes with nx % 4 == 0, nx >= 128 and 16-byte aligned buffers
                                          otherwise take; same stencil, for A/B measurements and tests. */
@@ -245,8 +248,9 @@ cbct_status cbct_fbs_reconstruct_host(const cbct_geometry *g, const float *h_pro
 
 /* NEXT-4 -- the reconstruction sharded over `world` GPUs by OUTPUT OWNERSHIP (one process and one handle per GPU, every
  * rank calling with the same arguments).  Every rank holds the whole volume and the whole data; per iteration
- *   - rank r projects ITS base views (cbct_shard_range over cbct_shard_units' n_base_views; with quarter-turn symmetry a
- *     base view stands for its four quarter-turn partners) and the residual chunks are broadcast from their owners;
+ *   - rank r projects ITS forward units (cbct_shard_range over cbct_shard_units' n_base_views: base views -- with quarter-turn
+ *     symmetry a base view stands for its four quarter-turn partners -- or, where the view set is also symmetric under
+ *     theta -> -theta, view PAIRS (p, n_base - p)) and the residual chunks are broadcast from their owners;
  *   - the blocks' partial sums of T^2 are added across ranks (every slot is written by exactly one rank, the others hold
  *     0, so the addition is exact) and summed in the single-GPU order;
  *   - rank r evaluates g = f - tau c_norm P^T T on ITS z-units (n_z_units of z_unit_slices slices of the lower half volume,

@@ -43,6 +43,8 @@ struct LevelParams {
     int nx, ny, nz, nu, nv, np;
     int nsym, nbase;           // views handled per thread by rotation symmetry (1 or 4); np / nsym
     int nmir;                  // 2 when the z-mirror image of every ray / voxel shares its weights, else 1
+    int nrefl, npairs;         // 2 when the view set is also symmetric under theta -> -theta (forward.cu walks view pairs:
+                               // npairs = nbase / 2 + 1 units), else 1
     int stage_cells, t_entries; // cells of the staged copy / entries (R floats) of the residual stack: bounds of the gathers
     int tP, tXP;               // residual stack: rows of a detector column stored in tP planes by row % tP (1 = plain), tXP = nv / tP
                                // entries each: row iv sits at (iv % tP) * tXP + iv / tP of its column (back_tma.cu)
@@ -129,6 +131,7 @@ struct cbct_geometry {
     int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
     int host_armijo = 0;            // bit 1: the host-sequenced Armijo loop instead of the cooperative TV-prox kernel
     int tv_scalar_tiles = 0;        // bit 2: the TV passes on the 32-voxel warp tiles only
+    int no_reflection = 0;          // bit 4: the forward projector walks base views, never view pairs
     int back_lists_on_the_fly = 0;  // bit 3: the TMA back-projector works its in-plane lists out itself (no table at create)
     unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always
 };
@@ -197,6 +200,7 @@ static inline const Level *get_level(const cbct_geometry *g, int level)
 struct Shard {
     int base_lo, base_hi, zu_lo, zu_hi;
 };
+int forward_units(const Level &L);
 int back_zunit(const Level &L);
 int back_nzunits(const Level &L);
 

@@ -96,16 +96,30 @@ cbct_status sharded_forward(const cbct_geometry *g, const Level &L, const cbct_c
     const LevelParams &P = L.p;
     cbct_status s;
     Shard sh = {0, 0, 0, 0};
-    shard_range(P.nbase, cm->world, cm->rank, &sh.base_lo, &sh.base_hi);
-    const size_t nblk = (size_t)((P.nu + 7) / 8) * P.nbase * ((P.nv / P.nmir + 31) / 32);      // forward.cu's full grid
+    const int units = forward_units(L);         // base views, or view pairs (p, n_base - p) where the walk serves the reflections too
+    shard_range(units, cm->world, cm->rank, &sh.base_lo, &sh.base_hi);
+    const size_t nblk = (size_t)((P.nu + 7) / 8) * units * ((P.nv / P.nmir + 31) / 32);         // forward.cu's full grid
     if (nblk > (size_t)g->partials_stride) return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
     CBCT_CUDA(cudaMemsetAsync(g->d_partials, 0, nblk * sizeof(double), st));
     if ((s = launch_forward(g, L, f, y, L.d_T, 1, nullptr, st, &sh)) != CBCT_OK) return s;
     const size_t per_base = (size_t)P.nu * P.nv * P.nsym * sizeof(float);                       // one base view of the stack
     for (int r = 0; r < cm->world; ++r) {
         int lo, hi;
-        shard_range(P.nbase, cm->world, r, &lo, &hi);
-        if (hi > lo) CBCT_COMM(cm->broadcast(cm->ctx, (char *)L.d_T + (size_t)lo * per_base, (unsigned long long)(hi - lo) * per_base, r, st));
+        shard_range(units, cm->world, r, &lo, &hi);
+        if (hi <= lo) continue;
+        if (units == P.nbase) {
+            CBCT_COMM(cm->broadcast(cm->ctx, (char *)L.d_T + (size_t)lo * per_base, (unsigned long long)(hi - lo) * per_base, r, st));
+        } else {
+            // pairs lo .. hi-1 own the base views lo .. hi-1 and their partners n_base-(hi-1) .. n_base-lo (pair 0 and the
+            // middle pair of an even n_base are their own partners): two contiguous runs, trimmed where they meet or repeat
+            const int a_hi = hi < P.nbase ? hi : P.nbase;                                        // first run: [lo, a_hi)
+            CBCT_COMM(cm->broadcast(cm->ctx, (char *)L.d_T + (size_t)lo * per_base, (unsigned long long)(a_hi - lo) * per_base, r, st));
+            int p_lo = P.nbase - (hi - 1), p_hi = P.nbase - lo + 1;                              // second run: [p_lo, p_hi)
+            if (p_hi > P.nbase) p_hi = P.nbase;                                                  // partner of pair 0 is view 0 itself
+            if (p_lo < a_hi) p_lo = a_hi;                                                        // the middle view, already sent
+            if (p_hi > p_lo)
+                CBCT_COMM(cm->broadcast(cm->ctx, (char *)L.d_T + (size_t)p_lo * per_base, (unsigned long long)(p_hi - p_lo) * per_base, r, st));
+        }
     }
     CBCT_COMM(cm->allreduce_sum_f64(cm->ctx, g->d_partials, (unsigned long long)nblk, st));
     finalize_sums_kernel<<<1, 256, 0, st>>>(g->d_partials, (int)nblk, 1, g->partials_stride, d_sum_sq);
@@ -291,7 +305,7 @@ extern "C" cbct_status cbct_shard_units(const cbct_geometry *g, int level, int *
 {
     const Level *L = get_level(g, level);
     if (!L) return cbct_fail(CBCT_ERR_INVALID_ARG, "cbct_shard_units: bad handle or level");
-    if (n_base_views) *n_base_views = L->p.nbase;
+    if (n_base_views) *n_base_views = forward_units(*L);
     if (n_z_units) *n_z_units = back_nzunits(*L);
     if (z_unit_slices) *z_unit_slices = back_zunit(*L);
     return CBCT_OK;

@@ -140,7 +140,12 @@ __device__ __forceinline__ float cell_hi(float2 c) { return c.y; }
 // R = quarter-turn views per thread (1 or 4), M = 2 when the thread also walks the mirror image
 // z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again, and -- the staged
 // copy being mirror-packed -- the same loads.  MODE as in launch_forward.
-template <int R, int M, int MODE>
+// F = 2 (with R == 4 only): the thread also walks the REFLECTIONS y -> -y of its four rays.  On a view set that is symmetric
+// under theta -> -theta (theta_0 = 0, detector centred in u, nu even) the reflected ray of (base view a, quarter turn q, column
+// iu) is (base view (n_base - a) % n_base, quarter turn (3 - q) % 4 -- (4 - q) % 4 for a = 0 --, column nu-1-iu) and crosses
+// the cells (i, ny-1-j) with the same weights: one walk then serves 16 rays.  The grid's y dimension counts view PAIRS
+// p = 0 .. n_base/2; the self-paired views (p = 0, and p = n_base/2 when n_base is even) walk the columns iu < nu/2 only.
+template <int R, int M, int MODE, int F>
 __global__ void __launch_bounds__(FWD_BV *FWD_BU, FWD_MINB)
 forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU *__restrict__ rayu,
                const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
@@ -153,10 +158,13 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
     // staged copy for every view, which stays in L2 (with the view slowest, every view re-reads the whole copy)
     const int iv = blockIdx.z * FWD_BV + threadIdx.x;
     const int iu = blockIdx.x * FWD_BU + threadIdx.y;
-    const int a = blockIdx.y + a_off;          // base view (a_off: first base view of a sharded launch)
+    const int a = blockIdx.y + a_off;          // base view, or view pair (a_off: first unit of a sharded launch)
     const int nvh = M == 2 ? P.nv / 2 : P.nv;  // rows this grid walks; the others are their mirrors
+    constexpr int RF = R * F;                  // images of the walk in-plane
+    const int ar = F == 2 ? (P.nbase - a) % P.nbase : a;                 // base view of the reflected rays
+    const int nuw = (F == 2 && ar == a) ? P.nu / 2 : P.nu;               // columns this unit walks
     double sq = 0.0;
-    if (iu < P.nu && iv < nvh) {
+    if (iu < nuw && iv < nvh) {
         const RayU r = load_rayu(rayu, a * P.nu + iu);
         const float v = fmaf((float)iv, P.dv, P.v0);
         const RayZ rz = ray_z(r, v, P.sz);
@@ -171,9 +179,9 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
             const float t3 = ((float)(-P.cz) - 0.5f - rz.za) * rz.inv_mz, t4 = ((float)(P.nz - P.cz) + 0.5f - rz.za) * rz.inv_mz;
             dlo = fmaxf(dlo, fminf(t3, t4)); dhi = fminf(dhi, fmaxf(t3, t4));
         }
-        float acc[R * M];
+        float acc[RF * M];
 #pragma unroll
-        for (int q = 0; q < R * M; ++q) acc[q] = 0.0f;
+        for (int q = 0; q < RF * M; ++q) acc[q] = 0.0f;
         if (dhi > dlo) {
             const int s_lo = max(0, (int)floorf(dlo) + cd), s_hi = min(nd, (int)ceilf(dhi) + cd);
             float d = (float)(s_lo - cd);
@@ -189,12 +197,17 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
             int ci = r.drive ? jm : s_lo, cj = r.drive ? s_lo : jm;
             int si = r.drive ? 0 : 1, sj = r.drive ? 1 : 0;
             int mi = r.drive ? dj : 0, mj = r.drive ? 0 : dj;
-            int off[R], drow[R], dcol[R];       // element offsets into the staged copy (< 2^31, checked at create)
+            int off[RF], drow[RF], dcol[RF];    // element offsets into the staged copy (< 2^31, checked at create)
 #pragma unroll
             for (int q = 0; q < R; ++q) {
                 off[q] = (ci + PAD_M) * P.istride + (cj + PAD_M) * P.jstride + kk;
                 drow[q] = si * P.istride + sj * P.jstride;
                 dcol[q] = mi * P.istride + mj * P.jstride;
+                if (F == 2) {                   // the reflection y -> -y of this turned copy: cell (i, ny-1-j), steps (di, -dj)
+                    off[R + q] = (ci + PAD_M) * P.istride + (P.ny - 1 - cj + PAD_M) * P.jstride + kk;
+                    drow[R + q] = si * P.istride - sj * P.jstride;
+                    dcol[R + q] = mi * P.istride - mj * P.jstride;
+                }
                 int t = ci; ci = P.nx - 1 - cj; cj = t;
                 t = si; si = -sj; sj = t;
                 t = mi; mi = -mj; mj = t;
@@ -212,33 +225,33 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                 const float wl = 1.0f - hi;
                 const int zc = cz ? dk : 0;
                 // issue every load of the step before the first use: the loop is bound by load latency otherwise
-                int offc[R];
-                cell va[R], vc[R];
+                int offc[RF];
+                cell va[RF], vc[RF];
 #pragma unroll
-                for (int q = 0; q < R; ++q) offc[q] = off[q] + (cy ? dcol[q] : 0) + zc;
+                for (int q = 0; q < RF; ++q) offc[q] = off[q] + (cy ? dcol[q] : 0) + zc;
 #pragma unroll
-                for (int q = 0; q < R; ++q) {
+                for (int q = 0; q < RF; ++q) {
                     CBCT_DEV_ASSERT(off[q] >= 0 && off[q] < P.stage_cells && offc[q] >= 0 && offc[q] < P.stage_cells);
                     va[q] = __ldg(stage + off[q]); vc[q] = __ldg(stage + offc[q]);
                 }
 #pragma unroll
-                for (int q = 0; q < R; ++q) {
+                for (int q = 0; q < RF; ++q) {
                     acc[q] = fmaf(wl, cell_lo(vc[q]), fmaf(lo, cell_lo(va[q]), acc[q]));
-                    if (M == 2) acc[R + q] = fmaf(wl, cell_hi(vc[q]), fmaf(lo, cell_hi(va[q]), acc[R + q]));
+                    if (M == 2) acc[RF + q] = fmaf(wl, cell_hi(vc[q]), fmaf(lo, cell_hi(va[q]), acc[RF + q]));
                 }
                 if (hi > lo) {      // both planes crossed inside this slab, at different parameters (rare): a third cell
                     const float wm = hi - lo;
                     const bool yfirst = sy < sz;
 #pragma unroll
-                    for (int q = 0; q < R; ++q) {
+                    for (int q = 0; q < RF; ++q) {
                         CBCT_DEV_ASSERT(off[q] + (yfirst ? dcol[q] : dk) >= 0 && off[q] + (yfirst ? dcol[q] : dk) < P.stage_cells);
                         const cell vm = __ldg(stage + off[q] + (yfirst ? dcol[q] : dk));
                         acc[q] = fmaf(wm, cell_lo(vm), acc[q]);
-                        if (M == 2) acc[R + q] = fmaf(wm, cell_hi(vm), acc[R + q]);
+                        if (M == 2) acc[RF + q] = fmaf(wm, cell_hi(vm), acc[RF + q]);
                     }
                 }
 #pragma unroll
-                for (int q = 0; q < R; ++q) off[q] = offc[q] + drow[q];
+                for (int q = 0; q < RF; ++q) off[q] = offc[q] + drow[q];
                 if (cy) nexty += sgny;
                 if (cz) nextz += sgnz;
                 d += 1.0f;
@@ -252,30 +265,41 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
 #pragma unroll
         for (int mm = 0; mm < M; ++mm) {
             const int ivm = mm ? P.nv - 1 - iv : iv;
-            const size_t pix = (size_t)ivm * P.nu + iu;
-            float res[R];
 #pragma unroll
-            for (int q = 0; q < R; ++q) {
-                const float pr = acc[mm * R + q] * scale;
-                const size_t o1 = (size_t)(a + q * P.nbase) * plane + pix;
-                if (MODE == 0) {
-                    out[o1] = pr;
-                } else if (MODE == 4) {                // plain residual for the Eq. 6 back-projector
-                    const float T = pr - __ldg(y + o1);
-                    out[o1] = T;
-                    sq += (double)T * (double)T;
-                } else if (MODE == 2) {
-                    res[q] = pr * scale;               // L inv_dd * (P f): input of the transpose without a residual
-                } else {
-                    const float T = pr - __ldg(y + o1);
-                    res[q] = T * scale;                // what the transpose consumes (see back.cu)
-                    sq += (double)T * (double)T;
+            for (int fl = 0; fl < F; ++fl) {                // the walk's own rays, then their reflections
+                const int av = fl ? ar : a, iuv = fl ? P.nu - 1 - iu : iu;
+                const size_t pix = (size_t)ivm * P.nu + iuv;
+                float res[R];
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    // the quarter turn of view `av` this image belongs to
+                    const int qv = fl ? ((a == 0 ? 4 - q : 3 - q) & 3) : q;
+                    const float pr = acc[mm * RF + fl * R + q] * scale;
+                    const size_t o1 = (size_t)(av + qv * P.nbase) * plane + pix;
+                    float val = 0.0f;
+                    if (MODE == 0) {
+                        out[o1] = pr;
+                    } else if (MODE == 4) {                // plain residual for the Eq. 6 back-projector
+                        const float T = pr - __ldg(y + o1);
+                        out[o1] = T;
+                        sq += (double)T * (double)T;
+                    } else if (MODE == 2) {
+                        val = pr * scale;                  // L inv_dd * (P f): input of the transpose without a residual
+                    } else {
+                        const float T = pr - __ldg(y + o1);
+                        val = T * scale;                   // what the transpose consumes (see back.cu)
+                        sq += (double)T * (double)T;
+                    }
+                    // position of this quarter turn in the interleaved entry (a compile-time permutation per a == 0 or not)
+                    if (!fl) res[q] = val;
+                    else if (a == 0) res[(4 - q) & 3 & (R - 1)] = val;
+                    else res[(3 - q) & 3 & (R - 1)] = val;
                 }
-            }
-            if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
-                const size_t ot = ((size_t)a * P.nu + iu) * P.nv + t_row_slot(P, ivm);
-                if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
-                else out[ot] = res[0];
+                if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
+                    const size_t ot = ((size_t)av * P.nu + iuv) * P.nv + t_row_slot(P, ivm);
+                    if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+                    else out[ot] = res[0];
+                }
             }
         }
     }
@@ -283,7 +307,7 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
         double s[1];
         s[0] = block_sum(sq, slot);
         if (counter) publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
-        else publish_only<1>(s, 1, partials, stride, ((unsigned)blockIdx.z * P.nbase + a) * gridDim.x + blockIdx.x);   // sharded launch
+        else publish_only<1>(s, 1, partials, stride, ((unsigned)blockIdx.z * (F == 2 ? P.npairs : P.nbase) + a) * gridDim.x + blockIdx.x);   // sharded launch
     }
 }
 
@@ -328,19 +352,22 @@ count_samples_kernel(const LevelParams P, const RayU *__restrict__ rayu, double 
         partials[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = s;
 }
 
-template <int R, int M>
+template <int R, int M, int F>
 static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode,
                                 const void *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq,
                                 int a_off, bool fused_sum)
 {
     unsigned int *ctr = fused_sum ? g->d_counter : nullptr;
-    if (mode == 0) forward_kernel<R, M, 0><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
-    else if (mode == 2) forward_kernel<R, M, 2><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
-    else if (mode == 4) forward_kernel<R, M, 4><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
-                                                                 ctr, d_sum_sq, a_off);
-    else forward_kernel<R, M, 1><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
-                                                   ctr, d_sum_sq, a_off);
+    if (mode == 0) forward_kernel<R, M, 0, F><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
+    else if (mode == 2) forward_kernel<R, M, 2, F><<<gr, b, 0, st>>>(P, stage, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
+    else if (mode == 4) forward_kernel<R, M, 4, F><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                                    ctr, d_sum_sq, a_off);
+    else forward_kernel<R, M, 1, F><<<gr, b, 0, st>>>(P, stage, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                      ctr, d_sum_sq, a_off);
 }
+
+// units of a forward launch (its grid's y dimension, and what a sharded launch splits): base views, or view pairs
+int forward_units(const Level &L) { return (L.p.nsym == 4 && L.p.nmir == 2 && L.p.nrefl == 2) ? L.p.npairs : L.p.nbase; }
 
 cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *d_vol, const float *d_y,
                            float *d_out, int mode, double *d_sum_sq, cudaStream_t st, const Shard *sh)
@@ -378,13 +405,14 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         CBCT_LAUNCH_CHECK(g);
     }
     b = dim3(FWD_BV, FWD_BU);
-    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, P.nbase, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
+    const int units = forward_units(L);          // base views, or view pairs where the walk also serves the reflected rays
+    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, units, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;             // of the full launch: the numbering of the partial sums
     if ((mode == 1 || mode == 4) && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
     int a_off = 0;
     if (sh) {
-        if (sh->base_lo < 0 || sh->base_hi > P.nbase || sh->base_lo > sh->base_hi) return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_forward: bad shard");
+        if (sh->base_lo < 0 || sh->base_hi > units || sh->base_lo > sh->base_hi) return cbct_fail(CBCT_ERR_INVALID_ARG, "launch_forward: bad shard");
         a_off = sh->base_lo;
         gr.y = sh->base_hi - sh->base_lo;
         if (gr.y == 0) return CBCT_OK;
@@ -392,10 +420,11 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     {
         StageTimer t(g, st, ST_FORWARD);
         const bool fused = sh == nullptr;
-        if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
-        else if (P.nsym == 4) launch_forward_mode<4, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
-        else if (P.nmir == 2) launch_forward_mode<1, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
-        else launch_forward_mode<1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        if (P.nsym == 4 && P.nmir == 2 && P.nrefl == 2) launch_forward_mode<4, 2, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nsym == 4) launch_forward_mode<4, 1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nmir == 2) launch_forward_mode<1, 2, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else launch_forward_mode<1, 1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
         CBCT_LAUNCH_CHECK(g);
     }
     return CBCT_OK;

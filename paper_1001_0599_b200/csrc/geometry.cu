@@ -151,6 +151,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     g->host_armijo = (desc->kernel_flags & CBCT_KERNEL_HOST_ARMIJO) ? 1 : 0;
     g->tv_scalar_tiles = (desc->kernel_flags & CBCT_KERNEL_TV_SCALAR_TILES) ? 1 : 0;
     g->back_lists_on_the_fly = (desc->kernel_flags & CBCT_KERNEL_BACK_LISTS_ON_THE_FLY) ? 1 : 0;
+    g->no_reflection = (desc->kernel_flags & CBCT_KERNEL_NO_REFLECTION) ? 1 : 0;
     {   // the cooperative TV-prox kernel needs cooperative launches (every sm_100 device has them; checked all the same)
         int coop = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) g->host_armijo = 1;
@@ -199,6 +200,15 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
             if (ok) p.nsym = 4;
         }
         p.nbase = p.np / p.nsym;
+        // reflection symmetry theta -> -theta on top of the quarter turns: theta_0 = 0 and theta_a + theta_(nbase-a) = 90 degrees,
+        // detector centred in u with an even column count (column iu <-> nu-1-iu)
+        p.nrefl = 1; p.npairs = p.nbase;
+        if (p.nsym == 4 && !g->no_reflection && desc->det_off_u == 0.0 && p.nu % 2 == 0 && fabs(g->angles[0]) < 1e-12) {
+            bool ok = true;
+            for (int a = 1; a < p.nbase && ok; ++a)
+                ok = fabs(g->angles[a] + g->angles[p.nbase - a] - 0.5 * M_PI) < 1e-12;
+            if (ok) { p.nrefl = 2; p.npairs = p.nbase / 2 + 1; }
+        }
         // mirror symmetry z -> -z: volume centred in z, detector centred in v, even sizes
         p.nmir = (g->allow_symmetry && desc->vol_off[2] == 0.0 && desc->det_off_v == 0.0 && p.nz % 2 == 0 && p.nv % 2 == 0) ? 2 : 1;
 
