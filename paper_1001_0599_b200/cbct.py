@@ -189,7 +189,8 @@ class Geometry:
     """
 
     def __init__(self, desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False, host_armijo: bool = False,
-                 tv_scalar_tiles: bool = False, back_lists_on_the_fly: bool = False, no_reflection: bool = False):
+                 tv_scalar_tiles: bool = False, back_lists_on_the_fly: bool = False, no_reflection: bool = False,
+                 no_fold: bool = False):
         lib = load_library()
         self._h = C.c_void_p()
         self.desc = desc
@@ -208,7 +209,8 @@ class Geometry:
         d.no_symmetry = int(bool(no_symmetry))
         # CBCT_KERNEL_NO_TMA | CBCT_KERNEL_HOST_ARMIJO | CBCT_KERNEL_TV_SCALAR_TILES | CBCT_KERNEL_BACK_LISTS_ON_THE_FLY
         d.kernel_flags = ((1 if no_tma else 0) | (2 if host_armijo else 0) | (4 if tv_scalar_tiles else 0) |
-                          (8 if back_lists_on_the_fly else 0) | (16 if no_reflection else 0))      # ... | CBCT_KERNEL_NO_REFLECTION
+                          (8 if back_lists_on_the_fly else 0) | (16 if no_reflection else 0) |   # ... | CBCT_KERNEL_NO_REFLECTION
+                          (32 if no_fold else 0))                                                # | CBCT_KERNEL_NO_FOLD
         _check(lib.cbct_geometry_create(C.byref(d), C.byref(self._h)))
 
     def close(self):
@@ -493,8 +495,9 @@ def gather_ceiling(buf, variant: int, reuse: int = 1, iters: int = 64, stream=No
 
 def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma: bool = False,
                     host_armijo: bool = False, tv_scalar_tiles: bool = False, back_lists_on_the_fly: bool = False,
-                    no_reflection: bool = False) -> Geometry:
-    return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo, tv_scalar_tiles, back_lists_on_the_fly, no_reflection)
+                    no_reflection: bool = False, no_fold: bool = False) -> Geometry:
+    return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo, tv_scalar_tiles, back_lists_on_the_fly, no_reflection,
+                    no_fold)
 
 
 def version() -> str:

@@ -50,6 +50,8 @@ struct LevelParams {
                                // entries each: row iv sits at (iv % tP) * tXP + iv / tP of its column (back_tma.cu)
     int nyP, nzP;              // padded extents of the staged volume [i + PM][j + PM][k + PZ] (k fastest)
     int istride, jstride;      // its element strides along i and j (nyP * nzP, nzP)
+    int fold, nhP, fis, fjs;   // fold != 0: the staged copy is folded onto the first quadrant (forward.cu): [i0 + PM][j0 + PM][kk]
+                               // entries of 8 floats, nhP = nx / 2 + PM canonical cells per axis, entry strides fis = nhP * nzP, fjs = nzP
     int cx, cy, cz;            // n/2 (integer): index of the grid plane at index coordinate 0
     float hx, hy, hz;
     float x0, y0, z0;          // centre of voxel 0 in mm
@@ -131,6 +133,7 @@ struct cbct_geometry {
     int disable_tma = 0;            // cbct_geometry_desc::kernel_flags bit 0
     int host_armijo = 0;            // bit 1: the host-sequenced Armijo loop instead of the cooperative TV-prox kernel
     int tv_scalar_tiles = 0;        // bit 2: the TV passes on the 32-voxel warp tiles only
+    int no_fold = 0;                // bit 5: the forward projector never reads the folded staged copy
     int no_reflection = 0;          // bit 4: the forward projector walks base views, never view pairs
     int back_lists_on_the_fly = 0;  // bit 3: the TMA back-projector works its in-plane lists out itself (no table at create)
     unsigned int *d_errflag = nullptr;  // device-side "a create-time bound did not hold" counter (back_tma.cu); 0 always

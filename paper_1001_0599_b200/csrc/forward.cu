@@ -137,6 +137,58 @@ __device__ __forceinline__ float cell_lo(float2 c) { return c.x; }
 __device__ __forceinline__ float cell_hi(float c) { return c; }
 __device__ __forceinline__ float cell_hi(float2 c) { return c.y; }
 
+// What a walk leaves behind: the RF * M sums of a thread's rays (acc[mm * R * F + fl * R + q]: mirror image mm, reflection fl,
+// quarter turn q of the walk) scaled to line integrals and written as MODE says; returns through sq the squared residuals.
+template <int R, int M, int MODE, int F>
+__device__ __forceinline__ void forward_epilogue(const LevelParams &P, const RayU &r, float v, const float (&acc)[R * F * M], int a, int ar,
+                                                 int iu, int iv, const float *__restrict__ y, float *__restrict__ out, double &sq)
+{
+    constexpr int RF = R * F;
+    const float Lr = ray_len_L(r, v);
+    const float scale = Lr * r.inv_dd;
+    const size_t plane = (size_t)P.nv * P.nu;
+#pragma unroll
+    for (int mm = 0; mm < M; ++mm) {
+        const int ivm = mm ? P.nv - 1 - iv : iv;
+#pragma unroll
+        for (int fl = 0; fl < F; ++fl) {                // the walk's own rays, then their reflections
+            const int av = fl ? ar : a, iuv = fl ? P.nu - 1 - iu : iu;
+            const size_t pix = (size_t)ivm * P.nu + iuv;
+            float res[R];
+#pragma unroll
+            for (int q = 0; q < R; ++q) {
+                // the quarter turn of view `av` this image belongs to
+                const int qv = fl ? ((a == 0 ? 4 - q : 3 - q) & 3) : q;
+                const float pr = acc[mm * RF + fl * R + q] * scale;
+                const size_t o1 = (size_t)(av + qv * P.nbase) * plane + pix;
+                float val = 0.0f;
+                if (MODE == 0) {
+                    out[o1] = pr;
+                } else if (MODE == 4) {                // plain residual for the Eq. 6 back-projector
+                    const float T = pr - __ldg(y + o1);
+                    out[o1] = T;
+                    sq += (double)T * (double)T;
+                } else if (MODE == 2) {
+                    val = pr * scale;                  // L inv_dd * (P f): input of the transpose without a residual
+                } else {
+                    const float T = pr - __ldg(y + o1);
+                    val = T * scale;                   // what the transpose consumes (see back.cu)
+                    sq += (double)T * (double)T;
+                }
+                // position of this quarter turn in the interleaved entry (a compile-time permutation per a == 0 or not)
+                if (!fl) res[q] = val;
+                else if (a == 0) res[(4 - q) & 3 & (R - 1)] = val;
+                else res[(3 - q) & 3 & (R - 1)] = val;
+            }
+            if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
+                const size_t ot = ((size_t)av * P.nu + iuv) * P.nv + t_row_slot(P, ivm);
+                if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
+                else out[ot] = res[0];
+            }
+        }
+    }
+}
+
 // R = quarter-turn views per thread (1 or 4), M = 2 when the thread also walks the mirror image
 // z -> -z of its ray (detector row nv-1-iv, cells nz-1-k): same weights again, and -- the staged
 // copy being mirror-packed -- the same loads.  MODE as in launch_forward.
@@ -259,55 +311,366 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
                 z0 = fmaf(d, rz.mz, rz.za);
             }
         }
-        const float Lr = ray_len_L(r, v);
-        const float scale = Lr * r.inv_dd;
-        const size_t plane = (size_t)P.nv * P.nu;
-#pragma unroll
-        for (int mm = 0; mm < M; ++mm) {
-            const int ivm = mm ? P.nv - 1 - iv : iv;
-#pragma unroll
-            for (int fl = 0; fl < F; ++fl) {                // the walk's own rays, then their reflections
-                const int av = fl ? ar : a, iuv = fl ? P.nu - 1 - iu : iu;
-                const size_t pix = (size_t)ivm * P.nu + iuv;
-                float res[R];
-#pragma unroll
-                for (int q = 0; q < R; ++q) {
-                    // the quarter turn of view `av` this image belongs to
-                    const int qv = fl ? ((a == 0 ? 4 - q : 3 - q) & 3) : q;
-                    const float pr = acc[mm * RF + fl * R + q] * scale;
-                    const size_t o1 = (size_t)(av + qv * P.nbase) * plane + pix;
-                    float val = 0.0f;
-                    if (MODE == 0) {
-                        out[o1] = pr;
-                    } else if (MODE == 4) {                // plain residual for the Eq. 6 back-projector
-                        const float T = pr - __ldg(y + o1);
-                        out[o1] = T;
-                        sq += (double)T * (double)T;
-                    } else if (MODE == 2) {
-                        val = pr * scale;                  // L inv_dd * (P f): input of the transpose without a residual
-                    } else {
-                        const float T = pr - __ldg(y + o1);
-                        val = T * scale;                   // what the transpose consumes (see back.cu)
-                        sq += (double)T * (double)T;
-                    }
-                    // position of this quarter turn in the interleaved entry (a compile-time permutation per a == 0 or not)
-                    if (!fl) res[q] = val;
-                    else if (a == 0) res[(4 - q) & 3 & (R - 1)] = val;
-                    else res[(3 - q) & 3 & (R - 1)] = val;
-                }
-                if (MODE != 0 && MODE != 4) {              // d_T layout: [base view][iu][iv] (x4 interleaved)
-                    const size_t ot = ((size_t)av * P.nu + iuv) * P.nv + t_row_slot(P, ivm);
-                    if (R == 4) reinterpret_cast<float4 *>(out)[ot] = make_float4(res[0], res[1 % R], res[2 % R], res[3 % R]);
-                    else out[ot] = res[0];
-                }
-            }
-        }
+        forward_epilogue<R, M, MODE, F>(P, r, v, acc, a, ar, iu, iv, y, out, sq);
     }
     if (MODE == 1 || MODE == 4) {        // E2 numerator: sum of squared residuals, second stage fused (reduce.cuh)
         double s[1];
         s[0] = block_sum(sq, slot);
         if (counter) publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
         else publish_only<1>(s, 1, partials, stride, ((unsigned)blockIdx.z * (F == 2 ? P.npairs : P.nbase) + a) * gridDim.x + blockIdx.x);   // sharded launch
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// The FOLDED staged copy and its walk (quarter-turn + mirror symmetric levels: nsym == 4, nmir == 2).
+//
+// The 8 (16 with view pairs) rays of a thread read, in every cell (i, j, k) they cross, the cell's images under the quarter
+// turns (and the reflection y -> -y) and under the mirror z -> -z.  forward_kernel fetches each image with its own 8-byte load at
+// its own offset: per slab step of 16 rays, 16 loads + 16 address computations + 16 offset updates of 113 instructions.  Here
+// the staged copy is folded onto the first quadrant instead: the entry of the canonical cell (i0, j0), i0, j0 < n/2, holds
+//     E(i0, j0, kk) = ( f(R^q (i0, j0), k), q = 0..3 | f(R^q (i0, j0), nz-1-k), q = 0..3 ),   R (i, j) = (n-1-j, i),  k = kk - PZ
+// -- two float4, each in a plane of its own (the lanes of a warp are consecutive detector rows: their entries are neighbours in kk,
+// and a 16-byte load per lane at a 16-byte stride costs half the L1 wavefronts of one at a 32-byte stride), the same
+// 8 n^2 nzP / 4 floats in all.  A cell (i, j) in quadrant m (m = 0: i, j < n/2; 1: i >= n/2 >
+// j; 2: both >=; 3: j >= n/2 > i) is R^m of its canonical cell, so the q-th turned copy of the ray reads component (q + m) mod 4
+// of ONE entry (two 16-byte loads); its reflection's q-th copy reads component (3 - q - m) mod 4 of the entry of the TRANSPOSED
+// canonical cell (j0, i0) (S R^m (i0, j0) = R^(3-m) (j0, i0) with S the reflection).  A slab step of 16 rays is then 8 loads of
+// 16 bytes at 4 offsets.  The sums are kept in the frame of the current quadrant (accumulator c belongs to component c) and
+// rotated when the walk changes quadrant -- at the centre plane of the driving axis, between two slabs, and in the one slab
+// where the ray crosses the centre plane of the minor axis, which takes a generic path (fold_cell); a walk changes quadrant
+// at most three times.  Same weights, same order of the FMAs of every ray as forward_kernel: the same bits.
+// Margins: canonical coordinates run from -PAD_M (a cell outside the grid folds to a negative canonical coordinate); those
+// entries, and the components of k outside the grid, are written as zeros by the staging kernel.
+
+constexpr int FOLD_T = 16, FOLD_K = 4;       // staging tile: 16 x 16 canonical cells x 4 cells in kk
+// vol [k][j][i] -> fold[half][(i0+PM)][(j0+PM)][kk] (float4): every image's 16 x 16 patch is read with x fastest (64-byte runs) and
+// the tile leaves as 64-byte runs (4 entries of one canonical column and half).
+__global__ void __launch_bounds__(256)
+stage_volume_fold_kernel(const float *__restrict__ in, float4 *__restrict__ fold, int n, int nz, int nhP, int nzP)
+{
+    __shared__ float tile[2][4][FOLD_K][FOLD_T][FOLD_T + 1];         // [half][q][kk][i0][j0]
+    const int a0 = blockIdx.x * FOLD_T, b0 = blockIdx.y * FOLD_T, kk0 = blockIdx.z * FOLD_K;
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4, n1 = n - 1;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        // thread (tx, ty) of image q's patch: x runs with tx.  q = 0: (x, y) = (i0, j0); 1: (n1 - j0, i0); 2: (n1 - i0, n1 - j0);
+        // 3: (j0, n1 - i0)
+        int il, jl;
+        if (q == 0) { il = tx; jl = ty; }
+        else if (q == 1) { jl = FOLD_T - 1 - tx; il = ty; }
+        else if (q == 2) { il = FOLD_T - 1 - tx; jl = FOLD_T - 1 - ty; }
+        else { jl = tx; il = FOLD_T - 1 - ty; }
+        const int i0 = a0 + il - PAD_M, j0 = b0 + jl - PAD_M;
+        const int x = q == 0 ? i0 : q == 1 ? n1 - j0 : q == 2 ? n1 - i0 : j0;
+        const int y = q == 0 ? j0 : q == 1 ? i0 : q == 2 ? n1 - j0 : n1 - i0;
+        const bool inpl = i0 >= 0 && j0 >= 0 && i0 < n / 2 && j0 < n / 2;
+#pragma unroll
+        for (int c = 0; c < FOLD_K; ++c) {
+            const int k = kk0 + c - PAD_Z, km = nz - 1 - k;
+            float lo = 0.0f, hi = 0.0f;
+            if (inpl && k >= 0 && k < nz) {                          // km is in range exactly when k is
+                lo = __ldg(in + ((size_t)k * n + y) * n + x);
+                hi = __ldg(in + ((size_t)km * n + y) * n + x);
+            }
+            tile[0][q][c][il][jl] = lo; tile[1][q][c][il][jl] = hi;
+        }
+    }
+    __syncthreads();
+    const int f4 = threadIdx.x & 7, c = f4 >> 1, half = f4 & 1;      // 8 float4 = 4 entries = 128 bytes per canonical column
+#pragma unroll
+    for (int it = 0; it < 8; ++it) {
+        const int cell = (threadIdx.x >> 3) + 32 * it, il = cell >> 4, jl = cell & 15;
+        const int a = a0 + il, b = b0 + jl, kk = kk0 + c;
+        if (a < nhP && b < nhP && kk < nzP)
+            fold[(size_t)half * nhP * nhP * nzP + ((size_t)a * nhP + b) * nzP + kk] =
+                make_float4(tile[half][0][c][il][jl], tile[half][1][c][il][jl], tile[half][2][c][il][jl], tile[half][3][c][il][jl]);
+    }
+}
+
+// frame rotations of four sums: up: new[(c + 1) & 3] = old[c]; down: new[(c - 1) & 3] = old[c]
+__device__ __forceinline__ void fold_rot_up(float (&a)[4]) { const float t = a[3]; a[3] = a[2]; a[2] = a[1]; a[1] = a[0]; a[0] = t; }
+__device__ __forceinline__ void fold_rot_dn(float (&a)[4]) { const float t = a[0]; a[0] = a[1]; a[1] = a[2]; a[2] = a[3]; a[3] = t; }
+// component c of the result = component (c + d) & 3 of v
+__device__ __forceinline__ float4 fold_rot4(float4 v, int d)
+{
+    if (d & 1) v = make_float4(v.y, v.z, v.w, v.x);
+    if (d & 2) v = make_float4(v.z, v.w, v.x, v.y);
+    return v;
+}
+__device__ __forceinline__ void fold_fma(float (&a)[4], float w, const float4 v)
+{
+    a[0] = fmaf(w, v.x, a[0]); a[1] = fmaf(w, v.y, a[1]); a[2] = fmaf(w, v.z, a[2]); a[3] = fmaf(w, v.w, a[3]);
+}
+
+// quadrant m of the cell (ci, cj) and its canonical cell (i0, j0): (ci, cj) = R^m (i0, j0)
+__device__ __forceinline__ int fold_canon(int ci, int cj, int nh, int n1, int &i0, int &j0)
+{
+    const bool qi = ci >= nh, qj = cj >= nh;
+    const int m = qi ? (qj ? 2 : 1) : (qj ? 3 : 0);
+    i0 = m == 0 ? ci : m == 1 ? cj : m == 2 ? n1 - ci : n1 - cj;
+    j0 = m == 0 ? cj : m == 1 ? n1 - ci : m == 2 ? n1 - cj : ci;
+    return m;
+}
+// a step (di, dj) of the cell seen from the canonical cell of quadrant m
+__device__ __forceinline__ void fold_step(int m, int di, int dj, int &d0i, int &d0j)
+{
+    d0i = m == 0 ? di : m == 1 ? dj : m == 2 ? -di : -dj;
+    d0j = m == 0 ? dj : m == 1 ? -di : m == 2 ? -dj : di;
+}
+
+// One cell of the slab that crosses the centre plane of the minor axis: any quadrant, added into the sums kept in frame m.
+template <int F>
+__device__ __forceinline__ void fold_cell(const LevelParams &P, const float4 *__restrict__ fold, int ci, int cj, int kk, float w, int m,
+                                          float (&accB)[2][4], float (&accT)[2][4])
+{
+    int i0, j0;
+    const int mc = fold_canon(ci, cj, P.nx / 2, P.nx - 1, i0, j0);
+    const int dlt = (mc - m) & 3;
+    const int oB = (i0 + PAD_M) * P.fis + (j0 + PAD_M) * P.fjs + kk;
+    CBCT_DEV_ASSERT(oB >= 0 && oB < P.stage_cells);
+    const float4 *__restrict__ fold_hi = fold + P.stage_cells;
+    const float4 b0 = __ldg(fold + oB), b1 = __ldg(fold_hi + oB);
+    fold_fma(accB[0], w, fold_rot4(b0, dlt));
+    fold_fma(accB[1], w, fold_rot4(b1, dlt));
+    if (F == 2) {
+        const int oT = (j0 + PAD_M) * P.fis + (i0 + PAD_M) * P.fjs + kk;
+        CBCT_DEV_ASSERT(oT >= 0 && oT < P.stage_cells);
+        const float4 t0 = __ldg(fold + oT), t1 = __ldg(fold_hi + oT);
+        fold_fma(accT[0], w, fold_rot4(t0, (4 - dlt) & 3));
+        fold_fma(accT[1], w, fold_rot4(t1, (4 - dlt) & 3));
+    }
+}
+
+#ifndef FOLD_BU
+#define FOLD_BU 8           // detector columns per block (x 32 rows)
+#endif
+#ifndef FOLD_MINB2
+#define FOLD_MINB2 3        // resident blocks per SM the view-pair walk is compiled for (80 registers), and the 8-ray walk
+#endif
+#ifndef FOLD_MINB1
+#define FOLD_MINB1 2
+#endif
+#ifndef FOLD_PIPE
+#define FOLD_PIPE 0
+#endif
+// one slab step in flight: its crossing parameters, the offsets its rare third cell needs, its loaded entries
+template <int F> struct FoldStep {
+    float lo, hi;
+    int oB, oT;
+    bool yfirst;
+    float4 v[4 * F];
+};
+// forward_kernel<4, 2, MODE, F> on the folded copy: same grid, same rays per thread, same epilogue.
+template <int MODE, int F>
+__global__ void __launch_bounds__(FWD_BV *FOLD_BU, F == 2 ? FOLD_MINB2 : FOLD_MINB1)
+forward_fold_kernel(const LevelParams P, const float4 *__restrict__ fold, const RayU *__restrict__ rayu,
+                    const float *__restrict__ y, float *__restrict__ out, double *__restrict__ partials, int stride,
+                    unsigned int *__restrict__ counter, double *__restrict__ sum_out, int a_off)
+{
+    __shared__ double slot[32];
+    const float4 *__restrict__ fold_hi = fold + P.stage_cells;     // the z-mirror components: a plane of their own
+    const int iv = blockIdx.z * FWD_BV + threadIdx.x;
+    const int iu = blockIdx.x * FOLD_BU + threadIdx.y;
+    const int a = blockIdx.y + a_off;
+    const int nvh = P.nv / 2;
+    const int ar = F == 2 ? (P.nbase - a) % P.nbase : a;
+    const int nuw = (F == 2 && ar == a) ? P.nu / 2 : P.nu;
+    double sq = 0.0;
+    if (iu < nuw && iv < nvh) {
+        const RayU r = load_rayu(rayu, a * P.nu + iu);
+        const float v = fmaf((float)iv, P.dv, P.v0);
+        const RayZ rz = ray_z(r, v, P.sz);
+        const int n = P.nx, nh = n / 2, n1 = n - 1;           // square, even, centred grid: cx = cy = nh
+        float dlo = (float)(-nh), dhi = (float)(n - nh);
+        {
+            const float t1 = ((float)(-nh) - 0.5f - r.a0) * r.inv_m, t2 = ((float)(n - nh) + 0.5f - r.a0) * r.inv_m;
+            dlo = fmaxf(dlo, fminf(t1, t2)); dhi = fminf(dhi, fmaxf(t1, t2));
+            const float t3 = ((float)(-P.cz) - 0.5f - rz.za) * rz.inv_mz, t4 = ((float)(P.nz - P.cz) + 0.5f - rz.za) * rz.inv_mz;
+            dlo = fmaxf(dlo, fminf(t3, t4)); dhi = fminf(dhi, fmaxf(t3, t4));
+        }
+        float accB[2][4], accT[2][4];                         // [mirror][component of the entry]: the frame of quadrant m
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { accB[0][c] = accB[1][c] = 0.0f; accT[0][c] = accT[1][c] = 0.0f; }
+        int m = 0;
+        if (dhi > dlo) {
+            const int s_lo = max(0, (int)floorf(dlo) + nh), s_hi = min(n, (int)ceilf(dhi) + nh);
+            float d = (float)(s_lo - nh);
+            float y0 = fmaf(d, r.m, r.a0), z0 = fmaf(d, rz.mz, rz.za);
+            const float fy = floorf(y0), fz = floorf(z0);
+            const bool posy = r.m >= 0.0f, posz = rz.mz >= 0.0f;
+            float nexty = posy ? fy + 1.0f : fy, nextz = posz ? fz + 1.0f : fz;
+            const float sgny = posy ? 1.0f : -1.0f, sgnz = posz ? 1.0f : -1.0f;
+            const int dj = posy ? 1 : -1, dk = posz ? 1 : -1;
+            const int si = r.drive ? 0 : 1, sj = r.drive ? 1 : 0;          // slab step and minor-axis step of the cell
+            const int mi = r.drive ? dj : 0, mj = r.drive ? 0 : dj;
+            int s = s_lo;
+            while (s < s_hi) {
+                // ---- a run of slabs inside one quadrant: the cell from the tracked planes, the sums turned into its frame ----
+                const int jm = (int)nexty - (posy ? 1 : 0) + nh, kk = (int)nextz - (posz ? 1 : 0) + P.cz + PAD_Z;
+                const int ci = r.drive ? jm : s, cj = r.drive ? s : jm;
+                int i0, j0, d0i, d0j, c0i, c0j;
+                const int mq = fold_canon(ci, cj, nh, n1, i0, j0);
+                fold_step(mq, si, sj, d0i, d0j);
+                fold_step(mq, mi, mj, c0i, c0j);
+                for (int t = (mq - m) & 3; t > 0; --t) {
+                    fold_rot_up(accB[0]); fold_rot_up(accB[1]);
+                    if (F == 2) { fold_rot_dn(accT[0]); fold_rot_dn(accT[1]); }
+                }
+                m = mq;
+                int offB = (i0 + PAD_M) * P.fis + (j0 + PAD_M) * P.fjs + kk, offT = (j0 + PAD_M) * P.fis + (i0 + PAD_M) * P.fjs + kk;
+                const int drowB = d0i * P.fis + d0j * P.fjs, drowT = d0j * P.fis + d0i * P.fjs;
+                const int dcolB = c0i * P.fis + c0j * P.fjs, dcolT = c0j * P.fis + c0i * P.fjs;
+                const int seg_end = s < nh ? min(nh, s_hi) : s_hi;
+                bool mixed = false;
+#if FOLD_PIPE
+                // Two slab steps in flight: the loads of slab s + 1 are issued before the sums of slab s are formed (two sets of
+                // load registers, the loop unrolled by two so that neither is ever moved).
+                auto issue = [&](FoldStep<F> &S) -> bool {
+                    if (s >= seg_end) return false;
+                    const float sy = __saturatef((nexty - y0) * r.inv_m);
+                    const float sz = __saturatef((nextz - z0) * rz.inv_mz);
+                    const bool cy = sy < 1.0f, cz = sz < 1.0f;
+                    if (cy && nexty == 0.0f) { mixed = true; return false; }   // crosses the centre plane of the minor axis
+                    S.lo = fminf(sy, sz);
+                    S.hi = (cy && cz) ? fmaxf(sy, sz) : S.lo;
+                    const int zc = cz ? dk : 0;
+                    const int offcB = offB + (cy ? dcolB : 0) + zc, offcT = offT + (cy ? dcolT : 0) + zc;
+                    CBCT_DEV_ASSERT(offB >= 0 && offB < P.stage_cells && offcB >= 0 && offcB < P.stage_cells);
+                    CBCT_DEV_ASSERT(F == 1 || (offT >= 0 && offT < P.stage_cells && offcT >= 0 && offcT < P.stage_cells));
+                    S.yfirst = sy < sz; S.oB = offB; S.oT = offT;
+                    S.v[0] = __ldg(fold + offB); S.v[1] = __ldg(fold_hi + offB); S.v[2] = __ldg(fold + offcB); S.v[3] = __ldg(fold_hi + offcB);
+                    if (F == 2) {
+                        S.v[4] = __ldg(fold + offT); S.v[5] = __ldg(fold_hi + offT); S.v[6] = __ldg(fold + offcT); S.v[7] = __ldg(fold_hi + offcT);
+                    }
+                    offB = offcB + drowB; offT = offcT + drowT;
+                    if (cy) nexty += sgny;
+                    if (cz) nextz += sgnz;
+                    d += 1.0f;
+                    y0 = fmaf(d, r.m, r.a0);
+                    z0 = fmaf(d, rz.mz, rz.za);
+                    ++s;
+                    return true;
+                };
+                auto consume = [&](const FoldStep<F> &S) {
+                    const float wl = 1.0f - S.hi;
+                    fold_fma(accB[0], S.lo, S.v[0]); fold_fma(accB[0], wl, S.v[2]);
+                    fold_fma(accB[1], S.lo, S.v[1]); fold_fma(accB[1], wl, S.v[3]);
+                    if (F == 2) {
+                        fold_fma(accT[0], S.lo, S.v[4]); fold_fma(accT[0], wl, S.v[6]);
+                        fold_fma(accT[1], S.lo, S.v[5]); fold_fma(accT[1], wl, S.v[7]);
+                    }
+                    if (S.hi > S.lo) {      // a third cell (rare): the in-plane neighbour lies in the same quadrant here
+                        const float wm = S.hi - S.lo;
+                        const int oB = S.oB + (S.yfirst ? dcolB : dk);
+                        CBCT_DEV_ASSERT(oB >= 0 && oB < P.stage_cells);
+                        fold_fma(accB[0], wm, __ldg(fold + oB)); fold_fma(accB[1], wm, __ldg(fold_hi + oB));
+                        if (F == 2) {
+                            const int oT = S.oT + (S.yfirst ? dcolT : dk);
+                            CBCT_DEV_ASSERT(oT >= 0 && oT < P.stage_cells);
+                            fold_fma(accT[0], wm, __ldg(fold + oT)); fold_fma(accT[1], wm, __ldg(fold_hi + oT));
+                        }
+                    }
+                };
+                {
+                    FoldStep<F> SA, SB;
+                    bool ok = issue(SA);
+                    while (ok) {
+                        const bool okb = issue(SB);
+                        consume(SA);
+                        if (!okb) break;
+                        ok = issue(SA);
+                        consume(SB);
+                    }
+                }
+#else
+                for (; s < seg_end; ++s) {
+                    const float sy = __saturatef((nexty - y0) * r.inv_m);
+                    const float sz = __saturatef((nextz - z0) * rz.inv_mz);
+                    const bool cy = sy < 1.0f, cz = sz < 1.0f;
+                    if (cy && nexty == 0.0f) { mixed = true; break; }      // crosses the centre plane of the minor axis
+                    const float lo = fminf(sy, sz);
+                    const float hi = (cy && cz) ? fmaxf(sy, sz) : lo;
+                    const float wl = 1.0f - hi;
+                    const int zc = cz ? dk : 0;
+                    const int offcB = offB + (cy ? dcolB : 0) + zc, offcT = offT + (cy ? dcolT : 0) + zc;
+                    CBCT_DEV_ASSERT(offB >= 0 && offB < P.stage_cells && offcB >= 0 && offcB < P.stage_cells);
+                    CBCT_DEV_ASSERT(F == 1 || (offT >= 0 && offT < P.stage_cells && offcT >= 0 && offcT < P.stage_cells));
+                    const float4 a0 = __ldg(fold + offB), a1 = __ldg(fold_hi + offB), c0 = __ldg(fold + offcB), c1 = __ldg(fold_hi + offcB);
+                    float4 ta0, ta1, tc0, tc1;
+                    if (F == 2) {
+                        ta0 = __ldg(fold + offT); ta1 = __ldg(fold_hi + offT); tc0 = __ldg(fold + offcT); tc1 = __ldg(fold_hi + offcT);
+                    }
+                    fold_fma(accB[0], lo, a0); fold_fma(accB[0], wl, c0);
+                    fold_fma(accB[1], lo, a1); fold_fma(accB[1], wl, c1);
+                    if (F == 2) {
+                        fold_fma(accT[0], lo, ta0); fold_fma(accT[0], wl, tc0);
+                        fold_fma(accT[1], lo, ta1); fold_fma(accT[1], wl, tc1);
+                    }
+                    if (hi > lo) {      // a third cell (rare): the in-plane neighbour lies in the same quadrant here
+                        const float wm = hi - lo;
+                        const bool yfirst = sy < sz;
+                        const int oB = offB + (yfirst ? dcolB : dk);
+                        CBCT_DEV_ASSERT(oB >= 0 && oB < P.stage_cells);
+                        fold_fma(accB[0], wm, __ldg(fold + oB)); fold_fma(accB[1], wm, __ldg(fold_hi + oB));
+                        if (F == 2) {
+                            const int oT = offT + (yfirst ? dcolT : dk);
+                            CBCT_DEV_ASSERT(oT >= 0 && oT < P.stage_cells);
+                            fold_fma(accT[0], wm, __ldg(fold + oT)); fold_fma(accT[1], wm, __ldg(fold_hi + oT));
+                        }
+                    }
+                    offB = offcB + drowB; offT = offcT + drowT;
+                    if (cy) nexty += sgny;
+                    if (cz) nextz += sgnz;
+                    d += 1.0f;
+                    y0 = fmaf(d, r.m, r.a0);
+                    z0 = fmaf(d, rz.mz, rz.za);
+                }
+#endif
+                if (mixed) {
+                    // ---- the slab that crosses the minor axis' centre plane: its cells lie in two quadrants ----
+                    const float sy = __saturatef((nexty - y0) * r.inv_m);
+                    const float sz = __saturatef((nextz - z0) * rz.inv_mz);
+                    const bool cz = sz < 1.0f;                              // cy holds
+                    const float lo = fminf(sy, sz);
+                    const float hi = cz ? fmaxf(sy, sz) : lo;
+                    const float wl = 1.0f - hi;
+                    const int zc = cz ? dk : 0;
+                    const int jx = (int)nexty - (posy ? 1 : 0) + nh, kx = (int)nextz - (posz ? 1 : 0) + P.cz + PAD_Z;
+                    const int xi = r.drive ? jx : s, xj = r.drive ? s : jx;
+                    fold_cell<F>(P, fold, xi, xj, kx, lo, m, accB, accT);
+                    fold_cell<F>(P, fold, xi + mi, xj + mj, kx + zc, wl, m, accB, accT);
+                    if (hi > lo) {
+                        const bool yfirst = sy < sz;
+                        fold_cell<F>(P, fold, xi + (yfirst ? mi : 0), xj + (yfirst ? mj : 0), kx + (yfirst ? 0 : dk), hi - lo, m, accB, accT);
+                    }
+                    nexty += sgny;
+                    if (cz) nextz += sgnz;
+                    d += 1.0f;
+                    y0 = fmaf(d, r.m, r.a0);
+                    z0 = fmaf(d, rz.mz, rz.za);
+                    ++s;
+                }
+            }
+        }
+        for (int t = (4 - m) & 3; t > 0; --t) {                // back to the frame of quadrant 0: component c = quarter turn c
+            fold_rot_up(accB[0]); fold_rot_up(accB[1]);
+            if (F == 2) { fold_rot_dn(accT[0]); fold_rot_dn(accT[1]); }
+        }
+        float acc[4 * F * 2];
+#pragma unroll
+        for (int mm = 0; mm < 2; ++mm)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                acc[mm * 4 * F + q] = accB[mm][q];
+                if (F == 2) acc[mm * 4 * F + 4 + q] = accT[mm][(3 - q) & 3];
+            }
+        forward_epilogue<4, 2, MODE, F>(P, r, v, acc, a, ar, iu, iv, y, out, sq);
+    }
+    if (MODE == 1 || MODE == 4) {
+        double s[1];
+        s[0] = block_sum(sq, slot);
+        if (counter) publish_and_finalize<1>(s, 1, partials, stride, counter, sum_out, slot);
+        else publish_only<1>(s, 1, partials, stride, ((unsigned)blockIdx.z * (F == 2 ? P.npairs : P.nbase) + a) * gridDim.x + blockIdx.x);
     }
 }
 
@@ -366,6 +729,21 @@ static void launch_forward_mode(const cbct_geometry *g, const LevelParams &P, di
                                                       ctr, d_sum_sq, a_off);
 }
 
+template <int F>
+static void launch_forward_fold_mode(const cbct_geometry *g, const LevelParams &P, dim3 gr, dim3 b, cudaStream_t st, int mode,
+                                     const void *stage, const RayU *rayu, const float *d_y, float *d_out, double *d_sum_sq,
+                                     int a_off, bool fused_sum)
+{
+    unsigned int *ctr = fused_sum ? g->d_counter : nullptr;
+    const float4 *fold = reinterpret_cast<const float4 *>(stage);
+    if (mode == 0) forward_fold_kernel<0, F><<<gr, b, 0, st>>>(P, fold, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
+    else if (mode == 2) forward_fold_kernel<2, F><<<gr, b, 0, st>>>(P, fold, rayu, nullptr, d_out, nullptr, 0, nullptr, nullptr, a_off);
+    else if (mode == 4) forward_fold_kernel<4, F><<<gr, b, 0, st>>>(P, fold, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                                  ctr, d_sum_sq, a_off);
+    else forward_fold_kernel<1, F><<<gr, b, 0, st>>>(P, fold, rayu, d_y, d_out, g->d_partials, g->partials_stride,
+                                                   ctr, d_sum_sq, a_off);
+}
+
 // units of a forward launch (its grid's y dimension, and what a sharded launch splits): base views, or view pairs
 int forward_units(const Level &L) { return (L.p.nsym == 4 && L.p.nmir == 2 && L.p.nrefl == 2) ? L.p.npairs : L.p.nbase; }
 
@@ -388,7 +766,10 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     {
         StageTimer t(g, st, ST_TRANSPOSE);
         dim3 tb(32, 8);
-        if (P.nmir == 2) {
+        if (P.fold) {
+            dim3 tg((P.nhP + FOLD_T - 1) / FOLD_T, (P.nhP + FOLD_T - 1) / FOLD_T, (P.nzP + FOLD_K - 1) / FOLD_K);
+            stage_volume_fold_kernel<<<tg, 256, 0, st>>>(d_vol, reinterpret_cast<float4 *>(L.d_stage), P.nx, P.nz, P.nhP, P.nzP);
+        } else if (P.nmir == 2) {
             if (P.nx % 4 == 0 && P.nzP % 2 == 0 && (uintptr_t)d_vol % 16 == 0) {
                 dim3 tg((P.nx + STG_I - 1) / STG_I, (P.nzP + STG_K - 1) / STG_K, P.ny);
                 stage_volume_packed_vec_kernel<<<tg, 256, 0, st>>>(d_vol, reinterpret_cast<float4 *>(L.d_stage), P.nx, P.ny, P.nz,
@@ -404,9 +785,10 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         }
         CBCT_LAUNCH_CHECK(g);
     }
-    b = dim3(FWD_BV, FWD_BU);
+    const int bu = P.fold ? FOLD_BU : FWD_BU;
+    b = dim3(FWD_BV, bu);
     const int units = forward_units(L);          // base views, or view pairs where the walk also serves the reflected rays
-    dim3 gr((P.nu + FWD_BU - 1) / FWD_BU, units, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
+    dim3 gr((P.nu + bu - 1) / bu, units, (P.nv / P.nmir + FWD_BV - 1) / FWD_BV);
     const size_t nblk = (size_t)gr.x * gr.y * gr.z;             // of the full launch: the numbering of the partial sums
     if ((mode == 1 || mode == 4) && nblk > (size_t)g->partials_stride)
         return cbct_fail(CBCT_ERR_INVALID_ARG, "projection stack too large for the reduction buffer");
@@ -420,7 +802,9 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
     {
         StageTimer t(g, st, ST_FORWARD);
         const bool fused = sh == nullptr;
-        if (P.nsym == 4 && P.nmir == 2 && P.nrefl == 2) launch_forward_mode<4, 2, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        if (P.fold && P.nrefl == 2) launch_forward_fold_mode<2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.fold) launch_forward_fold_mode<1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
+        else if (P.nsym == 4 && P.nmir == 2 && P.nrefl == 2) launch_forward_mode<4, 2, 2>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
         else if (P.nsym == 4 && P.nmir == 2) launch_forward_mode<4, 2, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
         else if (P.nsym == 4) launch_forward_mode<4, 1, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);
         else if (P.nmir == 2) launch_forward_mode<1, 2, 1>(g, P, gr, b, st, mode, L.d_stage, L.d_rayu, d_y, d_out, d_sum_sq, a_off, fused);

@@ -152,6 +152,7 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
     g->tv_scalar_tiles = (desc->kernel_flags & CBCT_KERNEL_TV_SCALAR_TILES) ? 1 : 0;
     g->back_lists_on_the_fly = (desc->kernel_flags & CBCT_KERNEL_BACK_LISTS_ON_THE_FLY) ? 1 : 0;
     g->no_reflection = (desc->kernel_flags & CBCT_KERNEL_NO_REFLECTION) ? 1 : 0;
+    g->no_fold = (desc->kernel_flags & CBCT_KERNEL_NO_FOLD) ? 1 : 0;
     {   // the cooperative TV-prox kernel needs cooperative launches (every sm_100 device has them; checked all the same)
         int coop = 0;
         if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) g->host_armijo = 1;
@@ -219,6 +220,13 @@ extern "C" cbct_status cbct_geometry_create(const cbct_geometry_desc *desc, cbct
         p.jstride = p.nzP; p.istride = p.nyP * p.nzP;
         L.stage_elems = (size_t)(p.nx + 2 * PAD_M) * p.nyP * p.nzP * p.nmir;
         p.stage_cells = (int)(L.stage_elems / p.nmir);
+        // quarter-turn + mirror symmetric levels: the copy folded onto the first quadrant, 8 floats per canonical cell (forward.cu)
+        p.fold = (p.nsym == 4 && p.nmir == 2 && !g->no_fold) ? 1 : 0;
+        p.nhP = p.nx / 2 + PAD_M; p.fjs = p.nzP; p.fis = p.nhP * p.nzP;
+        if (p.fold) {
+            L.stage_elems = (size_t)p.nhP * p.nhP * p.nzP * 8;
+            p.stage_cells = (int)(L.stage_elems / 8);
+        }
         p.t_entries = (int)(L.nray / p.nsym);
         p.tP = 1; p.tXP = p.nv;
         if (L.stage_elems >= (size_t)1 << 31) { free_all(g); return cbct_fail(CBCT_ERR_INVALID_ARG, "padded volume copy exceeds 2^31 elements"); }

@@ -155,6 +155,39 @@ def test_forward_projector_view_pairs_agree_with_base_views(torch, cbct, orc):
         assert h.shard_units(0)[0] == g.n_proj // 4            # no pairing with the detector off-centre
 
 
+def test_forward_projector_folded_copy_changes_no_bit(torch, cbct, orc):
+    """Quarter-turn + mirror symmetric levels read the staged copy FOLDED onto the first quadrant (one 32-byte entry = a cell's
+    four quarter-turn images and their z-mirrors; the sums are kept in the frame of the walk's current quadrant and turned when
+    it changes); CBCT_KERNEL_NO_FOLD keeps one 8-byte cell per image.  Same weights in the same order: bitwise equal projections
+    -- with and without view pairs, with an odd and an even number of base views, on a grid whose rays cross the centre plane of
+    the minor axis at every slope (all views of a full turn), with a detector that looks past the volume (rows and columns that
+    miss it, rays that leave through the top), and within 1e-5 of the oracle."""
+    cases = {"even": I.Geometry(nx=40, ny=40, nz=18, hx=1.5, hy=1.5, hz=2.0, nu=72, nv=30, du=1.3, dv=1.6, sad=600.0, sdd=900.0,
+                                n_proj=16),
+             "odd": I.Geometry(nx=40, ny=40, nz=18, hx=1.5, hy=1.5, hz=2.0, nu=72, nv=30, du=1.3, dv=1.6, sad=600.0, sdd=900.0,
+                               n_proj=12),
+             "wide": I.Geometry(nx=24, ny=24, nz=40, hx=2.0, hy=2.0, hz=1.0, nu=96, nv=64, du=1.5, dv=1.5, sad=300.0, sdd=500.0,
+                                n_proj=20),
+             # quarter turns without the reflection (first view off 0 degrees): the folded walk of 8 rays
+             "turned": I.Geometry(nx=40, ny=40, nz=18, hx=1.5, hy=1.5, hz=2.0, nu=72, nv=30, du=1.3, dv=1.6, sad=600.0, sdd=900.0,
+                                  n_proj=16, angles=np.deg2rad(11.0) + 2 * np.pi * np.arange(16) / 16),
+             "config1": GEOMS["config1"], "aniso": GEOMS["aniso"], "wide8": GEOMS["wide8"]}
+    for name, g in cases.items():
+        f = I.uniform_volume(g, 23)
+        want = orc.forward(g, f)
+        for no_refl in (False, True):
+            outs = {}
+            for no_fold in (False, True):
+                with cbct.geometry_create(g, no_reflection=no_refl, no_fold=no_fold) as h:
+                    assert h.symmetry == 8, name
+                    p = torch.empty(g.proj_shape, device="cuda", dtype=torch.float32)
+                    h.forward_project(dev(torch, f), p)
+                    outs[no_fold] = p.cpu().numpy()
+            for a in range(g.n_proj):
+                assert rel_l2(outs[False][a], want[a]) <= TOL_PROJ, (name, no_refl, a)
+            assert outs[False].tobytes() == outs[True].tobytes(), (name, no_refl, float(np.abs(outs[False] - outs[True]).max()))
+
+
 @pytest.mark.parametrize("name", ["ragged", "sym48"])
 def test_projectors_are_bitwise_deterministic(torch, cbct, name):
     g = GEOMS[name]
