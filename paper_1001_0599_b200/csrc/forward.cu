@@ -342,14 +342,14 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
 // Margins: canonical coordinates run from -PAD_M (a cell outside the grid folds to a negative canonical coordinate); those
 // entries, and the components of k outside the grid, are written as zeros by the staging kernel.
 
-constexpr int FOLD_T = 16, FOLD_K = 4;       // staging tile: 16 x 16 canonical cells x 4 cells in kk
+constexpr int FOLD_T = 16, FOLD_K = 8;       // staging tile: 16 x 16 canonical cells x 8 cells in kk of one half (k, or its mirror)
 // vol [k][j][i] -> fold[half][(i0+PM)][(j0+PM)][kk] (float4): every image's 16 x 16 patch is read with x fastest (64-byte runs) and
-// the tile leaves as 64-byte runs (4 entries of one canonical column and half).
+// the tile leaves as 128-byte runs (8 entries of one canonical column).  blockIdx.z = 2 * (tile in kk) + half.
 __global__ void __launch_bounds__(256)
 stage_volume_fold_kernel(const float *__restrict__ in, float4 *__restrict__ fold, int n, int nz, int nhP, int nzP)
 {
-    __shared__ float tile[2][4][FOLD_K][FOLD_T][FOLD_T + 1];         // [half][q][kk][i0][j0]
-    const int a0 = blockIdx.x * FOLD_T, b0 = blockIdx.y * FOLD_T, kk0 = blockIdx.z * FOLD_K;
+    __shared__ float tile[4][FOLD_K][FOLD_T][FOLD_T + 1];            // [q][kk][i0][j0]
+    const int a0 = blockIdx.x * FOLD_T, b0 = blockIdx.y * FOLD_T, kk0 = (blockIdx.z >> 1) * FOLD_K, half = blockIdx.z & 1;
     const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4, n1 = n - 1;
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
@@ -366,24 +366,19 @@ stage_volume_fold_kernel(const float *__restrict__ in, float4 *__restrict__ fold
         const bool inpl = i0 >= 0 && j0 >= 0 && i0 < n / 2 && j0 < n / 2;
 #pragma unroll
         for (int c = 0; c < FOLD_K; ++c) {
-            const int k = kk0 + c - PAD_Z, km = nz - 1 - k;
-            float lo = 0.0f, hi = 0.0f;
-            if (inpl && k >= 0 && k < nz) {                          // km is in range exactly when k is
-                lo = __ldg(in + ((size_t)k * n + y) * n + x);
-                hi = __ldg(in + ((size_t)km * n + y) * n + x);
-            }
-            tile[0][q][c][il][jl] = lo; tile[1][q][c][il][jl] = hi;
+            const int k = kk0 + c - PAD_Z, ks = half ? nz - 1 - k : k;       // the mirror is in range exactly when k is
+            tile[q][c][il][jl] = (inpl && k >= 0 && k < nz) ? __ldg(in + ((size_t)ks * n + y) * n + x) : 0.0f;
         }
     }
     __syncthreads();
-    const int f4 = threadIdx.x & 7, c = f4 >> 1, half = f4 & 1;      // 8 float4 = 4 entries = 128 bytes per canonical column
+    const int c = threadIdx.x & 7;                                   // 8 float4 = 8 entries = 128 bytes per canonical column
 #pragma unroll
     for (int it = 0; it < 8; ++it) {
         const int cell = (threadIdx.x >> 3) + 32 * it, il = cell >> 4, jl = cell & 15;
         const int a = a0 + il, b = b0 + jl, kk = kk0 + c;
         if (a < nhP && b < nhP && kk < nzP)
             fold[(size_t)half * nhP * nhP * nzP + ((size_t)a * nhP + b) * nzP + kk] =
-                make_float4(tile[half][0][c][il][jl], tile[half][1][c][il][jl], tile[half][2][c][il][jl], tile[half][3][c][il][jl]);
+                make_float4(tile[0][c][il][jl], tile[1][c][il][jl], tile[2][c][il][jl], tile[3][c][il][jl]);
     }
 }
 
@@ -767,7 +762,7 @@ cbct_status launch_forward(const cbct_geometry *g, const Level &L, const float *
         StageTimer t(g, st, ST_TRANSPOSE);
         dim3 tb(32, 8);
         if (P.fold) {
-            dim3 tg((P.nhP + FOLD_T - 1) / FOLD_T, (P.nhP + FOLD_T - 1) / FOLD_T, (P.nzP + FOLD_K - 1) / FOLD_K);
+            dim3 tg((P.nhP + FOLD_T - 1) / FOLD_T, (P.nhP + FOLD_T - 1) / FOLD_T, 2 * ((P.nzP + FOLD_K - 1) / FOLD_K));
             stage_volume_fold_kernel<<<tg, 256, 0, st>>>(d_vol, reinterpret_cast<float4 *>(L.d_stage), P.nx, P.nz, P.nhP, P.nzP);
         } else if (P.nmir == 2) {
             if (P.nx % 4 == 0 && P.nzP % 2 == 0 && (uintptr_t)d_vol % 16 == 0) {
