@@ -445,16 +445,9 @@ __device__ __forceinline__ void fold_cell(const LevelParams &P, const float4 *__
 #ifndef FOLD_MINB1
 #define FOLD_MINB1 2
 #endif
-#ifndef FOLD_PIPE
-#define FOLD_PIPE 0
-#endif
-// one slab step in flight: its crossing parameters, the offsets its rare third cell needs, its loaded entries
-template <int F> struct FoldStep {
-    float lo, hi;
-    int oB, oT;
-    bool yfirst;
-    float4 v[4 * F];
-};
+#ifndef FOLD_DEFER
+#define FOLD_DEFER 1        // 1: the view-pair walk fetches the z-neighbour cell of a slab without an in-plane crossing in batches
+#endif                      // (see the kernel; measured slower on the 8-ray walk: 0.682 against 0.637 ms at config 3)
 // forward_kernel<4, 2, MODE, F> on the folded copy: same grid, same rays per thread, same epilogue.
 template <int MODE, int F>
 __global__ void __launch_bounds__(FWD_BV *FOLD_BU, F == 2 ? FOLD_MINB2 : FOLD_MINB1)
@@ -517,72 +510,45 @@ forward_fold_kernel(const LevelParams P, const float4 *__restrict__ fold, const 
                 const int dcolB = c0i * P.fis + c0j * P.fjs, dcolT = c0j * P.fis + c0i * P.fjs;
                 const int seg_end = s < nh ? min(nh, s_hi) : s_hi;
                 bool mixed = false;
-#if FOLD_PIPE
-                // Two slab steps in flight: the loads of slab s + 1 are issued before the sums of slab s are formed (two sets of
-                // load registers, the loop unrolled by two so that neither is ever moved).
-                auto issue = [&](FoldStep<F> &S) -> bool {
-                    if (s >= seg_end) return false;
-                    const float sy = __saturatef((nexty - y0) * r.inv_m);
-                    const float sz = __saturatef((nextz - z0) * rz.inv_mz);
-                    const bool cy = sy < 1.0f, cz = sz < 1.0f;
-                    if (cy && nexty == 0.0f) { mixed = true; return false; }   // crosses the centre plane of the minor axis
-                    S.lo = fminf(sy, sz);
-                    S.hi = (cy && cz) ? fmaxf(sy, sz) : S.lo;
-                    const int zc = cz ? dk : 0;
-                    const int offcB = offB + (cy ? dcolB : 0) + zc, offcT = offT + (cy ? dcolT : 0) + zc;
-                    CBCT_DEV_ASSERT(offB >= 0 && offB < P.stage_cells && offcB >= 0 && offcB < P.stage_cells);
-                    CBCT_DEV_ASSERT(F == 1 || (offT >= 0 && offT < P.stage_cells && offcT >= 0 && offcT < P.stage_cells));
-                    S.yfirst = sy < sz; S.oB = offB; S.oT = offT;
-                    S.v[0] = __ldg(fold + offB); S.v[1] = __ldg(fold_hi + offB); S.v[2] = __ldg(fold + offcB); S.v[3] = __ldg(fold_hi + offcB);
-                    if (F == 2) {
-                        S.v[4] = __ldg(fold + offT); S.v[5] = __ldg(fold_hi + offT); S.v[6] = __ldg(fold + offcT); S.v[7] = __ldg(fold_hi + offcT);
-                    }
-                    offB = offcB + drowB; offT = offcT + drowT;
-                    if (cy) nexty += sgny;
-                    if (cz) nextz += sgnz;
-                    d += 1.0f;
-                    y0 = fmaf(d, r.m, r.a0);
-                    z0 = fmaf(d, rz.mz, rz.za);
-                    ++s;
-                    return true;
-                };
-                auto consume = [&](const FoldStep<F> &S) {
-                    const float wl = 1.0f - S.hi;
-                    fold_fma(accB[0], S.lo, S.v[0]); fold_fma(accB[0], wl, S.v[2]);
-                    fold_fma(accB[1], S.lo, S.v[1]); fold_fma(accB[1], wl, S.v[3]);
-                    if (F == 2) {
-                        fold_fma(accT[0], S.lo, S.v[4]); fold_fma(accT[0], wl, S.v[6]);
-                        fold_fma(accT[1], S.lo, S.v[5]); fold_fma(accT[1], wl, S.v[7]);
-                    }
-                    if (S.hi > S.lo) {      // a third cell (rare): the in-plane neighbour lies in the same quadrant here
-                        const float wm = S.hi - S.lo;
-                        const int oB = S.oB + (S.yfirst ? dcolB : dk);
-                        CBCT_DEV_ASSERT(oB >= 0 && oB < P.stage_cells);
-                        fold_fma(accB[0], wm, __ldg(fold + oB)); fold_fma(accB[1], wm, __ldg(fold_hi + oB));
-                        if (F == 2) {
-                            const int oT = S.oT + (S.yfirst ? dcolT : dk);
-                            CBCT_DEV_ASSERT(oT >= 0 && oT < P.stage_cells);
-                            fold_fma(accT[0], wm, __ldg(fold + oT)); fold_fma(accT[1], wm, __ldg(fold_hi + oT));
-                        }
+                constexpr bool DEFER = FOLD_DEFER && F == 2;
+                int pB = 0, pT = 0;
+                float pw = 0.0f;                                     // the noted z-neighbour cell of this lane and its weight (0: none)
+                auto flush = [&]() {
+                    if (pw > 0.0f) {
+                        CBCT_DEV_ASSERT(pB >= 0 && pB < P.stage_cells && (F == 1 || (pT >= 0 && pT < P.stage_cells)));
+                        fold_fma(accB[0], pw, __ldg(fold + pB)); fold_fma(accB[1], pw, __ldg(fold_hi + pB));
+                        if (F == 2) { fold_fma(accT[0], pw, __ldg(fold + pT)); fold_fma(accT[1], pw, __ldg(fold_hi + pT)); }
+                        pw = 0.0f;
                     }
                 };
-                {
-                    FoldStep<F> SA, SB;
-                    bool ok = issue(SA);
-                    while (ok) {
-                        const bool okb = issue(SB);
-                        consume(SA);
-                        if (!okb) break;
-                        ok = issue(SA);
-                        consume(SB);
-                    }
-                }
-#else
                 for (; s < seg_end; ++s) {
                     const float sy = __saturatef((nexty - y0) * r.inv_m);
                     const float sz = __saturatef((nextz - z0) * rz.inv_mz);
                     const bool cy = sy < 1.0f, cz = sz < 1.0f;
                     if (cy && nexty == 0.0f) { mixed = true; break; }      // crosses the centre plane of the minor axis
+                    if (DEFER && !cy) {
+                        // No in-plane crossing in this slab -- the same for every lane of the warp.  The first cell takes sz (1
+                        // unless the lane crosses a z-plane here); the z-neighbour's share 1 - sz is owed by the few lanes that do
+                        // cross.  The walk is bound by the bytes its loads REQUEST (a 16-byte load costs the LSU four passes however
+                        // many lanes are predicated off), so that cell is not fetched now: the lane notes its offset and weight, and
+                        // the warp fetches all noted cells at once when a lane must note a second one (and at the end of the run).
+                        const bool ov = cz && pw > 0.0f;
+                        if (__any_sync(__activemask(), ov)) flush();
+                        CBCT_DEV_ASSERT(offB >= 0 && offB < P.stage_cells && (F == 1 || (offT >= 0 && offT < P.stage_cells)));
+                        const float4 a0 = __ldg(fold + offB), a1 = __ldg(fold_hi + offB);
+                        float4 ta0, ta1;
+                        if (F == 2) { ta0 = __ldg(fold + offT); ta1 = __ldg(fold_hi + offT); }
+                        const int zc = cz ? dk : 0;
+                        if (cz) { pB = offB + dk; pT = offT + dk; pw = 1.0f - sz; }
+                        fold_fma(accB[0], sz, a0); fold_fma(accB[1], sz, a1);
+                        if (F == 2) { fold_fma(accT[0], sz, ta0); fold_fma(accT[1], sz, ta1); }
+                        offB += zc + drowB; offT += zc + drowT;
+                        if (cz) nextz += sgnz;
+                        d += 1.0f;
+                        y0 = fmaf(d, r.m, r.a0);
+                        z0 = fmaf(d, rz.mz, rz.za);
+                        continue;
+                    }
                     const float lo = fminf(sy, sz);
                     const float hi = (cy && cz) ? fmaxf(sy, sz) : lo;
                     const float wl = 1.0f - hi;
@@ -620,7 +586,7 @@ forward_fold_kernel(const LevelParams P, const float4 *__restrict__ fold, const 
                     y0 = fmaf(d, r.m, r.a0);
                     z0 = fmaf(d, rz.mz, rz.za);
                 }
-#endif
+                if (DEFER) flush();                                  // before the frame of the sums changes
                 if (mixed) {
                     // ---- the slab that crosses the minor axis' centre plane: its cells lie in two quadrants ----
                     const float sy = __saturatef((nexty - y0) * r.inv_m);

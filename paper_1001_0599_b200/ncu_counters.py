@@ -20,7 +20,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 
 # kernel-name prefix -> bench.py's stage name
-STAGES = {"forward_kernel": "forward", "back_tma_kernel": "back", "back_list_kernel": "back", "back_kernel": "back",
+STAGES = {"forward_kernel": "forward", "forward_fold_kernel": "forward", "stage_volume_fold_kernel": "transpose",
+          "back_tma_kernel": "back", "back_list_kernel": "back", "back_kernel": "back",
           "tv_grad_kernel": "tv_grad", "tv_energy_kernel": "tv_trial", "tv_update_kernel": "tv_update",
           "stage_volume_packed_kernel": "transpose", "stage_volume_packed_vec_kernel": "transpose",
           "stage_volume_kernel": "transpose", "tv_prox_coop_kernel": "tv_prox"}
@@ -39,6 +40,9 @@ METRICS = {
     "smsp__inst_executed.sum": "warp_instructions",
     "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum": "shared_wavefronts",
     "l1tex__t_sectors_pipe_lsu_mem_global_op_ld.sum": "l1_global_load_sectors",
+    "l1tex__data_pipe_lsu_wavefronts.sum": "l1_data_pipe_wavefronts",
+    "l1tex__data_pipe_lsu_wavefronts.avg.pct_of_peak_sustained_elapsed": "l1_data_pipe_pct",
+    "l1tex__t_requests_pipe_lsu_mem_global_op_ld.sum": "l1_global_load_requests",
 }
 UNIT_SCALE = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0, "ms": 1e3, "us": 1.0, "ns": 1e-3, "s": 1e6, "second": 1e6,
               "msecond": 1e3, "usecond": 1.0, "nsecond": 1e-3}

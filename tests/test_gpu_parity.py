@@ -155,10 +155,10 @@ def test_forward_projector_view_pairs_agree_with_base_views(torch, cbct, orc):
         assert h.shard_units(0)[0] == g.n_proj // 4            # no pairing with the detector off-centre
 
 
-def test_forward_projector_folded_copy_changes_no_bit(torch, cbct, orc):
+def test_forward_projector_folded_copy_agrees_with_per_image_cells(torch, cbct, orc):
     """Quarter-turn + mirror symmetric levels read the staged copy FOLDED onto the first quadrant (one 32-byte entry = a cell's
     four quarter-turn images and their z-mirrors; the sums are kept in the frame of the walk's current quadrant and turned when
-    it changes); CBCT_KERNEL_NO_FOLD keeps one 8-byte cell per image.  Same weights in the same order: bitwise equal projections
+    it changes); CBCT_KERNEL_NO_FOLD keeps one 8-byte cell per image.  Same weights: projections equal to fp32 rounding
     -- with and without view pairs, with an odd and an even number of base views, on a grid whose rays cross the centre plane of
     the minor axis at every slope (all views of a full turn), with a detector that looks past the volume (rows and columns that
     miss it, rays that leave through the top), and within 1e-5 of the oracle."""
@@ -185,7 +185,9 @@ def test_forward_projector_folded_copy_changes_no_bit(torch, cbct, orc):
                     outs[no_fold] = p.cpu().numpy()
             for a in range(g.n_proj):
                 assert rel_l2(outs[False][a], want[a]) <= TOL_PROJ, (name, no_refl, a)
-            assert outs[False].tobytes() == outs[True].tobytes(), (name, no_refl, float(np.abs(outs[False] - outs[True]).max()))
+            # same weights; the z-neighbour cells of slabs without an in-plane crossing are added in batches (another order of the
+            # same terms): equal to fp32 rounding
+            assert rel_l2(outs[False], outs[True]) <= 1e-6, (name, no_refl, rel_l2(outs[False], outs[True]))
 
 
 @pytest.mark.parametrize("name", ["ragged", "sym48"])
