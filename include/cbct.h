@@ -187,6 +187,25 @@ cbct_status cbct_tv_energy(const cbct_geometry *g, int level, const float *d_f, 
 cbct_status cbct_quality_metrics(const cbct_geometry *g, int level, const float *d_f, const float *d_f0,
                                  double *rel_error, double *correlation, void *cuda_stream);
 
+/* The same two metrics for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): needs NO geometry handle and calls no cudaMalloc, cudaFree or allocating routine.
+ *   d_f, d_f0 : DEVICE, n floats each (caller-owned, read only);   d_out2 : DEVICE, 2 doubles: (rel_error, correlation).
+ * Asynchronous on `cuda_stream` (no synchronisation, no host copy: read d_out2 after the stream has reached this call).
+ * Scratch (fp64 block partials + a ticket) is a static __device__ array of CBCT_STATIC_SCRATCH_BYTES inside the library,
+ * held by every GPU that loads it until the process exits; a block sums a fixed chunk of CBCT_STATIC_CHUNK elements, so the
+ * summation order depends on n alone and n is limited to CBCT_STATIC_MAX_ELEMS (2^28 elements = 1 GiB per volume):
+ * CBCT_ERR_INVALID_ARG beyond it (use cbct_quality_metrics), for n = 0 and for NULL buffers.  The first call on a device
+ * looks the array's address up (cudaGetSymbolAddress): make that call once before capturing a graph.
+ * ALL calls share the scratch: calls that overlap on the GPU (two streams, two host threads) race on it -- serialise them.
+ * The ticket is cleared on the stream before every launch, so a call that failed half-way does not disturb the next.
+ * Same sums as cbct_quality_metrics in another fixed order: the two agree to fp64 rounding (~1e-13 relative). */
+#define CBCT_STATIC_CHUNK 16384
+#define CBCT_STATIC_MAX_BLOCKS 16384
+#define CBCT_STATIC_MAX_ELEMS 268435456ull
+#define CBCT_STATIC_SCRATCH_BYTES (8 * (6 * CBCT_STATIC_MAX_BLOCKS + 32))
+cbct_status cbct_quality_metrics_static(const float *d_f, const float *d_f0, unsigned long long n, double *d_out2,
+                                        void *cuda_stream);
+
 /* A8 grid transfers (L215-L223; readings S12, S13).  `level` is the FINE level of the pair.  Buffers need only
  * their natural 4-byte alignment (8-byte aligned fine buffers take a faster load path).
  *   restrict: fine volume -> 2x2x2 mean on level+1.   bin: fine projections -> 2x2 mean.

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcbct.so")
-SOURCES = ["geometry.cu", "forward.cu", "back.cu", "back_tma.cu", "back_eq6.cu", "tv.cu", "transfer.cu", "metrics.cu", "fbs.cu", "calib.cu"]
+SOURCES = ["geometry.cu", "forward.cu", "back.cu", "back_tma.cu", "back_eq6.cu", "tv.cu", "transfer.cu", "metrics.cu", "metrics_static.cu", "fbs.cu", "calib.cu"]
 HEADERS = ["cbct_internal.cuh", "ray.cuh", "reduce.cuh", os.path.join("..", "..", "include", "cbct.h")]
 # static cudart (nvcc's default): no run-time dependency on a libcudart path; device pointers and
 # streams made by torch's runtime are valid here because both use the device's primary context.

@@ -30,7 +30,7 @@ EXPORTS = [
     "cbct_geometry_create", "cbct_geometry_destroy", "cbct_geometry_symmetry", "cbct_geometry_device_bytes",
     "cbct_geometry_back_path", "cbct_bound_violations",
     "cbct_forward_project", "cbct_back_project", "cbct_back_project_eq6", "cbct_count_samples", "cbct_step_bound", "cbct_tv_prox", "cbct_tv_energy",
-    "cbct_quality_metrics",
+    "cbct_quality_metrics", "cbct_quality_metrics_static",
     "cbct_restrict_volume", "cbct_bin_projections", "cbct_prolong_volume",
     "cbct_fbs_reconstruct", "cbct_fbs_reconstruct_host", "cbct_fbs_reconstruct_sharded", "cbct_shard_range",
     "cbct_shard_units", "cbct_launch_count",
@@ -135,6 +135,7 @@ def load_library():
     lib.cbct_count_samples.argtypes = [vp, ip, C.POINTER(C.c_ulonglong), vp]
     lib.cbct_step_bound.argtypes = [vp, ip, C.POINTER(dp), vp]
     lib.cbct_quality_metrics.argtypes = [vp, ip, vp, vp, C.POINTER(dp), C.POINTER(dp), vp]
+    lib.cbct_quality_metrics_static.argtypes = [vp, vp, C.c_ulonglong, vp, vp]
     lib.cbct_tv_prox.argtypes = [vp, ip, vp, vp, dp, ip, C.POINTER(_TvParams), C.POINTER(_TvReport), vp]
     lib.cbct_tv_energy.argtypes = [vp, ip, vp, dp, C.POINTER(dp), vp]
     lib.cbct_restrict_volume.argtypes = [vp, ip, vp, vp, vp]
@@ -498,6 +499,28 @@ def geometry_create(desc, max_levels: int = 1, no_symmetry: bool = False, no_tma
                     no_reflection: bool = False, no_fold: bool = False) -> Geometry:
     return Geometry(desc, max_levels, no_symmetry, no_tma, host_armijo, tv_scalar_tiles, back_lists_on_the_fly, no_reflection,
                     no_fold)
+
+
+STATIC_MAX_ELEMS = 1 << 28      # CBCT_STATIC_MAX_ELEMS
+
+
+def quality_metrics_static(f, f0, out2, stream=None, n: int | None = None):
+    """cbct_quality_metrics_static: (e, c) of f against f0 into the 2-element float64 CUDA tensor `out2`, asynchronously on the
+    stream; no geometry handle, no allocation (the scratch is a static __device__ array inside the library, shared by all
+    calls: do not overlap them).  `n` (default: all elements of f) may not exceed STATIC_MAX_ELEMS."""
+    import torch
+    n = f.numel() if n is None else int(n)
+    if not (isinstance(out2, torch.Tensor) and out2.is_cuda and out2.dtype == torch.float64 and out2.is_contiguous()
+            and out2.numel() == 2):
+        raise TypeError("out2: need a contiguous float64 CUDA tensor of 2 elements")
+    for name, t in (("f", f), ("f0", f0)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+            raise TypeError(f"{name}: need a contiguous float32 CUDA tensor")
+        if n <= STATIC_MAX_ELEMS and t.numel() < n:        # beyond the maximum the library refuses before it reads anything
+            raise ValueError(f"{name}: {t.numel()} elements, fewer than n = {n}")
+    _check(load_library().cbct_quality_metrics_static(C.c_void_p(f.data_ptr()), C.c_void_p(f0.data_ptr()), C.c_ulonglong(n),
+                                                      C.c_void_p(out2.data_ptr()), _stream_ptr(stream)))
+    return out2
 
 
 def version() -> str:
