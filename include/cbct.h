@@ -86,7 +86,8 @@ typedef struct {
 #define CBCT_KERNEL_NO_FOLD 32 /* the forward projector of a quarter-turn + mirror symmetric level reads one staged cell per image of
                                   a ray (8 or 16 loads of 8 bytes per slab step) instead of the copy folded onto the first
                                   quadrant (one 32-byte entry holds a cell's four quarter-turn images and their z-mirrors);
-                                  same bits either way.  For A/B measurements and tests. */
+                                  same weights either way (bitwise equal projections without view pairs; with them the folded
+                                  walk adds some terms in another order: equal to ~4e-8).  For A/B measurements and tests. */
 #define CBCT_KERNEL_TV_SCALAR_TILES 4 /* the TV passes always on the 32-voxel warp tiles (one voxel per lane), never on the
                                          16-byte tiles that volumes with nx % 4 == 0, nx >= 128 and 16-byte aligned buffers
                                          otherwise take; same stencil, for A/B measurements and tests. */

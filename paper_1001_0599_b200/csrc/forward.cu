@@ -338,7 +338,8 @@ forward_kernel(const LevelParams P, const void *__restrict__ stage_v, const RayU
 // 16 bytes at 4 offsets.  The sums are kept in the frame of the current quadrant (accumulator c belongs to component c) and
 // rotated when the walk changes quadrant -- at the centre plane of the driving axis, between two slabs, and in the one slab
 // where the ray crosses the centre plane of the minor axis, which takes a generic path (fold_cell); a walk changes quadrant
-// at most three times.  Same weights, same order of the FMAs of every ray as forward_kernel: the same bits.
+// at most three times.  Same weights as forward_kernel; the 8-ray walk adds them in the same order (the same bits), the
+// view-pair walk adds the z-neighbour cells of slabs without an in-plane crossing in batches (FOLD_DEFER: equal to 4e-8).
 // Margins: canonical coordinates run from -PAD_M (a cell outside the grid folds to a negative canonical coordinate); those
 // entries, and the components of k outside the grid, are written as zeros by the staging kernel.
 
