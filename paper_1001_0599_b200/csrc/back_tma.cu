@@ -312,10 +312,13 @@ back_tma_kernel(const __grid_constant__ BtMaps maps, const LevelParams P, const 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // within a brick the slices nearest to the central plane first (the truncated bottom units are the cheap ones)
     constexpr int ZPB = 32 * ZV;                       // slices per block
-    // grid = (z-units, bricks in i, bricks in j): the z-units of a brick are neighbours in launch order, run at the same time and
-    // share the brick's list-table lines in L2 (with the z-unit slowest every unit re-read the 84 MB table from DRAM: 445 MB of
-    // DRAM reads per launch at config 3, 218 MB now)
-    const int bz = blockIdx.x, bx = blockIdx.y, by = blockIdx.z, gx = gridDim.y, gy = gridDim.z;
+    // Q.zu_fast: grid = (z-units, bricks in i, bricks in j) -- the z-units of a brick are neighbours in launch order, run at the
+    // same time and share the brick's list-table lines in L2 (with the z-unit slowest every unit re-reads the table from DRAM:
+    // 445 MB of DRAM reads per launch at config 3, 218 MB so).  Where the residual stack itself does not fit L2 (360 views of
+    // 512 x 384: 283 MB) the z-unit stays the slowest index, so that the blocks in flight share one band of detector rows.
+    const bool zf = Q.zu_fast != 0;
+    const int bz = zf ? blockIdx.x : blockIdx.z, bx = zf ? blockIdx.y : blockIdx.x, by = zf ? blockIdx.z : blockIdx.y;
+    const int gx = zf ? gridDim.y : gridDim.x, gy = zf ? gridDim.z : gridDim.y;
     const int i0 = bx * BI, j0 = by * BJ, k0 = (kb_top - 1 - bz) * ZPB;     // kb_top: one past the last z-unit of this launch
     const int ni = P.nx / 2, nj = P.ny / 2, n1 = P.nx - 1;
     const int n_stages = 4 * P.nbase;
@@ -590,7 +593,7 @@ cbct_status bt_launch(const Level &L, const float *d_f, float coef, float *d_out
     dim3 gr((ni + BI - 1) / BI, (nj + BJ - 1) / BJ, (B.q.nzh + 32 * ZV - 1) / (32 * ZV)), b((BI * BJ / CPW + 1) * 32);
     int kb_top = gr.z;
     if (sh) { kb_top = sh->zu_hi; gr.z = sh->zu_hi - sh->zu_lo; if (gr.z == 0) return CBCT_OK; }
-    gr = dim3(gr.z, gr.x, gr.y);        // z-unit fastest (see the kernel)
+    if (B.q.zu_fast) gr = dim3(gr.z, gr.x, gr.y);        // z-unit fastest (see the kernel)
     kern<<<gr, b, B.q.total, st>>>(B.maps, P, B.q, L.d_rayu, L.d_view, d_f, coef, d_out, errflag, kb_top, B.d_lists, B.d_hdrs);
     return CBCT_OK;
 }
@@ -611,7 +614,13 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     // a voxel's shadow narrower than ~1.5 detector columns (in-plane voxels much finer than the pixels, config 4 and the
     // 512^3 sweep): a 4 x 4 brick then has too little work per stage for the tile ring to pay; measured 18.4 ms against
     // the list kernel's 16.4 ms at config 4, 0.84 ms against 0.95 ms at config 3 (shadow 1.9 columns)
-    if (d.sdd / d.sad * fmin(L.hx, L.hy) / L.du < 1.5) return CBCT_OK;
+#ifndef BT_MIN_SHADOW
+#define BT_MIN_SHADOW 1.5
+#endif
+#ifndef BT_MAX_TABLE_GIB
+#define BT_MAX_TABLE_GIB 2
+#endif
+    if (d.sdd / d.sad * fmin(L.hx, L.hy) / L.du < BT_MIN_SHADOW) return CBCT_OK;
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return CBCT_OK;
     const int BI = 4, BJ = 4;
@@ -687,6 +696,7 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
         if (q.total <= 227 * 1024) ZV = zv;
     }
     if (!ZV) return CBCT_OK;
+    q.zu_fast = (L.nray * sizeof(float) <= ((size_t)64 << 20)) ? 1 : 0;     // the residual stack stays in L2 beside the lists
     q.ic_scale = (float)K;
     q.c0v_m = (float)c0v_m;
     q.vec4 = (P.nx % 4 == 0 && BI % 4 == 0 && BJ % 4 == 0) ? 1 : 0;
@@ -713,7 +723,7 @@ cbct_status bt_plan_level(const cbct_geometry *g, Level &L)
     // image has more than BT_TABH hitting columns somewhere, when the table would pass 2 GB, or on request.
     B.d_lists = nullptr;
     const size_t n_lists = (size_t)ni * nj * P.nbase, bytes = n_lists * 512;
-    if (ZV == 1 && !g->back_lists_on_the_fly && bytes <= ((size_t)2 << 30)) {
+    if (ZV == 1 && !g->back_lists_on_the_fly && bytes <= ((size_t)BT_MAX_TABLE_GIB << 30)) {
         float4 *tab = nullptr;
         unsigned int *ovf = nullptr;
         if (cudaMalloc((void **)&tab, bytes) != cudaSuccess || cudaMalloc((void **)&ovf, sizeof(unsigned int)) != cudaSuccess) {

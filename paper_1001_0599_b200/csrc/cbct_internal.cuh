@@ -74,6 +74,7 @@ struct BtParams {
     int list_off, view_off, hdr_off, bar_off, total;   // shared-memory carve-up (bytes)
     int nzh;                    // nz / 2
     int vec4;                   // results may leave with 16-byte stores
+    int zu_fast;                // launch order: the z-units of a brick next to one another (else the z-unit is the slowest index)
     float ic_scale;             // hz * sdd / dv: detector rows per z-index at unit depth
     float c0v_m;                // -v0 / dv - 2e-3: row index of v = 0, minus the range tolerance
 };
