@@ -75,3 +75,25 @@ def test_static_metrics_refuse_sizes_beyond_the_scratch():
     cbct.quality_metrics_static(a, a, out)                                        # and the entry point still works: all-zero volumes
     torch.cuda.synchronize()
     assert out.cpu().tolist() == [0.0, 0.0]
+
+
+def test_static_metrics_argument_checks_need_no_gpu():
+    """NULL buffers, n = 0 and n beyond CBCT_STATIC_MAX_ELEMS are refused before the first CUDA call: checked here without a
+    device (the pointers are never dereferenced)."""
+    import ctypes as C
+    from paper_1001_0599_b200 import cbct
+    lib = cbct.load_library()
+    fake = C.c_void_p(0x1000)
+    call = lib.cbct_quality_metrics_static
+    assert call(None, fake, C.c_ulonglong(8), fake, None) == 1                     # CBCT_ERR_INVALID_ARG
+    assert call(fake, fake, C.c_ulonglong(8), None, None) == 1
+    assert call(fake, fake, C.c_ulonglong(0), fake, None) == 1
+    assert call(fake, fake, C.c_ulonglong(cbct.STATIC_MAX_ELEMS + 1), fake, None) == 1
+    assert b"CBCT_STATIC_MAX_ELEMS" in lib.cbct_last_error()
+    # the header's limits are the binding's
+    import os, re
+    text = open(os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "cbct.h")).read()
+    assert int(re.search(r"#define CBCT_STATIC_MAX_ELEMS (\d+)ull", text).group(1)) == cbct.STATIC_MAX_ELEMS
+    chunk = int(re.search(r"#define CBCT_STATIC_CHUNK (\d+)", text).group(1))
+    blocks = int(re.search(r"#define CBCT_STATIC_MAX_BLOCKS (\d+)", text).group(1))
+    assert chunk * blocks == cbct.STATIC_MAX_ELEMS
