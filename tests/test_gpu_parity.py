@@ -171,6 +171,9 @@ def test_forward_projector_folded_copy_agrees_with_per_image_cells(torch, cbct, 
              # quarter turns without the reflection (first view off 0 degrees): the folded walk of 8 rays
              "turned": I.Geometry(nx=40, ny=40, nz=18, hx=1.5, hy=1.5, hz=2.0, nu=72, nv=30, du=1.3, dv=1.6, sad=600.0, sdd=900.0,
                                   n_proj=16, angles=np.deg2rad(11.0) + 2 * np.pi * np.arange(16) / 16),
+             # a first quadrant of 18 x 18 cells: staging tiles with ragged edges on both in-plane axes
+             "n36": I.Geometry(nx=36, ny=36, nz=14, hx=1.5, hy=1.5, hz=2.0, nu=64, nv=24, du=1.3, dv=1.6, sad=600.0, sdd=900.0,
+                               n_proj=8),
              "config1": GEOMS["config1"], "aniso": GEOMS["aniso"], "wide8": GEOMS["wide8"]}
     for name, g in cases.items():
         f = I.uniform_volume(g, 23)
